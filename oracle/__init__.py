@@ -1,0 +1,107 @@
+"""CPU oracle for the el-ph Wannier->Bloch |g|^2 hot path -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+``--impl reference`` legs may import this package.  It shares no code with the
+CUDA path (paper_2111_14999_b200/csrc, binding) and neither imports the other.
+
+``oracle.direct / setk / setk_slab / qbatch`` are thin ctypes wrappers around
+oracle_elph.c (plain C99; see its header for the paper passages it follows).
+``oracle.oracle_einsum`` is the independent NumPy twin (pin P11).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(_build.build())
+        _lib.oracle_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _c(a, dtype, shape=None):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if shape is not None:
+        assert a.shape == tuple(shape), (a.shape, tuple(shape))
+    return a
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def direct(gW, Re, Rp, deg_e, deg_p, k, Uk, q, Ukq, ev, omega):
+    """Plain double sum over (Re,Rp), Eq. 13 + Eq. 7.  Returns out[nq][nb1][nb2][nm]."""
+    nRp, nRe, nw, _, nm = gW.shape
+    nb1 = Uk.shape[1]
+    nq, _, nb2 = Ukq.shape
+    gW = _c(gW, np.complex128); Re = _c(Re, np.float64, (nRe, 3)); Rp = _c(Rp, np.float64, (nRp, 3))
+    deg_e = None if deg_e is None else _c(deg_e, np.float64, (nRe,))
+    deg_p = None if deg_p is None else _c(deg_p, np.float64, (nRp,))
+    k = _c(k, np.float64, (3,)); Uk = _c(Uk, np.complex128, (nw, nb1))
+    q = _c(q, np.float64, (nq, 3)); Ukq = _c(Ukq, np.complex128, (nq, nw, nb2))
+    ev = _c(ev, np.complex128, (nq, nm, nm)); omega = _c(omega, np.float64, (nq, nm))
+    out = np.empty((nq, nb1, nb2, nm), dtype=np.float64)
+    rc = _load().oracle_direct(nRe, nRp, nw, nm, nb1, nb2, nq, _p(gW), _p(Re), _p(Rp), _p(deg_e),
+                               _p(deg_p), _p(k), _p(Uk), _p(q), _p(Ukq), _p(ev), _p(omega), _p(out))
+    assert rc == 0
+    return out
+
+
+def setk_slab(gW_p, Re, deg_e, k, Uk):
+    """Eq. 71 for one phonon lattice vector: g1_p[nb1][nw][nm]."""
+    nRe, nw, _, nm = gW_p.shape
+    nb1 = Uk.shape[1]
+    gW_p = _c(gW_p, np.complex128); Re = _c(Re, np.float64, (nRe, 3))
+    deg_e = None if deg_e is None else _c(deg_e, np.float64, (nRe,))
+    k = _c(k, np.float64, (3,)); Uk = _c(Uk, np.complex128, (nw, nb1))
+    g1 = np.empty((nb1, nw, nm), dtype=np.complex128)
+    rc = _load().oracle_setk_slab(nRe, nw, nm, nb1, _p(gW_p), _p(Re), _p(deg_e), _p(k), _p(Uk), _p(g1))
+    assert rc == 0
+    return g1
+
+
+def setk(gW, Re, deg_e, k, Uk):
+    """Eq. 71 (steps a1+a2): g1[nRp][nb1][nw][nm]."""
+    nRp, nRe, nw, _, nm = gW.shape
+    nb1 = Uk.shape[1]
+    gW = _c(gW, np.complex128); Re = _c(Re, np.float64, (nRe, 3))
+    deg_e = None if deg_e is None else _c(deg_e, np.float64, (nRe,))
+    k = _c(k, np.float64, (3,)); Uk = _c(Uk, np.complex128, (nw, nb1))
+    g1 = np.empty((nRp, nb1, nw, nm), dtype=np.complex128)
+    rc = _load().oracle_setk(nRe, nRp, nw, nm, nb1, _p(gW), _p(Re), _p(deg_e), _p(k), _p(Uk), _p(g1))
+    assert rc == 0
+    return g1
+
+
+def qbatch(g1, Rp, deg_p, q, Ukq, ev, omega):
+    """Rest of Eq. 70 + Eq. 7 (steps a3..a7): out[nq][nb1][nb2][nm]."""
+    nRp, nb1, nw, nm = g1.shape
+    nq, _, nb2 = Ukq.shape
+    g1 = _c(g1, np.complex128); Rp = _c(Rp, np.float64, (nRp, 3))
+    deg_p = None if deg_p is None else _c(deg_p, np.float64, (nRp,))
+    q = _c(q, np.float64, (nq, 3)); Ukq = _c(Ukq, np.complex128, (nq, nw, nb2))
+    ev = _c(ev, np.complex128, (nq, nm, nm)); omega = _c(omega, np.float64, (nq, nm))
+    out = np.empty((nq, nb1, nb2, nm), dtype=np.float64)
+    rc = _load().oracle_qbatch(nRp, nw, nm, nb1, nb2, nq, _p(g1), _p(Rp), _p(deg_p), _p(q), _p(Ukq),
+                               _p(ev), _p(omega), _p(out))
+    assert rc == 0
+    return out
+
+
+def elph(gW, Re, Rp, deg_e, deg_p, k, Uk, q, Ukq, ev, omega):
+    """setk followed by qbatch (the factorised two-step form, Eq. 71 then Eq. 70)."""
+    return qbatch(setk(gW, Re, deg_e, k, Uk), Rp, deg_p, q, Ukq, ev, omega)

@@ -1,0 +1,209 @@
+/*
+ * oracle_elph.c -- CPU ORACLE for the el-ph Wannier->Bloch |g|^2 hot path.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call this.  It shares
+ * no code, header, table or helper with the CUDA path under
+ * paper_2111_14999_b200/csrc and neither side includes the other.
+ *
+ * Plain, slow, obviously-correct C99 (double complex, nested loops), written
+ * from /root/reference/PAPER.md:
+ *
+ *   Eq. 13  g0(k,q) = sum_{Re,Rp} e^{ik.Re + iq.Rp}
+ *                                      U_{k+q} g0(Re,Rp) U_k^dagger z_q
+ *   Eq. 7   g = (1/(2 m omega_{q nu}))^{1/2} g0 ;  b <-> k (ket),
+ *                           b' <-> k+q (bra)
+ *   Eq. 11  columns of U_k are the eigenvectors
+ *   Eq. 70/71 (L564-L570)   the factorisation: fixed-k precompute (set_k),
+ *                           then completion per k' (q_batch)
+ *
+ * Readings of the garbled / silent points:
+ *   R1  phase = exp(+2*pi*i * k.R), k,q fractional (crystal) coords, L510
+ *   R2  every term divided by deg_e[e]*deg_p[p] (Wigner-Seitz weights)
+ *   R3  U_k plain on the k (ket) index, conj(U_kq) on the k+q (bra) index
+ *   R5  g_W[p][e][w1][w2][kappa]: w1 <-> k / U_k / b1,  w2 <-> k+q / U_kq / b2
+ *   R6  ev[q][kappa][nu] used unconjugated; masses folded into ev by the caller
+ *   R7  out = 0 where omega <= 0
+ *
+ * Definition computed (exact; the factorised form reaches the same number):
+ *
+ *   G(k,q)[b1][b2][nu] = sum_e sum_p (e^{2 pi i k.Re_e}/deg_e[e]) (e^{2 pi i q.Rp_p}/deg_p[p])
+ *        sum_{w1,w2,kappa} U_k[w1][b1] conj(U_kq[w2][b2]) ev[kappa][nu] g_W[p][e][w1][w2][kappa]
+ *   out[q][b1][b2][nu] = |G|^2 / (2 omega[q][nu])
+ *
+ * Layouts: all arrays C-order; complex = (re, im) pairs of doubles.
+ *   g_W [nRp][nRe][nw][nw][nm]   Re [nRe][3]  Rp [nRp][3]  deg_e [nRe]  deg_p [nRp]
+ *   U_k [nw][nb1]   U_kq [nq][nw][nb2]   ev [nq][nm][nm]   omega [nq][nm]
+ *   g1  [nRp][nb1][nw][nm]      out [nq][nb1][nb2][nm] (double)
+ *
+ * Parity pins: tests/test_oracle_pins.py (P1..P12 of SURVEY 8(c)); nothing
+ * here is "parity unpinned".
+ */
+#include <complex.h>
+#include <math.h>
+#include <stddef.h>
+#include <stdlib.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+
+static const double ORACLE_PI = 3.14159265358979323846264338327950288;
+
+/* e^{2 pi i k.R}: the integer part of x = k.R is dropped first (exact
+ * subtraction; e^{2 pi i n} = 1), then cos/sin of 2*pi*frac.  Reading R1. */
+static cplx oracle_phase(const double *k, const double *R)
+{
+    double x = k[0] * R[0] + k[1] * R[1] + k[2] * R[2];
+    x -= round(x);
+    return cos(2.0 * ORACLE_PI * x) + I * sin(2.0 * ORACLE_PI * x);
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------
+ * oracle_direct: Eq. 13 + Eq. 7 written out as the plain double sum over
+ * (Re, Rp) with all three rotations inside -- nothing factorised, nothing
+ * precomputed.  Accumulates in long double.  Tiny inputs only.
+ * ---------------------------------------------------------------------- */
+int oracle_direct(int nRe, int nRp, int nw, int nm, int nb1, int nb2, int nq,
+                  const cplx *gW, const double *Re, const double *Rp,
+                  const double *deg_e, const double *deg_p,
+                  const double *k, const cplx *Uk,
+                  const double *q, const cplx *Ukq, const cplx *ev,
+                  const double *omega, double *out)
+{
+    for (int iq = 0; iq < nq; ++iq)
+        for (int b1 = 0; b1 < nb1; ++b1)
+            for (int b2 = 0; b2 < nb2; ++b2)
+                for (int nu = 0; nu < nm; ++nu) {
+                    long double complex G = 0.0L;
+                    for (int e = 0; e < nRe; ++e) {
+                        cplx phe = oracle_phase(k, Re + 3 * e) / (deg_e ? deg_e[e] : 1.0);
+                        for (int p = 0; p < nRp; ++p) {
+                            cplx php = oracle_phase(q + 3 * iq, Rp + 3 * p) / (deg_p ? deg_p[p] : 1.0);
+                            long double complex s = 0.0L;
+                            for (int w1 = 0; w1 < nw; ++w1)
+                                for (int w2 = 0; w2 < nw; ++w2)
+                                    for (int ka = 0; ka < nm; ++ka) {
+                                        cplx g = gW[((((size_t)p * nRe + e) * nw + w1) * nw + w2) * nm + ka];
+                                        cplx u1 = Uk[(size_t)w1 * nb1 + b1];
+                                        cplx u2 = conj(Ukq[((size_t)iq * nw + w2) * nb2 + b2]);
+                                        cplx z = ev[((size_t)iq * nm + ka) * nm + nu];
+                                        s += (long double complex)(u1 * u2) * (long double complex)(z * g);
+                                    }
+                            G += (long double complex)(phe * php) * s;
+                        }
+                    }
+                    double w = omega[(size_t)iq * nm + nu];
+                    long double m2 = creall(G) * creall(G) + cimagl(G) * cimagl(G);
+                    out[(((size_t)iq * nb1 + b1) * nb2 + b2) * nm + nu] =
+                        (w > 0.0) ? (double)(m2 / (2.0L * (long double)w)) : 0.0;
+                }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------
+ * oracle_setk_slab: Eq. 71 for ONE phonon lattice vector p (steps a1, a2).
+ *   T[w1][w2][ka]   = sum_e (e^{2 pi i k.Re_e}/deg_e[e]) gW_p[e][w1][w2][ka]
+ *   g1_p[b1][w2][ka] = sum_{w1} U_k[w1][b1] T[w1][w2][ka]
+ * gW_p is the slab [nRe][nw][nw][nm]; g1_p is [nb1][nw][nm].
+ * ---------------------------------------------------------------------- */
+int oracle_setk_slab(int nRe, int nw, int nm, int nb1,
+                     const cplx *gW_p, const double *Re, const double *deg_e,
+                     const double *k, const cplx *Uk, cplx *g1_p)
+{
+    size_t X = (size_t)nw * nw * nm;
+    cplx *T = (cplx *)calloc(X, sizeof(cplx));
+    if (!T) return -1;
+    for (int e = 0; e < nRe; ++e) {
+        cplx ph = oracle_phase(k, Re + 3 * e) / (deg_e ? deg_e[e] : 1.0);
+        const cplx *g = gW_p + (size_t)e * X;
+        for (size_t x = 0; x < X; ++x) T[x] += ph * g[x];
+    }
+    for (int b1 = 0; b1 < nb1; ++b1)
+        for (int w2 = 0; w2 < nw; ++w2)
+            for (int ka = 0; ka < nm; ++ka) {
+                cplx s = 0.0;
+                for (int w1 = 0; w1 < nw; ++w1)
+                    s += Uk[(size_t)w1 * nb1 + b1] * T[((size_t)w1 * nw + w2) * nm + ka];
+                g1_p[((size_t)b1 * nw + w2) * nm + ka] = s;
+            }
+    free(T);
+    return 0;
+}
+
+/* oracle_setk: Eq. 71 for all p (g_W fully resident on the host). */
+int oracle_setk(int nRe, int nRp, int nw, int nm, int nb1,
+                const cplx *gW, const double *Re, const double *deg_e,
+                const double *k, const cplx *Uk, cplx *g1)
+{
+    size_t slab = (size_t)nRe * nw * nw * nm, N = (size_t)nb1 * nw * nm;
+    int rc = 0;
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < nRp; ++p) {
+        int r = oracle_setk_slab(nRe, nw, nm, nb1, gW + (size_t)p * slab, Re, deg_e, k, Uk,
+                                 g1 + (size_t)p * N);
+        if (r) rc = r;
+    }
+    return rc;
+}
+
+/* ------------------------------------------------------------------------
+ * oracle_qbatch: the rest of Eq. 70 + Eq. 7 (steps a3..a7), one q at a time.
+ *   C[b1][w2][ka]  = sum_p (e^{2 pi i q.Rp_p}/deg_p[p]) g1[p][b1][w2][ka]
+ *   D[b1][b2][ka]  = sum_{w2} conj(U_kq[w2][b2]) C[b1][w2][ka]
+ *   E[b1][b2][nu]  = sum_{ka} D[b1][b2][ka] ev[ka][nu]
+ *   out            = |E|^2 / (2 omega[nu])          (0 where omega <= 0)
+ * OpenMP over q only (used when the oracle is timed as the CPU baseline).
+ * ---------------------------------------------------------------------- */
+int oracle_qbatch(int nRp, int nw, int nm, int nb1, int nb2, int nq,
+                  const cplx *g1, const double *Rp, const double *deg_p,
+                  const double *q, const cplx *Ukq, const cplx *ev,
+                  const double *omega, double *out)
+{
+    size_t N = (size_t)nb1 * nw * nm;
+    int rc = 0;
+#pragma omp parallel for schedule(static)
+    for (int iq = 0; iq < nq; ++iq) {
+        cplx *C = (cplx *)calloc(N, sizeof(cplx));
+        cplx *D = (cplx *)malloc((size_t)nb1 * nb2 * nm * sizeof(cplx));
+        if (!C || !D) { rc = -1; free(C); free(D); continue; }
+        for (int p = 0; p < nRp; ++p) {
+            cplx ph = oracle_phase(q + 3 * iq, Rp + 3 * p) / (deg_p ? deg_p[p] : 1.0);
+            const cplx *g = g1 + (size_t)p * N;
+            for (size_t n = 0; n < N; ++n) C[n] += ph * g[n];
+        }
+        const cplx *U = Ukq + (size_t)iq * nw * nb2;
+        const cplx *Z = ev + (size_t)iq * nm * nm;
+        for (int b1 = 0; b1 < nb1; ++b1)
+            for (int b2 = 0; b2 < nb2; ++b2)
+                for (int ka = 0; ka < nm; ++ka) {
+                    cplx s = 0.0;
+                    for (int w2 = 0; w2 < nw; ++w2)
+                        s += conj(U[(size_t)w2 * nb2 + b2]) * C[((size_t)b1 * nw + w2) * nm + ka];
+                    D[((size_t)b1 * nb2 + b2) * nm + ka] = s;
+                }
+        for (int b1 = 0; b1 < nb1; ++b1)
+            for (int b2 = 0; b2 < nb2; ++b2)
+                for (int nu = 0; nu < nm; ++nu) {
+                    cplx s = 0.0;
+                    for (int ka = 0; ka < nm; ++ka)
+                        s += D[((size_t)b1 * nb2 + b2) * nm + ka] * Z[(size_t)ka * nm + nu];
+                    double w = omega[(size_t)iq * nm + nu];
+                    double m2 = creal(s) * creal(s) + cimag(s) * cimag(s);
+                    out[(((size_t)iq * nb1 + b1) * nb2 + b2) * nm + nu] = (w > 0.0) ? m2 / (2.0 * w) : 0.0;
+                }
+        free(C);
+        free(D);
+    }
+    return rc;
+}
