@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the el-ph Wannier->Bloch |g|^2 hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (set_k + q_batch for every k of the
+workload: SURVEY.md 8(a) rows a1..a7) over one batch of seeded synthetic input.
+Prints ONE JSON line.  `--impl reference` times the
+CPU oracle (oracle/, as it stands) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2111_14999_b200 import workloads as wl  # noqa: E402
+
+METRIC = "interpolated el-ph (k,q) pairs/sec"
+UNIT = "pairs/s"
+DEFAULT_WORKLOAD = "4-atom"
+
+# FP64 "alu" peak derived from unit counts and clocks:
+# 64 FP64 FMA / clk / SM  x 2 flop x 148 SMs x 1.965 GHz (clocks.max.sm)
+FP64_PEAK_TFLOPS = 64 * 2 * 148 * 1.965e9 / 1e12
+HBM_FALLBACK_GBS = 6650.0
+
+
+# ----------------------------------------------------------------------------- utilities
+def _measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        try:
+            rows = [r.strip().split(",") for r in open(self.path) if r.strip()]
+            os.unlink(self.path)
+            sm = [float(r[0]) for r in rows if len(r) >= 7]
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            reasons = set()
+            for r in rows:
+                if len(r) >= 7:
+                    for nme, v in zip(names, r[3:7]):
+                        if v.strip().lower() == "active":
+                            reasons.add(nme)
+            if sm:
+                out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(rows[0][1]), reasons=sorted(reasons),
+                           samples=len(sm), power_w_max=max(float(r[2]) for r in rows if len(r) >= 7))
+        except Exception:
+            pass
+        return out
+
+
+def _dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def shard_k(nk: int, rank: int, world: int, scaling: str = "weak"):
+    """k-point indices a rank processes.  (k,q) pairs are independent, so the
+    path shards over k with no data-path collective.  weak: every rank runs nk k-points of its
+    own (indices rank*nk ..); strong: the nk k-points are dealt round-robin."""
+    if scaling == "weak":
+        return list(range(rank * nk, (rank + 1) * nk))
+    return list(range(rank, nk, world))
+
+
+def _k_inputs(w, ik):
+    """Inputs of k-point index ik; indices beyond the workload's own nk (other ranks' shards under weak
+    scaling) reuse the recipe with a fresh seed index."""
+    nk = w.nk
+    ks = wl.k_points(w)
+    k = ks[ik % nk] if ik < nk else np.random.default_rng([w.seed, w.cfg_id, 1, ik]).random(3)
+    return k, wl.U_k(w, ik), wl.q_inputs(w, ik)
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+def time_oracle(w, budget_s: float = 20.0):
+    """The oracle as it stands, timed on the host cores on a bounded sample of workload w.
+    Returns (pairs_per_s, cores, sample_description).  set_k is timed on a subset of the Rp slabs and
+    scaled by nRp/slabs (it is a plain sum over independent slabs); q_batch is timed on a subset of the
+    q list against a g1' of the right shape, and scaled by nq/sample."""
+    import oracle
+    cores = oracle.num_threads()
+    Re, Rp = wl.Re_vectors(w), wl.Rp_vectors(w)
+    k, Uk = wl.k_points(w)[0], wl.U_k(w, 0)
+    slab_flop = 8.0 * w.nRe * w.X
+    # assume >= 0.3 GFLOP/s/core for sizing; the measured time is what is reported
+    n_slab = int(max(cores, min(w.nRp, (0.3 * budget_s * 0.3e9 * cores) / slab_flop)))
+    n_slab = max(1, min(w.nRp, n_slab, int(2e9 // (16 * w.nRe * w.X))))      # <= 2 GB of g_W on the host
+    slabs = np.empty((n_slab, w.nRe, w.nw, w.nw, w.nm), dtype=np.complex128)
+    import concurrent.futures as cf
+    with cf.ThreadPoolExecutor(min(16, os.cpu_count() or 4)) as pool:
+        list(pool.map(lambda p: wl.gW_slab(w, p, slabs[p]), range(n_slab)))
+    t0 = time.perf_counter()
+    g1_part = oracle.setk(slabs, Re, None, k, Uk)
+    t_setk = (time.perf_counter() - t0) * (w.nRp / n_slab)
+    # q part: g1' of the right shape (values are irrelevant for timing): tile what set_k produced
+    reps = -(-w.nRp // n_slab)
+    g1 = np.ascontiguousarray(np.concatenate([g1_part] * reps)[: w.nRp])
+    q_flop = 8.0 * w.nRp * w.N + 8.0 * w.nb1 * w.nb2 * w.nm * (w.nw + w.nm)
+    nq_s = int(max(cores, min(w.nq, (0.7 * budget_s * 0.4e9 * cores) / q_flop)))
+    nq_s = min(w.nq, nq_s)
+    q, Ukq, ev, om = wl.q_inputs(w, 0)
+    idx = wl.sample_indices(w.nq, nq_s)
+    qa, Ua, ea, oa = q[idx], np.ascontiguousarray(Ukq[idx]), np.ascontiguousarray(ev[idx]), om[idx]
+    t0 = time.perf_counter()
+    oracle.qbatch(g1, Rp, None, qa, Ua, ea, oa)
+    t_q = (time.perf_counter() - t0) * (w.nq / nq_s)
+    pairs_per_s = w.nq / (t_setk + t_q)
+    sample = (f"1 k-point of {w.nk}: set_k on {n_slab}/{w.nRp} Rp slabs (scaled x{w.nRp / n_slab:.2f}), "
+              f"q_batch on {nq_s}/{w.nq} q (scaled x{w.nq / nq_s:.2f}); gcc -O2 -fopenmp, {cores} threads")
+    return pairs_per_s, cores, sample, (t_setk, t_q)
+
+
+def run_reference(args):
+    rank, world, _ = _dist_env()
+    if rank != 0:
+        return
+    w = wl.CONFIGS[args.workload]
+    vals = []
+    sample = ""
+    cores = 0
+    budget = max(2.0, min(20.0, 90.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        v, cores, sample, _ = time_oracle(w, budget)
+        if i >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    ms_per_step = 1e3 * (w.nk * w.nq) / value
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": _config_dict(w, args.gpus),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def _config_dict(w, n_gpus):
+    return {"workload": w.name, "nw": w.nw, "nb1": w.nb1, "nb2": w.nb2, "nmodes": w.nm, "nRe": w.nRe, "nRp": w.nRp,
+            "nk": w.nk, "nq_per_k": w.nq, "gW_GB": round(w.gW_bytes / 1e9, 3),
+            "cache": "inputs larger than L2 (g_W is streamed from HBM every step)",
+            "parallelism": f"k-sharded x{n_gpus}, g_W replicated, no collective"}
+
+
+# ----------------------------------------------------------------------------- GPU leg
+def run_ours(args):
+    import torch
+    from paper_2111_14999_b200 import binding, build, harness
+
+    rank, world, local = _dist_env()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if rank == 0:
+        build.build()
+    if dist is not None:
+        dist.barrier()
+    binding.load_library()
+
+    w = wl.CONFIGS[args.workload]
+    t_gen = time.perf_counter()
+    gW = harness.upload_gW(w, dev)
+    k_ids = shard_k(w.nk, rank, world, "weak")
+    host_inputs = [_k_inputs(w, ik) for ik in k_ids]
+    dev_inputs = []
+    for k, Uk, (q, Ukq, ev, om) in host_inputs:
+        dev_inputs.append((k, harness.to_device([Uk], dev)[0], harness.to_device([q, Ukq, ev, om], dev)))
+    t_gen = time.perf_counter() - t_gen
+    ctx = harness.make_context(w, gW)
+    out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+
+    def step():
+        for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
+            ctx.set_k(k, Uk_d)
+            ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def maxreduce(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident timing ------------------------------------------------
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = sum(ctx.launch_counts().values())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = maxreduce(e0.elapsed_time(e1))
+    clocks = sampler.stop() if rank == 0 else {}
+    gpu_launches = sum(ctx.launch_counts().values()) - launches0
+    pairs_per_step_all = world * w.nk * w.nq
+    value = pairs_per_step_all * args.steps / (ms_total * 1e-3)
+
+    # ---- per-kernel durations (CUDA events inside the library, on its stream) ---
+    ctx.profile(True)
+    prof_steps = max(1, min(args.steps, 3))
+    for _ in range(prof_steps):
+        step()
+    prof = ctx.profile_read()
+    ctx.profile(False)
+    counts = harness.algorithmic_counts(w)
+    peaks, peak_src = _measured_peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
+    kernels = {}
+    for kind, (ms, n) in prof.items():
+        if n == 0:
+            continue
+        kernels[kind] = {"ms_total": ms / prof_steps, "launches_per_step": n // prof_steps, "avg_ms": ms / n}
+    n_k = len(dev_inputs)
+    # algorithmic work per LAUNCH of each kernel
+    per_launch = {
+        "setk_stream": ("hbm", counts["setk_stream_bytes"]),
+        "contract": ("alu", counts["contract_flop"] * n_k / max(1, kernels.get("contract", {}).get("launches_per_step", 1))),
+        "rotate_epilogue": ("alu", counts["rotate_flop"] * n_k / max(1, kernels.get("rotate_epilogue", {}).get("launches_per_step", 1))),
+    }
+    for kind, (bound, work) in per_launch.items():
+        if kind in kernels:
+            dur = kernels[kind]["avg_ms"] * 1e-3
+            if bound == "hbm":
+                kernels[kind].update(bound="hbm", achieved=work / dur / 1e9, peak=hbm_peak, unit="GB/s")
+            else:
+                kernels[kind].update(bound="alu", achieved=work / dur / 1e12, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s")
+            kernels[kind]["frac"] = kernels[kind]["achieved"] / kernels[kind]["peak"]
+    dominant = max(kernels, key=lambda kk: kernels[kk]["ms_total"])
+    dk = kernels[dominant]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(w.name, {}).get(dominant)
+        except Exception:
+            traffic = None
+    roofline = {"kernel": dominant, "bound": dk.get("bound"), "achieved": dk.get("achieved"), "peak": dk.get("peak"),
+                "unit": dk.get("unit"), "frac": dk.get("frac"), "traffic": traffic,
+                "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % peak_src) if dk.get("bound") == "hbm"
+                else "derived: 64 FP64 FMA/clk/SM x 148 SMs x 1.965 GHz x 2 = 37.24 TFLOP/s",
+                "share_of_step": dk["ms_total"] / sum(v["ms_total"] for v in kernels.values())}
+    fp64_probe = None
+    if rank == 0:
+        try:
+            fp64_probe = {"dmma_tflops": binding.probe_fp64("dmma", 4000), "dfma_tflops": binding.probe_fp64("dfma", 4000)}
+        except Exception:
+            fp64_probe = None
+
+    # ---- end to end: host buffers through the C ABI, copies inside the timed region ----
+    pinned = []
+    for k, Uk, (q, Ukq, ev, om) in host_inputs:
+        pin = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (Uk, q, Ukq, ev, om)]
+        pinned.append((k, pin))
+    out_host = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory()
+    h2d = sum(sum(t.numel() * t.element_size() for t in pin) + 24 for _, pin in pinned)
+    d2h = len(pinned) * out_host.numel() * 8
+
+    def step_e2e():
+        for k, (Uk_p, q_p, Ukq_p, ev_p, om_p) in pinned:
+            ctx.set_k_host(k, Uk_p.numpy())
+            ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
+
+    e2e_steps = max(1, min(args.steps, 3))
+    step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(e2e_steps):
+        step_e2e()
+    e1.record()
+    barrier()
+    ms_e2e = maxreduce(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3))
+    e2e_value = pairs_per_step_all * e2e_steps / (ms_e2e * 1e-3)
+
+    # ---- CPU baseline: the oracle on the host cores (rank 0, N=1 only) ----------
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, cores, sample, _ = time_oracle(w, 20.0)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": _config_dict(w, world),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "steps": e2e_steps},
+            "gpu_launches": int(gpu_launches),
+            "roofline": roofline,
+            "kernels": kernels,
+            "fp64_probe": fp64_probe,
+            "cpu_baseline": cpu_baseline,
+            "fp64_tflops_whole_path": (counts["setk_flop"] + counts["contract_flop"] + counts["rotate_flop"]) * w.nk * world
+            * args.steps / (ms_total * 1e-3) / 1e12,
+            "input_gen_s": round(t_gen, 1),
+        }
+        print(json.dumps(line))
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(wl.CONFIGS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

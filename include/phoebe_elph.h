@@ -1,0 +1,174 @@
+/*
+ * phoebe_elph.h -- C ABI of the B200-native el-ph Wannier->Bloch |g|^2 hot path.
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, the Phoebe
+ * paper, arXiv 2111.14999):
+ *
+ *   Eq. 13 (L133)  g0(k,q) = sum_{Re,Rp} e^{ik.Re + iq.Rp} U_{k+q} g0(Re,Rp) U_k^dagger z_q
+ *   Eq. 7  (L98)   g = (1 / (2 m omega_{q nu}))^{1/2} g0
+ *   Eq. 70-71 (L564-L570)  the factorisation: a fixed-k precompute, then the
+ *                  completion for a set {k'} batched on the GPU (L576)
+ *
+ * in the reading fixed by SURVEY.md 8(c) / DESIGN.md "Readings":
+ *
+ *   out[q][b1][b2][nu] = | sum_{e,p} (e^{2 pi i k.Re_e}/deg_e[e]) (e^{2 pi i q.Rp_p}/deg_p[p])
+ *                           sum_{w1,w2,kappa} U_k[w1][b1] conj(U_kq[q][w2][b2]) ev[q][kappa][nu]
+ *                           g_W[p][e][w1][w2][kappa] |^2  /  (2 omega[q][nu])        (0 where omega <= 0)
+ *
+ * Conventions
+ *   - every array is C-order (last index fastest); complex128 = (re, im) pair
+ *     of doubles, 16-byte aligned; wavevectors and lattice vectors are in
+ *     crystal (fractional) coordinates (L510), hence the explicit 2 pi.
+ *   - "DEVICE" pointers are CUDA device pointers on the current device,
+ *     "HOST" pointers are ordinary host memory.  BORROWED = the caller keeps
+ *     ownership and must keep the memory valid until the stream given at
+ *     setup has finished the work of the call that used it.
+ *   - every call only enqueues work on that stream and returns (no implicit
+ *     device synchronisation) unless its comment says otherwise.
+ *   - return value: 0 = OK, negative = error (see PHOEBE_ELPH_E_*).  The
+ *     library never aborts, throws or prints.  There is no CPU fallback: on a
+ *     machine without a CUDA device every compute call fails with
+ *     PHOEBE_ELPH_E_CUDA.
+ */
+#ifndef PHOEBE_ELPH_H
+#define PHOEBE_ELPH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PHOEBE_ELPH_OK            0
+#define PHOEBE_ELPH_E_NULL       -1   /* a required pointer is NULL                        */
+#define PHOEBE_ELPH_E_DIMS       -2   /* a dimension is <= 0 or exceeds its declared max   */
+#define PHOEBE_ELPH_E_ALIGN      -3   /* a complex / workspace pointer is not 16-B aligned */
+#define PHOEBE_ELPH_E_NO_K       -4   /* q_batch called before any set_k                   */
+#define PHOEBE_ELPH_E_WORKSPACE  -5   /* workspace too small for these dims                */
+#define PHOEBE_ELPH_E_CUDA       -6   /* CUDA error; text via phoebe_elph_last_error       */
+
+typedef struct phoebe_elph_ctx phoebe_elph_ctx;     /* opaque, library-owned */
+
+/* Problem sizes (paper's notation):
+ * nRe/nRp electron/phonon lattice vectors, nw Wannier functions, nmodes = 3*atoms,
+ * nb1_max/nb2_max = most bands ever kept at k / at k+q (<= nw), nq_max = most
+ * q-points ever passed to one q_batch call. */
+typedef struct {
+    int32_t nRe, nRp, nw, nmodes, nb1_max, nb2_max, nq_max;
+} phoebe_elph_dims;
+
+/* Kernel kinds, for launch counts and profiling. */
+enum {
+    PHOEBE_ELPH_K_SETK_STREAM = 0,  /* a1: Fourier sum over Re (streams g_W once)         */
+    PHOEBE_ELPH_K_SETK_ROTATE = 1,  /* a2: rotation by U_k -> g1'                          */
+    PHOEBE_ELPH_K_QPHASE      = 2,  /* a3: phases e^{2 pi i q.Rp}/deg_p                    */
+    PHOEBE_ELPH_K_CONTRACT    = 3,  /* a4: Rp contraction (complex FP64 GEMM, DMMA)        */
+    PHOEBE_ELPH_K_ROTATE_EPI  = 4,  /* a5-a7: U_kq^dagger, phonon rotation, |.|^2/(2 omega) */
+    PHOEBE_ELPH_K_COUNT       = 5
+};
+
+/* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
+ * that most of the on-board GPU's memory is used").
+ * In : dims (dims->nq_max may be 0 = "as many as fit"), hbm_budget_bytes = device
+ *      bytes the caller can give to the workspace (g_W itself excluded).
+ * Out: *nq_batch_out = largest q-batch that fits (<= dims->nq_max when that is > 0),
+ *      *bytes_out    = workspace bytes needed for that batch size.
+ * Errors: E_NULL, E_DIMS, E_WORKSPACE (budget too small for even one tile of q). */
+int phoebe_elph_workspace_bytes(const phoebe_elph_dims* dims, size_t hbm_budget_bytes,
+                                size_t* bytes_out, int32_t* nq_batch_out);
+
+/* Step a0.  Creates a context bound to one device stream.
+ *   gW_dev      DEVICE, BORROWED for the life of ctx, complex128 [nRp][nRe][nw][nw][nmodes]
+ *               (first Wannier index <-> k / U_k, second <-> k+q / U_kq; Eq. 13).
+ *               Never copied or re-laid-out (57.8 GB in the largest workload).
+ *   Re_host     HOST [nRe][3], Rp_host HOST [nRp][3]: lattice vectors, crystal coords; copied.
+ *   deg_e_host  HOST [nRe], deg_p_host HOST [nRp]: Wigner-Seitz degeneracies (> 0), each
+ *               Fourier term is divided by them; NULL = all 1; copied.
+ *   dims->nq_max must be > 0 here.
+ *   workspace_dev DEVICE, BORROWED for the life of ctx, >= phoebe_elph_workspace_bytes(), 256-B aligned.
+ *   cuda_stream a cudaStream_t (NULL = default stream).
+ * Synchronises the stream once (the small copies use pageable host memory).
+ * Errors: E_NULL, E_DIMS, E_ALIGN, E_WORKSPACE, E_CUDA. */
+int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev,
+                      const double* Re_host, const double* Rp_host,
+                      const double* deg_e_host, const double* deg_p_host,
+                      const phoebe_elph_dims* dims,
+                      void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Steps a1 + a2, Eq. 71 (L570):
+ *   g1'[p][b1][w2][kappa] = sum_{w1} U_k[w1][b1] sum_e (e^{2 pi i k.Re_e}/deg_e[e]) g_W[p][e][w1][w2][kappa]
+ * kept inside the context for the following q_batch calls.
+ *   k_host  HOST [3] (read before returning);  Uk_dev DEVICE complex128 [nw][nb1], columns = eigenvectors
+ *   (Eq. 11), 1 <= nb1 <= nb1_max; nb1 may change from call to call (band windows, L540).
+ * Errors: E_NULL, E_DIMS, E_ALIGN, E_CUDA. */
+int phoebe_elph_set_k(phoebe_elph_ctx* ctx, const double* k_host, const void* Uk_dev, int32_t nb1);
+
+/* Same, U_k in HOST memory (copied to the device on the stream; the host buffer
+ * may be reused when the call returns only if it is pageable -- for pinned memory
+ * keep it valid until the stream has passed the copy). */
+int phoebe_elph_set_k_host(phoebe_elph_ctx* ctx, const double* k_host, const void* Uk_host, int32_t nb1);
+
+/* Steps a3..a7, rest of Eq. 70 + Eq. 7, for nq q-points at the k of the last set_k:
+ *   C[q][b1][w2][kappa] = sum_p (e^{2 pi i q.Rp_p}/deg_p[p]) g1'[p][b1][w2][kappa]
+ *   D[q][b1][b2][kappa] = sum_{w2} conj(U_kq[q][w2][b2]) C[q][b1][w2][kappa]
+ *   E[q][b1][b2][nu]    = sum_kappa D[q][b1][b2][kappa] ev[q][kappa][nu]
+ *   out[q][b1][b2][nu]  = |E|^2 / (2 omega[q][nu])      (0 where omega <= 0)
+ *   q_dev DEVICE [nq][3]; Ukq_dev DEVICE complex128 [nq][nw][nb2]; ev_dev DEVICE complex128
+ *   [nq][nmodes][nmodes] (row kappa = 3*atom+cartesian, column nu = mode; used unconjugated, any
+ *   1/sqrt(mass) folded in by the caller); omega_dev DEVICE [nq][nmodes];
+ *   out_dev DEVICE double [nq][nb1][nb2][nmodes], written, caller-owned.
+ *   1 <= nq <= nq_max, 1 <= nb2 <= nb2_max (uniform within the batch).
+ * Errors: E_NULL, E_DIMS, E_ALIGN, E_NO_K, E_CUDA. */
+int phoebe_elph_q_batch(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                        const double* q_dev, const void* Ukq_dev, const void* ev_dev,
+                        const double* omega_dev, double* out_dev);
+
+/* Same with HOST buffers: copies the four inputs host->device into staging inside the
+ * workspace, runs the batch, copies out device->host, and SYNCHRONISES the stream before
+ * returning (so pageable buffers are safe).  This is the end-to-end call. */
+int phoebe_elph_q_batch_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                             const double* q_host, const void* Ukq_host, const void* ev_host,
+                             const double* omega_host, double* out_host);
+
+/* Copy the current g1' (complex128 [nRp][nb1][nw][nmodes]) to dst_dev (DEVICE, >= bytes
+ * nRp*nb1*nw*nmodes*16); for tests of set_k on its own.  Errors: E_NULL, E_NO_K, E_WORKSPACE, E_CUDA. */
+int phoebe_elph_copy_g1(phoebe_elph_ctx* ctx, void* dst_dev, size_t dst_bytes);
+
+/* Launch accounting: counts[PHOEBE_ELPH_K_COUNT] = kernels launched so far, per kind. */
+int phoebe_elph_launch_counts(const phoebe_elph_ctx* ctx, int64_t* counts);
+
+/* Per-kernel device timing.  profile(ctx, 1) starts recording a CUDA event pair around
+ * every kernel launch on the context's stream (a few microseconds of overhead per launch:
+ * do not time whole-job throughput with it on); profile_read synchronises the stream,
+ * returns accumulated milliseconds and launch counts per kind since the last read and
+ * clears them.  profile(ctx, 0) stops recording. */
+int phoebe_elph_profile(phoebe_elph_ctx* ctx, int32_t enable);
+int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches);
+
+/* Tuning knobs (integers); unknown key -> E_DIMS.  Keys:
+ *   "nq_sub"  q sub-batch kept L2-resident between the contraction and the rotation kernel
+ *   "s_split" number of Re chunks in the set_k stream (0 = automatic)                       */
+int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
+int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);
+
+int phoebe_elph_destroy(phoebe_elph_ctx* ctx);
+
+/* Text of the last error on this context ("" if none); valid until the next call on ctx. */
+const char* phoebe_elph_last_error(const phoebe_elph_ctx* ctx);
+
+/* FP64 ceiling probes used for the roofline denominators: runs a
+ * register-resident loop of dependent-free FP64 FMAs (kind 0: DFMA, kind 1: mma.sync
+ * m8n8k4 DMMA) on every SM for `iters` iterations and writes the achieved TFLOP/s.
+ * Synchronises the stream.  Errors: E_NULL, E_DIMS, E_CUDA. */
+int phoebe_elph_probe_fp64(int32_t kind, int32_t iters, void* cuda_stream, double* tflops_out);
+
+/* HBM read-stream probe: sums `bytes` of DEVICE memory with 128-bit loads; writes GB/s. */
+int phoebe_elph_probe_hbm_read(const void* buf_dev, size_t bytes, void* cuda_stream, double* gbs_out);
+
+const char* phoebe_elph_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PHOEBE_ELPH_H */

@@ -1,0 +1,252 @@
+"""Thin ctypes binding of include/phoebe_elph.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libphoebe_elph.so; PyTorch is
+used for device memory and streams only.  There is no CPU fallback: if the
+shared library is missing or no CUDA device is present, the calls raise.
+This module never imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_t, c_void_p
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libphoebe_elph.so")
+
+KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue"]
+
+#: every symbol declared in include/phoebe_elph.h
+EXPORTS = [
+    "phoebe_elph_workspace_bytes", "phoebe_elph_setup", "phoebe_elph_set_k", "phoebe_elph_set_k_host",
+    "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_copy_g1", "phoebe_elph_launch_counts",
+    "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
+    "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
+    "phoebe_elph_version",
+]
+
+ERRORS = {0: "OK", -1: "E_NULL", -2: "E_DIMS", -3: "E_ALIGN", -4: "E_NO_K", -5: "E_WORKSPACE", -6: "E_CUDA"}
+
+
+class Dims(ctypes.Structure):
+    _fields_ = [(n, c_int32) for n in ("nRe", "nRp", "nw", "nmodes", "nb1_max", "nb2_max", "nq_max")]
+
+
+class PhoebeElphError(RuntimeError):
+    def __init__(self, code, where, text=""):
+        self.code = code
+        super().__init__(f"{where}: {ERRORS.get(code, code)} {text}".strip())
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree C-ABI library; raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_2111_14999_b200.build` "
+                                "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.phoebe_elph_workspace_bytes.argtypes = [POINTER(Dims), c_size_t, POINTER(c_size_t), POINTER(c_int32)]
+    lib.phoebe_elph_setup.argtypes = [POINTER(c_void_p), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                                      POINTER(Dims), c_void_p, c_size_t, c_void_p]
+    lib.phoebe_elph_set_k.argtypes = [c_void_p, c_void_p, c_void_p, c_int32]
+    lib.phoebe_elph_set_k_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32]
+    lib.phoebe_elph_q_batch.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_q_batch_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.phoebe_elph_launch_counts.argtypes = [c_void_p, POINTER(c_int64)]
+    lib.phoebe_elph_profile.argtypes = [c_void_p, c_int32]
+    lib.phoebe_elph_profile_read.argtypes = [c_void_p, POINTER(c_double), POINTER(c_int64)]
+    lib.phoebe_elph_set_tuning.argtypes = [c_void_p, c_char_p, c_int64]
+    lib.phoebe_elph_get_tuning.argtypes = [c_void_p, c_char_p, POINTER(c_int64)]
+    lib.phoebe_elph_destroy.argtypes = [c_void_p]
+    lib.phoebe_elph_last_error.argtypes = [c_void_p]
+    lib.phoebe_elph_last_error.restype = c_char_p
+    lib.phoebe_elph_probe_fp64.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
+    lib.phoebe_elph_probe_hbm_read.argtypes = [c_void_p, c_size_t, c_void_p, POINTER(c_double)]
+    lib.phoebe_elph_version.restype = c_char_p
+    _lib = lib
+    return lib
+
+
+def version() -> str:
+    return load_library().phoebe_elph_version().decode()
+
+
+def workspace_bytes(dims: Dims, hbm_budget_bytes: int):
+    """-> (bytes, nq_batch).  Raises PhoebeElphError."""
+    nbytes, nqb = c_size_t(0), c_int32(0)
+    rc = load_library().phoebe_elph_workspace_bytes(byref(dims), hbm_budget_bytes, byref(nbytes), byref(nqb))
+    if rc:
+        raise PhoebeElphError(rc, "phoebe_elph_workspace_bytes")
+    return int(nbytes.value), int(nqb.value)
+
+
+def _host_ptr(a):
+    """pointer of a C-contiguous numpy array (or None)."""
+    if a is None:
+        return None
+    assert a.flags.c_contiguous
+    return a.ctypes.data
+
+
+class ElphContext:
+    """phoebe_elph_ctx with the same method names as the C ABI (set_k, q_batch, ...).
+
+    ``gW`` is a CUDA torch tensor (complex128 [nRp][nRe][nw][nw][nm]) that is
+    BORROWED; the workspace is allocated here with torch and kept alive with the
+    context.  Array arguments of the device entry points are CUDA torch tensors,
+    those of the ``*_host`` entry points are NumPy arrays (or pinned CPU tensors).
+    """
+
+    def __init__(self, gW, Re, Rp, deg_e=None, deg_p=None, *, nb1_max=None, nb2_max=None, nq_max,
+                 hbm_budget_bytes=None, stream=None):
+        import numpy as np
+        import torch
+
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise PhoebeElphError(-6, "ElphContext", "no CUDA device (there is no CPU fallback)")
+        assert gW.is_cuda and gW.dtype == torch.complex128 and gW.is_contiguous() and gW.dim() == 5
+        nRp, nRe, nw, nw2, nm = gW.shape
+        assert nw == nw2
+        self.dims = Dims(nRe, nRp, nw, nm, nb1_max or nw, nb2_max or nw, nq_max)
+        self._gW = gW
+        self._torch = torch
+        self.device = gW.device
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        if hbm_budget_bytes is None:
+            free, _total = torch.cuda.mem_get_info(self.device)
+            hbm_budget_bytes = int(free * 0.9)
+        nbytes, nqb = workspace_bytes(self.dims, hbm_budget_bytes)
+        if nqb < nq_max:
+            self.dims.nq_max = nqb
+        self.nq_batch = nqb
+        self.workspace_nbytes = nbytes
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ws_ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        Re = np.ascontiguousarray(Re, dtype=np.float64); Rp = np.ascontiguousarray(Rp, dtype=np.float64)
+        assert Re.shape == (nRe, 3) and Rp.shape == (nRp, 3)
+        deg_e = None if deg_e is None else np.ascontiguousarray(deg_e, dtype=np.float64)
+        deg_p = None if deg_p is None else np.ascontiguousarray(deg_p, dtype=np.float64)
+        ctx = c_void_p(0)
+        rc = self._lib.phoebe_elph_setup(byref(ctx), gW.data_ptr(), _host_ptr(Re), _host_ptr(Rp), _host_ptr(deg_e),
+                                         _host_ptr(deg_p), byref(self.dims), ws_ptr, nbytes, self.stream.cuda_stream)
+        if rc:
+            raise PhoebeElphError(rc, "phoebe_elph_setup")
+        self._ctx = ctx
+        self.nb1 = 0
+
+    # -- helpers -----------------------------------------------------------
+    def _check(self, rc, where):
+        if rc:
+            raise PhoebeElphError(rc, where, self._lib.phoebe_elph_last_error(self._ctx).decode())
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._lib.phoebe_elph_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C ABI, same names ----------------------------------------------
+    def set_k(self, k, Uk):
+        """k: 3 floats (host); Uk: CUDA complex128 tensor [nw][nb1]."""
+        import numpy as np
+        k = np.ascontiguousarray(k, dtype=np.float64)
+        assert k.shape == (3,) and Uk.is_cuda and Uk.is_contiguous() and Uk.dim() == 2
+        nb1 = Uk.shape[1]
+        self._check(self._lib.phoebe_elph_set_k(self._ctx, k.ctypes.data, Uk.data_ptr(), nb1), "phoebe_elph_set_k")
+        self.nb1 = nb1
+
+    def set_k_host(self, k, Uk):
+        import numpy as np
+        k = np.ascontiguousarray(k, dtype=np.float64)
+        Uk = np.ascontiguousarray(Uk, dtype=np.complex128)
+        nb1 = Uk.shape[1]
+        self._check(self._lib.phoebe_elph_set_k_host(self._ctx, k.ctypes.data, Uk.ctypes.data, nb1),
+                    "phoebe_elph_set_k_host")
+        self.nb1 = nb1
+
+    def q_batch(self, q, Ukq, ev, omega, out=None):
+        """All CUDA tensors: q [nq][3] f64, Ukq [nq][nw][nb2] c128, ev [nq][nm][nm] c128, omega [nq][nm] f64.
+        Returns out [nq][nb1][nb2][nm] f64 (CUDA)."""
+        torch = self._torch
+        nq, nw, nb2 = Ukq.shape
+        nm = self.dims.nmodes
+        for t in (q, Ukq, ev, omega):
+            assert t.is_cuda and t.is_contiguous()
+        assert q.shape == (nq, 3) and ev.shape == (nq, nm, nm) and omega.shape == (nq, nm)
+        if out is None:
+            out = torch.empty((nq, self.nb1, nb2, nm), dtype=torch.float64, device=self.device)
+        else:
+            assert out.is_cuda and out.is_contiguous() and out.numel() == nq * self.nb1 * nb2 * nm
+        self._check(self._lib.phoebe_elph_q_batch(self._ctx, nq, nb2, q.data_ptr(), Ukq.data_ptr(), ev.data_ptr(),
+                                                  omega.data_ptr(), out.data_ptr()), "phoebe_elph_q_batch")
+        return out
+
+    def q_batch_host(self, q, Ukq, ev, omega, out):
+        """NumPy arrays (or pinned CPU tensors via .numpy()); synchronises before returning."""
+        nq, nw, nb2 = Ukq.shape
+        self._check(self._lib.phoebe_elph_q_batch_host(self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data,
+                                                       ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
+                    "phoebe_elph_q_batch_host")
+        return out
+
+    def copy_g1(self):
+        torch = self._torch
+        d = self.dims
+        g1 = torch.empty((d.nRp, self.nb1, d.nw, d.nmodes), dtype=torch.complex128, device=self.device)
+        self._check(self._lib.phoebe_elph_copy_g1(self._ctx, g1.data_ptr(), g1.numel() * 16), "phoebe_elph_copy_g1")
+        return g1
+
+    def launch_counts(self):
+        arr = (c_int64 * len(KERNEL_KINDS))()
+        self._check(self._lib.phoebe_elph_launch_counts(self._ctx, arr), "phoebe_elph_launch_counts")
+        return dict(zip(KERNEL_KINDS, [int(x) for x in arr]))
+
+    def profile(self, enable: bool):
+        self._check(self._lib.phoebe_elph_profile(self._ctx, 1 if enable else 0), "phoebe_elph_profile")
+
+    def profile_read(self):
+        """-> {kind: (ms, launches)} since the last read."""
+        ms = (c_double * len(KERNEL_KINDS))()
+        n = (c_int64 * len(KERNEL_KINDS))()
+        self._check(self._lib.phoebe_elph_profile_read(self._ctx, ms, n), "phoebe_elph_profile_read")
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+    def set_tuning(self, key: str, value: int):
+        self._check(self._lib.phoebe_elph_set_tuning(self._ctx, key.encode(), int(value)), "phoebe_elph_set_tuning")
+
+    def get_tuning(self, key: str) -> int:
+        v = c_int64(0)
+        self._check(self._lib.phoebe_elph_get_tuning(self._ctx, key.encode(), byref(v)), "phoebe_elph_get_tuning")
+        return int(v.value)
+
+
+def probe_fp64(kind: str = "dmma", iters: int = 20000, stream=None) -> float:
+    """FP64 ceiling in TFLOP/s measured on this device (kind: 'dfma' | 'dmma')."""
+    t = c_double(0.0)
+    st = None if stream is None else stream.cuda_stream
+    rc = load_library().phoebe_elph_probe_fp64({"dfma": 0, "dmma": 1}[kind], iters, st, byref(t))
+    if rc:
+        raise PhoebeElphError(rc, "phoebe_elph_probe_fp64")
+    return float(t.value)
+
+
+def probe_hbm_read(buf, stream=None) -> float:
+    """HBM read-stream bandwidth in GB/s over a CUDA tensor."""
+    t = c_double(0.0)
+    st = None if stream is None else stream.cuda_stream
+    rc = load_library().phoebe_elph_probe_hbm_read(buf.data_ptr(), buf.numel() * buf.element_size(), st, byref(t))
+    if rc:
+        raise PhoebeElphError(rc, "phoebe_elph_probe_hbm_read")
+    return float(t.value)

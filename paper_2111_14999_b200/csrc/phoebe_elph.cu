@@ -1,0 +1,547 @@
+// phoebe_elph.cu -- C ABI (include/phoebe_elph.h) and host-side orchestration of the
+// sm_100a kernels for the el-ph Wannier->Bloch |g|^2 hot path (Eq. 7, 13, 70, 71).
+// No CPU fallback: every compute call fails with PHOEBE_ELPH_E_CUDA without a device.
+#include "../../include/phoebe_elph.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "probe_kernels.cuh"
+#include "qbatch_kernels.cuh"
+#include "setk_kernels.cuh"
+
+namespace {
+
+constexpr int kSMs = 148;                 // B200
+constexpr size_t kAlign = 256;
+constexpr int kQPad = 128;                // q columns of Pt are padded to this (largest BM)
+constexpr int kBNMax = 128;               // over-read slack behind g1' (largest BN)
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// ---- set_k launch geometry --------------------------------------------------
+int setk_threads(int X)
+{
+    for (int t = 256; t >= 64; t -= 32)
+        if (X % t == 0) return t;
+    if (X < 256) return (int)align_up((size_t)X, 32);
+    return 256;
+}
+int setk_auto_split(int nRe, int nRp, int X)
+{
+    const int T = setk_threads(X);
+    const long base = (long)nRp * ceil_div(X, T);
+    long S = (kSMs * 12 + base - 1) / base;
+    const long cap = std::max(1, nRe / 16);
+    S = std::max(1L, std::min(S, std::min(16L, cap)));
+    return (int)S;
+}
+
+// ---- workspace layout ---------------------------------------------------------
+struct Layout {
+    int Kpad = 0, ldq = 0, nq_sub = 0, S_alloc = 0;
+    size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_Tpart = 0, off_g1 = 0, off_Pt = 0,
+           off_C = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+};
+
+int default_nq_sub(const phoebe_elph_dims& d, int nq_max)
+{
+    const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
+    const size_t per_q = 16 * (N + (size_t)d.nRp);
+    long n = (long)((64ull << 20) / per_q);
+    n = n / kQPad * kQPad;
+    n = std::max<long>(n, kQPad);
+    n = std::min<long>(n, (long)align_up((size_t)nq_max, kQPad));
+    return (int)n;
+}
+
+Layout make_layout(const phoebe_elph_dims& d, int nq_max)
+{
+    Layout L;
+    const size_t X = (size_t)d.nw * d.nw * d.nmodes;
+    const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
+    L.Kpad = (int)align_up((size_t)d.nRp, 4);
+    L.nq_sub = default_nq_sub(d, nq_max);
+    L.ldq = L.nq_sub;
+    const int S_auto = setk_auto_split(d.nRe, d.nRp, (int)X);
+    const int cap = std::max(1, std::min(16, d.nRe / 16));
+    L.S_alloc = ((size_t)cap * d.nRp * X * 16 <= (256ull << 20)) ? std::max(cap, S_auto) : S_auto;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, kAlign); return o; };
+    L.off_Re = take((size_t)d.nRe * 3 * 8);
+    L.off_Rp = take((size_t)d.nRp * 3 * 8);
+    L.off_dege = take((size_t)d.nRe * 8);
+    L.off_degp = take((size_t)d.nRp * 8);
+    L.off_Uk = take((size_t)d.nw * d.nb1_max * 16);
+    L.off_Tpart = take((size_t)L.S_alloc * d.nRp * X * 16);
+    L.off_g1 = take(((size_t)L.Kpad * N + kBNMax) * 16);
+    L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
+    L.off_C = take((size_t)L.nq_sub * N * 16);
+    // staging for the host-buffer entry points
+    L.off_sq = take((size_t)nq_max * 3 * 8);
+    L.off_sUkq = take((size_t)nq_max * d.nw * d.nb2_max * 16);
+    L.off_sev = take((size_t)nq_max * d.nmodes * d.nmodes * 16);
+    L.off_som = take((size_t)nq_max * d.nmodes * 8);
+    L.off_sout = take((size_t)nq_max * d.nb1_max * d.nb2_max * d.nmodes * 8);
+    L.total = off;
+    return L;
+}
+
+bool dims_ok(const phoebe_elph_dims* d, bool need_nq)
+{
+    if (d->nRe <= 0 || d->nRp <= 0 || d->nw <= 0 || d->nmodes <= 0) return false;
+    if (d->nb1_max <= 0 || d->nb1_max > d->nw || d->nb2_max <= 0 || d->nb2_max > d->nw) return false;
+    if (d->nq_max < 0 || (need_nq && d->nq_max == 0)) return false;
+    if (d->nRp > 65535) return false;                       // grid.z / grid.y limits of the kernels
+    if ((long)d->nw * d->nw * d->nmodes > (1L << 24)) return false;
+    return true;
+}
+
+struct EventPair { int kind; cudaEvent_t a, b; };
+
+}  // namespace
+
+struct phoebe_elph_ctx {
+    phoebe_elph_dims dims{};
+    const double2* gW = nullptr;
+    cudaStream_t stream = nullptr;
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    Layout L;
+    double *Re = nullptr, *Rp = nullptr, *deg_e = nullptr, *deg_p = nullptr;
+    double2 *Uk = nullptr, *Tpart = nullptr, *g1 = nullptr, *Pt = nullptr, *C = nullptr;
+    int nb1 = 0;
+    bool have_k = false;
+    int nq_sub = 0, s_split = 0;
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0};
+    bool prof = false;
+    std::vector<EventPair> evs;
+    std::vector<cudaEvent_t> ev_pool;
+    std::string err;
+};
+
+namespace {
+
+int fail(phoebe_elph_ctx* c, int code, const char* msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+int cuda_fail(phoebe_elph_ctx* c, cudaError_t e, const char* what)
+{
+    if (c) { c->err = std::string(what) + ": " + cudaGetErrorString(e); }
+    return PHOEBE_ELPH_E_CUDA;
+}
+#define PE_CUDA(ctx, expr)                                              \
+    do {                                                                \
+        cudaError_t _e = (expr);                                        \
+        if (_e != cudaSuccess) return cuda_fail((ctx), _e, #expr);      \
+    } while (0)
+
+cudaEvent_t get_event(phoebe_elph_ctx* c)
+{
+    if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+struct LaunchScope {          // counts the launch and, when profiling, brackets it with events
+    phoebe_elph_ctx* c; int kind; cudaEvent_t b = nullptr;
+    LaunchScope(phoebe_elph_ctx* c_, int kind_) : c(c_), kind(kind_)
+    {
+        c->launches[kind]++;
+        if (c->prof) {
+            cudaEvent_t a = get_event(c); b = get_event(c);
+            cudaEventRecord(a, c->stream);
+            c->evs.push_back({kind, a, b});
+        }
+    }
+    ~LaunchScope() { if (b) cudaEventRecord(b, c->stream); }
+};
+
+// ---- contraction launcher -------------------------------------------------------
+template <int BM, int BN, int WM, int WN, int KC, int ST>
+cudaError_t launch_contract(phoebe_elph_ctx* c, int nq, int N)
+{
+    using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
+    auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    dim3 grid(ceil_div(N, BN), ceil_div(nq, BM));
+    kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, c->stream>>>(c->Pt, c->L.ldq, c->g1, N, c->C, N, nq, N, c->L.Kpad);
+    return cudaGetLastError();
+}
+
+int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb1)
+{
+    const phoebe_elph_dims& d = c->dims;
+    const int X = d.nw * d.nw * d.nmodes, Y = d.nw * d.nmodes, N = nb1 * Y;
+    const int T = setk_threads(X);
+    int S = c->s_split > 0 ? c->s_split : setk_auto_split(d.nRe, d.nRp, X);
+    S = std::min(S, c->L.S_alloc);
+    const int epc = ceil_div(d.nRe, S);
+    S = ceil_div(d.nRe, epc);
+    {
+        LaunchScope ls(c, PHOEBE_ELPH_K_SETK_STREAM);
+        dim3 grid(ceil_div(X, T), S, d.nRp);
+        pe::k_setk_stream<<<grid, T, (size_t)epc * 16, c->stream>>>(c->gW, c->Re, c->deg_e, k[0], k[1], k[2], d.nRe,
+                                                                    d.nRp, X, epc, c->Tpart);
+        PE_CUDA(c, cudaGetLastError());
+    }
+    // zero the K-padding rows of g1' for this N (rows nRp..Kpad-1)
+    if (c->L.Kpad > d.nRp)
+        PE_CUDA(c, cudaMemsetAsync(c->g1 + (size_t)d.nRp * N, 0, (size_t)(c->L.Kpad - d.nRp) * N * 16, c->stream));
+    {
+        LaunchScope ls(c, PHOEBE_ELPH_K_SETK_ROTATE);
+        const int TR = 128;
+        if (nb1 <= 4) {
+            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 4));
+            pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y, nb1,
+                                                                                 c->g1, N);
+        } else if (nb1 <= 8) {
+            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 8));
+            pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y, nb1,
+                                                                                 c->g1, N);
+        } else {
+            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 16));
+            pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y,
+                                                                                   nb1, c->g1, N);
+        }
+        PE_CUDA(c, cudaGetLastError());
+    }
+    c->nb1 = nb1;
+    c->have_k = true;
+    return PHOEBE_ELPH_OK;
+}
+
+int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const double2* Ukq, const double2* ev,
+                const double* omega, double* out)
+{
+    const phoebe_elph_dims& d = c->dims;
+    const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
+    const int nq_sub = std::min(c->nq_sub, c->L.nq_sub);
+    // rotation kernel geometry: as many b1 per CTA as fit in ~96 KB of shared memory
+    const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;
+    const size_t per_b1 = ((size_t)Y + (size_t)nb2 * d.nmodes) * 16;
+    int gb1 = (int)std::max<size_t>(1, std::min<size_t>((size_t)nb1, ((96u << 10) - std::min<size_t>(fixed, 90u << 10)) / per_b1));
+    const size_t rot_smem = fixed + per_b1 * gb1;
+    if (rot_smem > (200u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+    static size_t rot_attr = 0;
+    if (rot_smem > (48u << 10) && rot_smem > rot_attr) {
+        PE_CUDA(c, cudaFuncSetAttribute(pe::k_rotate_epilogue, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
+        rot_attr = rot_smem;
+    }
+    const int work = gb1 * nb2 * d.nmodes;
+    const int rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
+
+    for (int qs = 0; qs < nq; qs += nq_sub) {
+        const int nqs = std::min(nq_sub, nq - qs);
+        const int ncols = (int)align_up((size_t)nqs, kQPad);
+        {
+            LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
+            dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
+            pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
+                                                      c->L.ldq, c->Pt);
+            PE_CUDA(c, cudaGetLastError());
+        }
+        {
+            LaunchScope ls(c, PHOEBE_ELPH_K_CONTRACT);
+            PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3>(c, nqs, N)));
+        }
+        {
+            LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
+            dim3 grid(ceil_div(nb1, gb1), nqs);
+            pe::k_rotate_epilogue<<<grid, rot_threads, rot_smem, c->stream>>>(
+                c->C, N, Ukq + (size_t)qs * d.nw * nb2, ev + (size_t)qs * d.nmodes * d.nmodes,
+                omega + (size_t)qs * d.nmodes, out + (size_t)qs * nb1 * nb2 * d.nmodes, d.nw, d.nmodes, nb1, nb2, gb1);
+            PE_CUDA(c, cudaGetLastError());
+        }
+    }
+    return PHOEBE_ELPH_OK;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+// =============================================================================
+extern "C" {
+
+const char* phoebe_elph_version(void) { return "phoebe-elph-b200 0.1 (sm_100a)"; }
+
+int phoebe_elph_workspace_bytes(const phoebe_elph_dims* dims, size_t budget, size_t* bytes_out, int32_t* nq_batch_out)
+{
+    if (!dims || !bytes_out || !nq_batch_out) return PHOEBE_ELPH_E_NULL;
+    if (!dims_ok(dims, false)) return PHOEBE_ELPH_E_DIMS;
+    int hi = dims->nq_max > 0 ? dims->nq_max : (1 << 24);
+    if (make_layout(*dims, 1).total > budget) return PHOEBE_ELPH_E_WORKSPACE;
+    int lo = 1;                                   // invariant: layout(lo) fits
+    if (make_layout(*dims, hi).total <= budget) lo = hi;
+    while (lo < hi) {
+        int mid = lo + (hi - lo + 1) / 2;
+        if (make_layout(*dims, mid).total <= budget) lo = mid; else hi = mid - 1;
+    }
+    *nq_batch_out = lo;
+    *bytes_out = make_layout(*dims, lo).total;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const double* Re_host, const double* Rp_host,
+                      const double* deg_e_host, const double* deg_p_host, const phoebe_elph_dims* dims,
+                      void* workspace_dev, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!ctx_out) return PHOEBE_ELPH_E_NULL;
+    *ctx_out = nullptr;
+    if (!gW_dev || !Re_host || !Rp_host || !dims || !workspace_dev) return PHOEBE_ELPH_E_NULL;
+    if (!dims_ok(dims, true)) return PHOEBE_ELPH_E_DIMS;
+    if (!aligned16(gW_dev) || (reinterpret_cast<uintptr_t>(workspace_dev) & (kAlign - 1))) return PHOEBE_ELPH_E_ALIGN;
+    for (int i = 0; deg_e_host && i < dims->nRe; ++i) if (!(deg_e_host[i] > 0.0)) return PHOEBE_ELPH_E_DIMS;
+    for (int i = 0; deg_p_host && i < dims->nRp; ++i) if (!(deg_p_host[i] > 0.0)) return PHOEBE_ELPH_E_DIMS;
+    Layout L = make_layout(*dims, dims->nq_max);
+    if (L.total > workspace_bytes) return PHOEBE_ELPH_E_WORKSPACE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return PHOEBE_ELPH_E_CUDA;
+
+    phoebe_elph_ctx* c = new (std::nothrow) phoebe_elph_ctx();
+    if (!c) return PHOEBE_ELPH_E_CUDA;
+    c->dims = *dims;
+    c->gW = static_cast<const double2*>(gW_dev);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->ws = static_cast<char*>(workspace_dev);
+    c->ws_bytes = workspace_bytes;
+    c->L = L;
+    c->nq_sub = L.nq_sub;
+    c->Re = reinterpret_cast<double*>(c->ws + L.off_Re);
+    c->Rp = reinterpret_cast<double*>(c->ws + L.off_Rp);
+    c->deg_e = reinterpret_cast<double*>(c->ws + L.off_dege);
+    c->deg_p = reinterpret_cast<double*>(c->ws + L.off_degp);
+    c->Uk = reinterpret_cast<double2*>(c->ws + L.off_Uk);
+    c->Tpart = reinterpret_cast<double2*>(c->ws + L.off_Tpart);
+    c->g1 = reinterpret_cast<double2*>(c->ws + L.off_g1);
+    c->Pt = reinterpret_cast<double2*>(c->ws + L.off_Pt);
+    c->C = reinterpret_cast<double2*>(c->ws + L.off_C);
+
+    std::vector<double> ones((size_t)std::max(dims->nRe, dims->nRp), 1.0);
+    cudaError_t e = cudaSuccess;
+    auto up = [&](void* dst, const void* src, size_t bytes) {
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream);
+    };
+    up(c->Re, Re_host, (size_t)dims->nRe * 24);
+    up(c->Rp, Rp_host, (size_t)dims->nRp * 24);
+    up(c->deg_e, deg_e_host ? deg_e_host : ones.data(), (size_t)dims->nRe * 8);
+    up(c->deg_p, deg_p_host ? deg_p_host : ones.data(), (size_t)dims->nRp * 8);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->g1, 0, L.off_Pt - L.off_g1, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { delete c; return PHOEBE_ELPH_E_CUDA; }
+    *ctx_out = c;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_set_k(phoebe_elph_ctx* c, const double* k_host, const void* Uk_dev, int32_t nb1)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!k_host || !Uk_dev) return fail(c, PHOEBE_ELPH_E_NULL, "set_k: null pointer");
+    if (nb1 <= 0 || nb1 > c->dims.nb1_max) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k: nb1 out of range");
+    if (!aligned16(Uk_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "set_k: Uk not 16-byte aligned");
+    return run_set_k(c, k_host, static_cast<const double2*>(Uk_dev), nb1);
+}
+
+int phoebe_elph_set_k_host(phoebe_elph_ctx* c, const double* k_host, const void* Uk_host, int32_t nb1)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!k_host || !Uk_host) return fail(c, PHOEBE_ELPH_E_NULL, "set_k_host: null pointer");
+    if (nb1 <= 0 || nb1 > c->dims.nb1_max) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_host: nb1 out of range");
+    PE_CUDA(c, cudaMemcpyAsync(c->Uk, Uk_host, (size_t)c->dims.nw * nb1 * 16, cudaMemcpyHostToDevice, c->stream));
+    return run_set_k(c, k_host, c->Uk, nb1);
+}
+
+int phoebe_elph_q_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_dev, const void* Ukq_dev,
+                        const void* ev_dev, const double* omega_dev, double* out_dev)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !out_dev) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch: nb2 out of range");
+    if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch: complex input not 16-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(q_dev) | reinterpret_cast<uintptr_t>(omega_dev) | reinterpret_cast<uintptr_t>(out_dev)) & 7u)
+        return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch: double array not 8-byte aligned");
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    return run_q_batch(c, nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
+                       omega_dev, out_dev);
+}
+
+int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
+                             const void* ev_host, const double* omega_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nb2 out of range");
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    const phoebe_elph_dims& d = c->dims;
+    double* sq = reinterpret_cast<double*>(c->ws + c->L.off_sq);
+    double2* sU = reinterpret_cast<double2*>(c->ws + c->L.off_sUkq);
+    double2* sZ = reinterpret_cast<double2*>(c->ws + c->L.off_sev);
+    double* sw = reinterpret_cast<double*>(c->ws + c->L.off_som);
+    double* so = reinterpret_cast<double*>(c->ws + c->L.off_sout);
+    PE_CUDA(c, cudaMemcpyAsync(sq, q_host, (size_t)nq * 24, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sZ, ev_host, (size_t)nq * d.nmodes * d.nmodes * 16, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sw, omega_host, (size_t)nq * d.nmodes * 8, cudaMemcpyHostToDevice, c->stream));
+    int rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
+    if (rc) return rc;
+    PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->stream));
+    PE_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_copy_g1(phoebe_elph_ctx* c, void* dst_dev, size_t dst_bytes)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!dst_dev) return fail(c, PHOEBE_ELPH_E_NULL, "copy_g1: null pointer");
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "copy_g1 before set_k");
+    const size_t bytes = (size_t)c->dims.nRp * c->nb1 * c->dims.nw * c->dims.nmodes * 16;
+    if (dst_bytes < bytes) return fail(c, PHOEBE_ELPH_E_WORKSPACE, "copy_g1: destination too small");
+    PE_CUDA(c, cudaMemcpyAsync(dst_dev, c->g1, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_launch_counts(const phoebe_elph_ctx* c, int64_t* counts)
+{
+    if (!c || !counts) return PHOEBE_ELPH_E_NULL;
+    for (int i = 0; i < PHOEBE_ELPH_K_COUNT; ++i) counts[i] = c->launches[i];
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_profile(phoebe_elph_ctx* c, int32_t enable)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    c->prof = enable != 0;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_profile_read(phoebe_elph_ctx* c, double* ms, int64_t* launches)
+{
+    if (!c || !ms || !launches) return PHOEBE_ELPH_E_NULL;
+    PE_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < PHOEBE_ELPH_K_COUNT; ++i) { ms[i] = 0.0; launches[i] = 0; }
+    for (const EventPair& p : c->evs) {
+        float t = 0.f;
+        PE_CUDA(c, cudaEventElapsedTime(&t, p.a, p.b));
+        ms[p.kind] += t;
+        launches[p.kind]++;
+        c->ev_pool.push_back(p.a);
+        c->ev_pool.push_back(p.b);
+    }
+    c->evs.clear();
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
+{
+    if (!c || !key) return PHOEBE_ELPH_E_NULL;
+    if (!strcmp(key, "nq_sub")) {
+        if (value < 1) return fail(c, PHOEBE_ELPH_E_DIMS, "nq_sub must be >= 1");
+        c->nq_sub = (int)std::min<int64_t>(value, c->L.nq_sub);
+        return PHOEBE_ELPH_OK;
+    }
+    if (!strcmp(key, "s_split")) {
+        if (value < 0 || value > c->L.S_alloc) return fail(c, PHOEBE_ELPH_E_DIMS, "s_split out of range");
+        c->s_split = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
+    return fail(c, PHOEBE_ELPH_E_DIMS, "unknown tuning key");
+}
+
+int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* value)
+{
+    if (!c || !key || !value) return PHOEBE_ELPH_E_NULL;
+    if (!strcmp(key, "nq_sub")) { *value = c->nq_sub; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "s_split")) {
+        *value = c->s_split > 0 ? c->s_split
+                                : setk_auto_split(c->dims.nRe, c->dims.nRp, c->dims.nw * c->dims.nw * c->dims.nmodes);
+        return PHOEBE_ELPH_OK;
+    }
+    if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "nq_sub_max")) { *value = c->L.nq_sub; return PHOEBE_ELPH_OK; }
+    return PHOEBE_ELPH_E_DIMS;
+}
+
+int phoebe_elph_destroy(phoebe_elph_ctx* c)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    for (const EventPair& p : c->evs) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    delete c;
+    return PHOEBE_ELPH_OK;
+}
+
+const char* phoebe_elph_last_error(const phoebe_elph_ctx* c) { return c ? c->err.c_str() : ""; }
+
+int phoebe_elph_probe_fp64(int32_t kind, int32_t iters, void* cuda_stream, double* tflops_out)
+{
+    if (!tflops_out) return PHOEBE_ELPH_E_NULL;
+    if (kind < 0 || kind > 1 || iters <= 0) return PHOEBE_ELPH_E_DIMS;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int grid = kSMs * 4, threads = 256;
+    double* out = nullptr;
+    if (cudaMalloc(&out, (size_t)grid * threads * 8) != cudaSuccess) return PHOEBE_ELPH_E_CUDA;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(a, st);
+        if (kind == 0) pe::k_probe_dfma<<<grid, threads, 0, st>>>(out, iters, 1.0000001, 1e-9);
+        else pe::k_probe_dmma<<<grid, threads, 0, st>>>(out, iters, 1.0000001, 1e-9);
+        cudaEventRecord(b, st);
+        if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(out); return PHOEBE_ELPH_E_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        if (rep > 0) best = std::min(best, ms);
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(out);
+    const double fma_per_thread_iter = (kind == 0) ? 64.0 : (32.0 * 256.0 / 32.0);   // DMMA: 256 FMA per warp instr
+    const double flops = 2.0 * fma_per_thread_iter * iters * (double)grid * threads;
+    *tflops_out = flops / (best * 1e-3) * 1e-12;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_probe_hbm_read(const void* buf_dev, size_t bytes, void* cuda_stream, double* gbs_out)
+{
+    if (!buf_dev || !gbs_out) return PHOEBE_ELPH_E_NULL;
+    if (bytes < 16 || !aligned16(buf_dev)) return PHOEBE_ELPH_E_DIMS;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    double* out = nullptr;
+    if (cudaMalloc(&out, 8) != cudaSuccess) return PHOEBE_ELPH_E_CUDA;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(a, st);
+        pe::k_probe_read<<<kSMs * 8, 256, 0, st>>>(static_cast<const double2*>(buf_dev), bytes / 16, out);
+        cudaEventRecord(b, st);
+        if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(out); return PHOEBE_ELPH_E_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        if (rep > 0) best = std::min(best, ms);
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    cudaFree(out);
+    *gbs_out = (double)(bytes / 16 * 16) / (best * 1e-3) * 1e-9;
+    return PHOEBE_ELPH_OK;
+}
+
+}  // extern "C"

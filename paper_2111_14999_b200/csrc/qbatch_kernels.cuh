@@ -1,0 +1,226 @@
+// qbatch_kernels.cuh -- steps a3..a7 (Eq. 70 + Eq. 7): completion for a batch of q.
+//
+//   a3  Pt[p][q]           = e^{2 pi i q.Rp_p}/deg_p[p]                      (k_qphase)
+//   a4  C[q][n]            = sum_p Pt[p][q] g1[p][n]      n=(b1,w2,kappa)     (k_contract, FP64 DMMA)
+//   a5  D[q][b1][b2][ka]   = sum_w2 conj(Ukq[q][w2][b2]) C[q][b1][w2][ka]     (k_rotate_epilogue)
+//   a6  E[q][b1][b2][nu]   = sum_ka D[q][b1][b2][ka] ev[q][ka][nu]
+//   a7  out                = |E|^2/(2 omega)   (0 where omega <= 0)
+#pragma once
+#include "ptx_helpers.cuh"
+
+namespace pe {
+
+// ---------------------------------------------------------------------------
+// a3: phases, written TRANSPOSED (p-major, q contiguous) so that both operands of
+// the contraction are "k-major" and a tile row is one contiguous bulk copy.
+// Columns q in [nq, ldq) and rows p in [nRp, Kpad) are written as zeros.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rp, const double* __restrict__ deg_p,
+         int nq, int nRp, int Kpad, int ldq, double2* __restrict__ Pt /* [Kpad][ldq] */)
+{
+    const int iq = blockIdx.x * blockDim.x + threadIdx.x;
+    if (iq >= ldq) return;
+    double q0 = 0.0, q1 = 0.0, q2 = 0.0;
+    const bool valid = iq < nq;
+    if (valid) { q0 = q[3 * (size_t)iq]; q1 = q[3 * (size_t)iq + 1]; q2 = q[3 * (size_t)iq + 2]; }
+    for (int p = blockIdx.y; p < Kpad; p += gridDim.y) {
+        double2 v = make_double2(0.0, 0.0);
+        if (valid && p < nRp) {
+            const double x = q0 * Rp[3 * p] + q1 * Rp[3 * p + 1] + q2 * Rp[3 * p + 2];
+            double sn, cs;
+            sincospi(2.0 * x, &sn, &cs);
+            const double w = 1.0 / deg_p[p];
+            v = make_double2(cs * w, sn * w);
+        }
+        Pt[(size_t)p * ldq + iq] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------
+// a4: C[q][n] = sum_k Pt[k][q] * B[k][n]   (complex128, K = Kpad rows, zero padded)
+//
+// Warp-specialised: one producer warp streams [KC x BM] tiles of Pt and [KC x BN]
+// tiles of g1' into a STAGES-deep shared-memory ring with TMA 1-D bulk copies
+// (one per tile row, completion on an mbarrier); WARPS_M x WARPS_N consumer warps
+// run FP64 tensor-core tiles (mma.sync m8n8k4 -> SASS DMMA.8x8x4):
+//     Cr += Pr*Br + (-Pi)*Bi ,   Ci += Pr*Bi + Pi*Br          (4 DMMA per 8x8 complex tile per k4)
+// Shared rows are padded by 2 complex so that the per-lane fragment loads
+// (LDS.128 at [k0+t][.. + g]) are bank-conflict free.
+// ---------------------------------------------------------------------------
+template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES>
+struct ContractCfg {
+    static constexpr int kConsumerWarps = WARPS_M * WARPS_N;
+    static constexpr int kThreads = (kConsumerWarps + 1) * 32;
+    static constexpr int TM = BM / WARPS_M / 8;
+    static constexpr int TN = BN / WARPS_N / 8;
+    static constexpr int LDA = BM + 2;     // complex elements per shared row
+    static constexpr int LDB = BN + 2;
+    static constexpr size_t kSmemBytes =
+        (size_t)STAGES * KC * (LDA + LDB) * sizeof(double2) + 2 * STAGES * sizeof(uint64_t);
+    static_assert(BM % (WARPS_M * 8) == 0 && BN % (WARPS_N * 8) == 0, "tile/warp mismatch");
+    static_assert(KC % 4 == 0 && KC <= 32, "KC rows are issued by the 32 producer lanes");
+};
+
+template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES>
+__global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32)
+k_contract(const double2* __restrict__ Pt, int ldq, const double2* __restrict__ B, int ldb,
+           double2* __restrict__ C, int ldc, int nq, int N, int Kpad)
+{
+    using Cfg = ContractCfg<BM, BN, WARPS_M, WARPS_N, KC, STAGES>;
+    constexpr int TM = Cfg::TM, TN = Cfg::TN, LDA = Cfg::LDA, LDB = Cfg::LDB;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* As = reinterpret_cast<double2*>(smem_raw);                  // [STAGES][KC][LDA]
+    double2* Bs = As + (size_t)STAGES * KC * LDA;                        // [STAGES][KC][LDB]
+    uint64_t* full = reinterpret_cast<uint64_t*>(Bs + (size_t)STAGES * KC * LDB);
+    uint64_t* empty = full + STAGES;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n0 = blockIdx.x * BN, q0 = blockIdx.y * BM;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, Cfg::kConsumerWarps); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int nchunks = (Kpad + KC - 1) / KC;
+
+    if (warp == Cfg::kConsumerWarps) {
+        // ---------------- producer warp ----------------
+        const double2* a_src = Pt + q0;
+        const double2* b_src = B + n0;
+        for (int c = 0; c < nchunks; ++c) {
+            const int s = c % STAGES;
+            const uint32_t use = (uint32_t)(c / STAGES);
+            mbar_wait(empty + s, (use & 1u) ^ 1u);
+            const int k0 = c * KC;
+            const int rows = min(KC, Kpad - k0);
+            if (lane == 0) mbar_arrive_expect_tx(full + s, (uint32_t)(rows * (BM + BN) * sizeof(double2)));
+            __syncwarp();
+            if (lane < rows) {
+                bulk_g2s(As + ((size_t)s * KC + lane) * LDA, a_src + (size_t)(k0 + lane) * ldq,
+                         BM * sizeof(double2), full + s);
+                bulk_g2s(Bs + ((size_t)s * KC + lane) * LDB, b_src + (size_t)(k0 + lane) * ldb,
+                         BN * sizeof(double2), full + s);
+            }
+        }
+        return;
+    }
+
+    // ---------------- consumer warps ----------------
+    const int wm = warp / WARPS_N, wn = warp % WARPS_N;
+    const int g = lane >> 2, t = lane & 3;
+    double cr[TM][TN][2], ci[TM][TN][2];
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) { cr[i][j][0] = cr[i][j][1] = 0.0; ci[i][j][0] = ci[i][j][1] = 0.0; }
+
+    for (int c = 0; c < nchunks; ++c) {
+        const int s = c % STAGES;
+        const uint32_t use = (uint32_t)(c / STAGES);
+        mbar_wait(full + s, use & 1u);
+        const int rows = min(KC, Kpad - c * KC);
+        const double2* a_base = As + ((size_t)s * KC + t) * LDA + wm * TM * 8 + g;
+        const double2* b_base = Bs + ((size_t)s * KC + t) * LDB + wn * TN * 8 + g;
+#pragma unroll
+        for (int k4 = 0; k4 < KC / 4; ++k4) {
+            if (k4 * 4 < rows) {
+                double2 a[TM], b[TN];
+#pragma unroll
+                for (int i = 0; i < TM; ++i) a[i] = a_base[(size_t)k4 * 4 * LDA + i * 8];
+#pragma unroll
+                for (int j = 0; j < TN; ++j) b[j] = b_base[(size_t)k4 * 4 * LDB + j * 8];
+#pragma unroll
+                for (int i = 0; i < TM; ++i) {
+                    const double npi = neg(a[i].y);
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) {
+                        dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+                        dmma884(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
+                        dmma884(cr[i][j][0], cr[i][j][1], npi, b[j].y);
+                        dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + s);
+    }
+
+    // ---------------- store C (complex interleaved) ----------------
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+        const int qq = q0 + wm * TM * 8 + i * 8 + g;
+        if (qq >= nq) continue;
+#pragma unroll
+        for (int j = 0; j < TN; ++j) {
+            const int n = n0 + wn * TN * 8 + j * 8 + 2 * t;
+            double2* dst = C + (size_t)qq * ldc + n;
+            if (n < N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
+            if (n + 1 < N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
+// a5..a7: per (q, group of b1): rotate by conj(Ukq), by ev, square, scale.
+// First, plain shared-memory version (DFMA).
+// smem: Uc[nw][nb2] (already conjugated), Z[nm][nm], Cs[gb1][nw*nm], Ds[gb1][nb2*nm]
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restrict__ Ukq,
+                  const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
+                  int nw, int nm, int nb1, int nb2, int gb1)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* Uc = reinterpret_cast<double2*>(smem_raw);
+    double2* Z = Uc + nw * nb2;
+    double2* Cs = Z + nm * nm;
+    double2* Ds = Cs + (size_t)gb1 * nw * nm;
+    const int iq = blockIdx.y;
+    const int b10 = blockIdx.x * gb1;
+    const int nb1l = min(gb1, nb1 - b10);
+    const int Y = nw * nm;
+    const double2* Uq = Ukq + (size_t)iq * nw * nb2;
+    for (int i = threadIdx.x; i < nw * nb2; i += blockDim.x) { double2 u = Uq[i]; Uc[i] = make_double2(u.x, -u.y); }
+    const double2* Zq = ev + (size_t)iq * nm * nm;
+    for (int i = threadIdx.x; i < nm * nm; i += blockDim.x) Z[i] = Zq[i];
+    const double2* Cq = C + (size_t)iq * ldc + (size_t)b10 * Y;
+    for (int i = threadIdx.x; i < nb1l * Y; i += blockDim.x) Cs[i] = Cq[i];
+    __syncthreads();
+    // a5
+    const int nD = nb1l * nb2 * nm;
+    for (int idx = threadIdx.x; idx < nD; idx += blockDim.x) {
+        const int ka = idx % nm;
+        const int b2 = (idx / nm) % nb2;
+        const int b1 = idx / (nm * nb2);
+        double sr = 0.0, si = 0.0;
+        const double2* cc = Cs + (size_t)b1 * Y + ka;
+        for (int w2 = 0; w2 < nw; ++w2) {
+            const double2 u = Uc[w2 * nb2 + b2];
+            const double2 c = cc[w2 * nm];
+            sr = fma(u.x, c.x, sr); sr = fma(-u.y, c.y, sr);
+            si = fma(u.x, c.y, si); si = fma(u.y, c.x, si);
+        }
+        Ds[idx] = make_double2(sr, si);
+    }
+    __syncthreads();
+    // a6 + a7
+    const double* om = omega + (size_t)iq * nm;
+    double* o = out + ((size_t)iq * nb1 + b10) * nb2 * nm;
+    for (int idx = threadIdx.x; idx < nD; idx += blockDim.x) {
+        const int nu = idx % nm;
+        const double2* d = Ds + (idx - nu);
+        double sr = 0.0, si = 0.0;
+        for (int ka = 0; ka < nm; ++ka) {
+            const double2 z = Z[ka * nm + nu];
+            const double2 c = d[ka];
+            sr = fma(c.x, z.x, sr); sr = fma(-c.y, z.y, sr);
+            si = fma(c.x, z.y, si); si = fma(c.y, z.x, si);
+        }
+        const double w = om[nu];
+        o[idx] = (w > 0.0) ? (sr * sr + si * si) / (2.0 * w) : 0.0;
+    }
+}
+
+}  // namespace pe

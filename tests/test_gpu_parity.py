@@ -1,0 +1,199 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by
+element, on the same seeded inputs.  Bar (BASELINE.json north_star, reading R10):
+    max |out_gpu - out_oracle| <= 1e-10 * max(out_oracle)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _relerr(got, ref):
+    return float(np.max(np.abs(got - ref)) / np.max(np.abs(ref)))
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import oracle
+    from paper_2111_14999_b200 import binding, build, harness, workloads as wl
+    build.build()
+    binding.load_library()
+    assert torch.cuda.is_available()
+    return dict(torch=torch, oracle=oracle, binding=binding, harness=harness, wl=wl)
+
+
+def _run_gpu(env, w, gW_np, k, Uk, q, Ukq, ev, om, deg_e=None, deg_p=None, nq_max=None, host=False):
+    torch, harness = env["torch"], env["harness"]
+    gW = torch.from_numpy(gW_np).cuda()
+    ctx = harness.make_context(w, gW, nq_max=nq_max or len(q), deg_e=deg_e, deg_p=deg_p)
+    if host:
+        ctx.set_k_host(k, Uk)
+        out = np.empty((len(q), Uk.shape[1], Ukq.shape[2], w.nm))
+        ctx.q_batch_host(q, Ukq, ev, om, out)
+        g1 = ctx.copy_g1().cpu().numpy()
+    else:
+        (Uk_d,) = harness.to_device([Uk])
+        ctx.set_k(k, Uk_d)
+        q_d, Ukq_d, ev_d, om_d = harness.to_device([q, Ukq, ev, om])
+        out = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
+        g1 = ctx.copy_g1().cpu().numpy()
+    torch.cuda.synchronize()
+    ctx.close()
+    return out, g1
+
+
+def _inputs(wl, w, ik=0):
+    return dict(gW=wl.gW_full(w), Re=wl.Re_vectors(w), Rp=wl.Rp_vectors(w), k=wl.k_points(w)[ik], Uk=wl.U_k(w, ik),
+                q=wl.q_points(w, ik), Ukq=wl.U_kq(w, ik), ev=wl.ph_eigvecs(w, ik), om=wl.omega(w, ik))
+
+
+def test_tiny_full(env):
+    wl, oracle = env["wl"], env["oracle"]
+    w = wl.CONFIGS["tiny"]
+    a = _inputs(wl, w)
+    out, g1 = _run_gpu(env, w, a["gW"], a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+    g1_ref = oracle.setk(a["gW"], a["Re"], None, a["k"], a["Uk"])
+    assert _relerr(g1, g1_ref) < 1e-12
+    ref = oracle.qbatch(g1_ref, a["Rp"], None, a["q"], a["Ukq"], a["ev"], a["om"])
+    assert out.shape == ref.shape == (64, 2, 2, 3)
+    assert _relerr(out, ref) <= TOL
+    # and against the un-factorised double sum on a few q
+    d = oracle.direct(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"][:4], a["Ukq"][:4], a["ev"][:4],
+                      a["om"][:4])
+    assert _relerr(out[:4], d) <= TOL
+
+
+RAGGED = [
+    # nw nb1 nb2 nm  grid_e     grid_p     nq
+    (3, 2, 1, 2, (5, 1, 1), (7, 1, 1), 1),
+    (3, 3, 2, 3, (1, 2, 3), (3, 3, 1), 130),
+    (4, 1, 4, 1, (2, 2, 2), (1, 1, 1), 65),
+    (5, 4, 3, 6, (3, 3, 2), (2, 5, 3), 257),
+    (1, 1, 1, 1, (1, 1, 1), (1, 1, 2), 3),
+    (8, 4, 4, 6, (3, 3, 3), (3, 3, 3), 200),
+    (6, 6, 5, 9, (4, 3, 2), (3, 2, 5), 96),
+]
+
+
+@pytest.mark.parametrize("case", RAGGED, ids=lambda c: "nw%d_nb%d_%d_nm%d_nq%d" % (c[0], c[1], c[2], c[3], c[6]))
+@pytest.mark.parametrize("host", [False, True], ids=["dev", "host"])
+def test_ragged_small_cases(env, case, host):
+    wl, oracle = env["wl"], env["oracle"]
+    nw, nb1, nb2, nm, ge, gp, nq = case
+    w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=ge, grid_p=gp, nq=nq, cfg_id=70 + nw)
+    a = _inputs(wl, w)
+    rng = np.random.default_rng(nq)
+    deg_e = rng.integers(1, 4, w.nRe).astype(np.float64)
+    deg_p = rng.integers(1, 4, w.nRp).astype(np.float64)
+    out, g1 = _run_gpu(env, w, a["gW"], a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"], deg_e, deg_p, host=host)
+    g1_ref = oracle.setk(a["gW"], a["Re"], deg_e, a["k"], a["Uk"])
+    assert _relerr(g1, g1_ref) < 1e-12
+    ref = oracle.qbatch(g1_ref, a["Rp"], deg_p, a["q"], a["Ukq"], a["ev"], a["om"])
+    assert out.shape == ref.shape
+    assert _relerr(out, ref) <= TOL
+
+
+def test_nonpositive_omega_and_sub_batches(env):
+    """R7 (omega <= 0 -> 0) and the internal q sub-batching (nq_sub smaller than nq)."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=4, nb1=3, nb2=4, nm=3, grid_e=(3, 3, 3), nq=300, cfg_id=81)
+    a = _inputs(wl, w)
+    om = a["om"].copy(); om[5, 1] = 0.0; om[299, 2] = -0.3
+    ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], om)
+    gW = torch.from_numpy(a["gW"]).cuda()
+    ctx = harness.make_context(w, gW, nq_max=300)
+    ctx.set_tuning("nq_sub", 128)
+    (Uk_d,) = harness.to_device([a["Uk"]])
+    ctx.set_k(a["k"], Uk_d)
+    q_d, Ukq_d, ev_d, om_d = harness.to_device([a["q"], a["Ukq"], a["ev"], om])
+    out = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
+    assert np.all(out[5, :, :, 1] == 0.0) and np.all(out[299, :, :, 2] == 0.0)
+    assert _relerr(out, ref) <= TOL
+    n = ctx.launch_counts()
+    assert n["contract"] == 3 and n["qphase"] == 3 and n["rotate_epilogue"] == 3 and n["setk_stream"] == 1
+    ctx.close()
+
+
+def test_band_windows_change_between_calls_and_errors(env):
+    """nb1 may change on every set_k, nb2 on every q_batch; error codes."""
+    wl, oracle, torch, harness, binding = env["wl"], env["oracle"], env["torch"], env["harness"], env["binding"]
+    w = wl.custom(nw=6, nm=3, grid_e=(3, 2, 3), nq=40, cfg_id=82)
+    a = _inputs(wl, w)
+    gW = torch.from_numpy(a["gW"]).cuda()
+    ctx = harness.make_context(w, gW, nq_max=40)
+    q_d, ev_d, om_d = harness.to_device([a["q"], a["ev"], a["om"]])
+    with pytest.raises(binding.PhoebeElphError) as e:
+        ctx.q_batch(q_d, harness.to_device([a["Ukq"]])[0], ev_d, om_d)
+    assert e.value.code == -4
+    for nb1, nb2 in [(6, 6), (2, 5), (5, 1), (1, 6)]:
+        Uk = np.ascontiguousarray(a["Uk"][:, :nb1]); Ukq = np.ascontiguousarray(a["Ukq"][:, :, :nb2])
+        Uk_d, Ukq_d = harness.to_device([Uk, Ukq])
+        ctx.set_k(a["k"], Uk_d)
+        out = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
+        ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], Uk, a["q"], Ukq, a["ev"], a["om"])
+        assert out.shape == (40, nb1, nb2, 3)
+        assert _relerr(out, ref) <= TOL
+    # nq beyond nq_max
+    big = torch.zeros((41, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(binding.PhoebeElphError) as e:
+        ctx.q_batch(big, torch.zeros((41, 6, 6), dtype=torch.complex128, device="cuda"),
+                    torch.zeros((41, 3, 3), dtype=torch.complex128, device="cuda"),
+                    torch.zeros((41, 3), dtype=torch.float64, device="cuda"))
+    assert e.value.code == -2
+    ctx.close()
+
+
+def test_periodicity_on_gpu(env):
+    """Eq. 87: out(k, q+G) = out(k, q) for integer G -- a property that holds at any size."""
+    wl, torch, harness = env["wl"], env["torch"], env["harness"]
+    w = wl.custom(nw=4, nm=3, grid_e=(3, 3, 3), nq=64, cfg_id=83)
+    a = _inputs(wl, w)
+    gW = torch.from_numpy(a["gW"]).cuda()
+    ctx = harness.make_context(w, gW, nq_max=64)
+    Uk_d, Ukq_d, ev_d, om_d = harness.to_device([a["Uk"], a["Ukq"], a["ev"], a["om"]])
+    ctx.set_k(a["k"], Uk_d)
+    (q_d,) = harness.to_device([a["q"]])
+    base = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
+    (q2_d,) = harness.to_device([a["q"] + np.array([1.0, -2.0, 3.0])])
+    shifted = ctx.q_batch(q2_d, Ukq_d, ev_d, om_d).cpu().numpy()
+    assert _relerr(shifted, base) < 1e-11
+    ctx.set_k(a["k"] + np.array([-1.0, 2.0, 1.0]), Uk_d)
+    shifted_k = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
+    assert _relerr(shifted_k, base) < 1e-11
+    ctx.close()
+
+
+def test_si_like_full(env):
+    """BASELINE.json configs[1], every one of the 4096 q."""
+    wl, oracle = env["wl"], env["oracle"]
+    w = wl.CONFIGS["si-like"]
+    a = _inputs(wl, w)
+    out, g1 = _run_gpu(env, w, a["gW"], a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+    g1_ref = oracle.setk(a["gW"], a["Re"], None, a["k"], a["Uk"])
+    assert _relerr(g1, g1_ref) < 1e-12
+    ref = oracle.qbatch(g1_ref, a["Rp"], None, a["q"], a["Ukq"], a["ev"], a["om"])
+    assert _relerr(out, ref) <= TOL
+
+
+def test_band_window_three_k(env):
+    """BASELINE.json configs[3] (rectangular U, nb < nw): 3 of the 256 k, all 4096 q each."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.CONFIGS["band-window"]
+    gW_np = wl.gW_full(w)
+    gW = torch.from_numpy(gW_np).cuda()
+    ctx = harness.make_context(w, gW)
+    Re, Rp, ks = wl.Re_vectors(w), wl.Rp_vectors(w), wl.k_points(w)
+    worst = 0.0
+    for ik in (0, 101, 255):
+        Uk = wl.U_k(w, ik)
+        q, Ukq, ev, om = wl.q_inputs(w, ik)
+        ctx.set_k(ks[ik], harness.to_device([Uk])[0])
+        out = ctx.q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
+        ref = oracle.elph(gW_np, Re, Rp, None, None, ks[ik], Uk, q, Ukq, ev, om)
+        assert out.shape == (4096, 4, 4, 6)
+        worst = max(worst, _relerr(out, ref))
+    assert worst <= TOL
+    ctx.close()
