@@ -47,6 +47,22 @@ def _measured_peaks():
     return {"hbm_gbs": HBM_FALLBACK_GBS}, "fallback"
 
 
+def _ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full
+    summary profiles/traffic.csv (columns: workload,kernel,dram_bytes_per_launch,source); None if not captured."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None
+    try:
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] == workload and f[1] == kernel:
+                return float(f[2])
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
 
@@ -95,20 +111,7 @@ class ClockSampler:
         return out
 
 
-def _dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
-
-
-def shard_k(nk: int, rank: int, world: int, scaling: str = "weak"):
-    """k-point indices a rank processes.  (k,q) pairs are independent, so the
-    path shards over k with no data-path collective.  weak: every rank runs nk k-points of its
-    own (indices rank*nk ..); strong: the nk k-points are dealt round-robin."""
-    if scaling == "weak":
-        return list(range(rank * nk, (rank + 1) * nk))
-    return list(range(rank, nk, world))
+from paper_2111_14999_b200.sharding import dist_env as _dist_env, max_over_ranks, shard_k  # noqa: E402
 
 
 def _k_inputs(w, ik):
@@ -236,11 +239,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def maxreduce(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return max_over_ranks(x, dist, dev)
 
     # ---- device-resident timing ------------------------------------------------
     for _ in range(max(3, args.warmup)):
@@ -295,13 +294,7 @@ def run_ours(args):
             kernels[kind]["frac"] = kernels[kind]["achieved"] / kernels[kind]["peak"]
     dominant = max(kernels, key=lambda kk: kernels[kk]["ms_total"])
     dk = kernels[dominant]
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(w.name, {}).get(dominant)
-        except Exception:
-            traffic = None
+    traffic = _ncu_traffic(w.name, dominant)
     roofline = {"kernel": dominant, "bound": dk.get("bound"), "achieved": dk.get("achieved"), "peak": dk.get("peak"),
                 "unit": dk.get("unit"), "frac": dk.get("frac"), "traffic": traffic,
                 "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % peak_src) if dk.get("bound") == "hbm"
