@@ -196,6 +196,12 @@ def _config_dict(w, n_gpus):
             "parallelism": f"k-sharded x{n_gpus}, g_W replicated, no collective"}
 
 
+def _with_kbatch(cfg, kb):
+    cfg = dict(cfg)
+    cfg["set_k_batch"] = kb
+    return cfg
+
+
 # ----------------------------------------------------------------------------- GPU leg
 def run_ours(args):
     import torch
@@ -225,13 +231,27 @@ def run_ours(args):
     for k, Uk, (q, Ukq, ev, om) in host_inputs:
         dev_inputs.append((k, harness.to_device([Uk], dev)[0], harness.to_device([q, Ukq, ev, om], dev)))
     t_gen = time.perf_counter() - t_gen
-    ctx = harness.make_context(w, gW)
+    kb = max(1, min(args.k_batch, 32, len(host_inputs)))
+    ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0)
     out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+    # k-points grouped into batches of kb: one pass over g_W per batch (set_k_batch)
+    groups = [list(range(i, min(i + kb, len(host_inputs)))) for i in range(0, len(host_inputs), kb)]
+    ks_np = [np.stack([host_inputs[i][0] for i in g]) for g in groups]
+    Uks_np = [np.ascontiguousarray(np.stack([host_inputs[i][1] for i in g])) for g in groups]
+    Uks_d = [harness.to_device([u], dev)[0] for u in Uks_np]
 
     def step():
-        for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
-            ctx.set_k(k, Uk_d)
-            ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
+        if kb == 1:
+            for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
+                ctx.set_k(k, Uk_d)
+                ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
+            return
+        for g, ks, Uk_d in zip(groups, ks_np, Uks_d):
+            ctx.set_k_batch(ks, Uk_d)
+            for j, i in enumerate(g):
+                ctx.select_k(j)
+                q_d, Ukq_d, ev_d, om_d = dev_inputs[i][2]
+                ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
 
     def barrier():
         if dist is not None:
@@ -279,8 +299,13 @@ def run_ours(args):
         kernels[kind] = {"ms_total": ms / prof_steps, "launches_per_step": n // prof_steps, "avg_ms": ms / n}
     n_k = len(dev_inputs)
     # algorithmic work per LAUNCH of each kernel
+    gemm_launches = max(1, kernels.get("setk_gemm", {}).get("launches_per_step", 1))
+    gemm_flop = counts["setk_stream_flop"] * n_k / gemm_launches
+    gemm_alu = gemm_flop / (FP64_PEAK_TFLOPS * 1e12) > counts["setk_stream_bytes"] / (hbm_peak * 1e9)
     per_launch = {
         "setk_stream": ("hbm", counts["setk_stream_bytes"]),
+        # multi-k a1: g_W read once per launch, nk_b x the flops; bound = whichever floor is higher
+        "setk_gemm": ("alu", gemm_flop) if gemm_alu else ("hbm", counts["setk_stream_bytes"]),
         "contract": ("alu", counts["contract_flop"] * n_k / max(1, kernels.get("contract", {}).get("launches_per_step", 1))),
         "rotate_epilogue": ("alu", counts["rotate_flop"] * n_k / max(1, kernels.get("rotate_epilogue", {}).get("launches_per_step", 1))),
     }
@@ -312,14 +337,23 @@ def run_ours(args):
     for k, Uk, (q, Ukq, ev, om) in host_inputs:
         pin = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (Uk, q, Ukq, ev, om)]
         pinned.append((k, pin))
+    Uks_pin = [torch.from_numpy(u).pin_memory() for u in Uks_np]
     out_host = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory()
     h2d = sum(sum(t.numel() * t.element_size() for t in pin) + 24 for _, pin in pinned)
     d2h = len(pinned) * out_host.numel() * 8
 
     def step_e2e():
-        for k, (Uk_p, q_p, Ukq_p, ev_p, om_p) in pinned:
-            ctx.set_k_host(k, Uk_p.numpy())
-            ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
+        if kb == 1:
+            for k, (Uk_p, q_p, Ukq_p, ev_p, om_p) in pinned:
+                ctx.set_k_host(k, Uk_p.numpy())
+                ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
+            return
+        for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
+            ctx.set_k_batch_host(ks, Uk_p.numpy())
+            for j, i in enumerate(g):
+                ctx.select_k(j)
+                _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
+                ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
 
     e2e_steps = max(1, min(args.steps, 3))
     step_e2e()
@@ -344,7 +378,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": _config_dict(w, world),
+            "config": _with_kbatch(_config_dict(w, world), kb),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps},
@@ -371,6 +405,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(wl.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--k-batch", type=int, default=16,
+                    help="k-points per pass over g_W (phoebe_elph_set_k_batch); 1 = one set_k per k")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

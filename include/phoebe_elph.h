@@ -56,6 +56,7 @@ typedef struct phoebe_elph_ctx phoebe_elph_ctx;     /* opaque, library-owned */
  * q-points ever passed to one q_batch call. */
 typedef struct {
     int32_t nRe, nRp, nw, nmodes, nb1_max, nb2_max, nq_max;
+    int32_t nk_max;   /* most k-points per phoebe_elph_set_k_batch (0 or 1 = single-k only; <= 32) */
 } phoebe_elph_dims;
 
 /* Kernel kinds, for launch counts and profiling. */
@@ -65,7 +66,8 @@ enum {
     PHOEBE_ELPH_K_QPHASE      = 2,  /* a3: phases e^{2 pi i q.Rp}/deg_p                    */
     PHOEBE_ELPH_K_CONTRACT    = 3,  /* a4: Rp contraction (complex FP64 GEMM, DMMA)        */
     PHOEBE_ELPH_K_ROTATE_EPI  = 4,  /* a5-a7: U_kq^dagger, phonon rotation, |.|^2/(2 omega) */
-    PHOEBE_ELPH_K_COUNT       = 5
+    PHOEBE_ELPH_K_SETK_GEMM   = 5,  /* a1 for a batch of k: one pass over g_W (FP64 GEMM, DMMA) */
+    PHOEBE_ELPH_K_COUNT       = 6
 };
 
 /* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
@@ -108,6 +110,22 @@ int phoebe_elph_set_k(phoebe_elph_ctx* ctx, const double* k_host, const void* Uk
  * may be reused when the call returns only if it is pageable -- for pinned memory
  * keep it valid until the stream has passed the copy). */
 int phoebe_elph_set_k_host(phoebe_elph_ctx* ctx, const double* k_host, const void* Uk_host, int32_t nb1);
+
+/* Steps a1 + a2 for a BATCH of k-points in one pass over g_W.  Eq. 71 (L570) is
+ * "precomputed at fixed k" once per k, which re-reads all of g_W (0.5 flop/byte) for every k; here the
+ * Fourier sum over Re of nk k-points is one [nk x nRe].[nRe x nw*nw*nmodes] complex GEMM per phonon
+ * vector, so g_W is read once per batch.  Results are identical to nk set_k calls up to rounding order.
+ *   nk <= dims.nk_max;  k_host HOST [nk][3] (read before returning);
+ *   Uk_dev DEVICE complex128 [nk][nw][nb1] (same nb1 for the whole batch).
+ * The g1' of all nk k-points stay in the context; q_batch uses the one chosen by
+ * phoebe_elph_select_k (index 0 right after this call).  A later set_k overwrites slot 0.
+ * Errors: E_NULL, E_DIMS, E_ALIGN, E_CUDA. */
+int phoebe_elph_set_k_batch(phoebe_elph_ctx* ctx, int32_t nk, const double* k_host, const void* Uk_dev, int32_t nb1);
+int phoebe_elph_set_k_batch_host(phoebe_elph_ctx* ctx, int32_t nk, const double* k_host, const void* Uk_host, int32_t nb1);
+
+/* Make the g1' of k-point i (0 <= i < nk of the last set_k_batch) the one q_batch uses.  Host-side only.
+ * Errors: E_NULL, E_NO_K, E_DIMS. */
+int phoebe_elph_select_k(phoebe_elph_ctx* ctx, int32_t i);
 
 /* Steps a3..a7, rest of Eq. 70 + Eq. 7, for nq q-points at the k of the last set_k:
  *   C[q][b1][w2][kappa] = sum_p (e^{2 pi i q.Rp_p}/deg_p[p]) g1'[p][b1][w2][kappa]

@@ -14,11 +14,12 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libphoebe_elph.so")
 
-KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue"]
+KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm"]
 
 #: every symbol declared in include/phoebe_elph.h
 EXPORTS = [
     "phoebe_elph_workspace_bytes", "phoebe_elph_setup", "phoebe_elph_set_k", "phoebe_elph_set_k_host",
+    "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_copy_g1", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
@@ -29,7 +30,10 @@ ERRORS = {0: "OK", -1: "E_NULL", -2: "E_DIMS", -3: "E_ALIGN", -4: "E_NO_K", -5: 
 
 
 class Dims(ctypes.Structure):
-    _fields_ = [(n, c_int32) for n in ("nRe", "nRp", "nw", "nmodes", "nb1_max", "nb2_max", "nq_max")]
+    _fields_ = [(n, c_int32) for n in ("nRe", "nRp", "nw", "nmodes", "nb1_max", "nb2_max", "nq_max", "nk_max")]
+
+    def __init__(self, nRe=0, nRp=0, nw=0, nmodes=0, nb1_max=0, nb2_max=0, nq_max=0, nk_max=0):
+        super().__init__(nRe, nRp, nw, nmodes, nb1_max, nb2_max, nq_max, nk_max)
 
 
 class PhoebeElphError(RuntimeError):
@@ -55,6 +59,9 @@ def load_library() -> ctypes.CDLL:
                                       POINTER(Dims), c_void_p, c_size_t, c_void_p]
     lib.phoebe_elph_set_k.argtypes = [c_void_p, c_void_p, c_void_p, c_int32]
     lib.phoebe_elph_set_k_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32]
+    lib.phoebe_elph_set_k_batch.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_int32]
+    lib.phoebe_elph_set_k_batch_host.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_int32]
+    lib.phoebe_elph_select_k.argtypes = [c_void_p, c_int32]
     lib.phoebe_elph_q_batch.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
@@ -103,7 +110,7 @@ class ElphContext:
     those of the ``*_host`` entry points are NumPy arrays (or pinned CPU tensors).
     """
 
-    def __init__(self, gW, Re, Rp, deg_e=None, deg_p=None, *, nb1_max=None, nb2_max=None, nq_max,
+    def __init__(self, gW, Re, Rp, deg_e=None, deg_p=None, *, nb1_max=None, nb2_max=None, nq_max, nk_max=0,
                  hbm_budget_bytes=None, stream=None):
         import numpy as np
         import torch
@@ -114,7 +121,7 @@ class ElphContext:
         assert gW.is_cuda and gW.dtype == torch.complex128 and gW.is_contiguous() and gW.dim() == 5
         nRp, nRe, nw, nw2, nm = gW.shape
         assert nw == nw2
-        self.dims = Dims(nRe, nRp, nw, nm, nb1_max or nw, nb2_max or nw, nq_max)
+        self.dims = Dims(nRe, nRp, nw, nm, nb1_max or nw, nb2_max or nw, nq_max, nk_max)
         self._gW = gW
         self._torch = torch
         self.device = gW.device
@@ -175,6 +182,30 @@ class ElphContext:
         self._check(self._lib.phoebe_elph_set_k_host(self._ctx, k.ctypes.data, Uk.ctypes.data, nb1),
                     "phoebe_elph_set_k_host")
         self.nb1 = nb1
+
+    def set_k_batch(self, k, Uk):
+        """k: [nk][3] floats (host); Uk: CUDA complex128 tensor [nk][nw][nb1].  One pass over g_W."""
+        import numpy as np
+        k = np.ascontiguousarray(k, dtype=np.float64)
+        assert k.ndim == 2 and k.shape[1] == 3 and Uk.is_cuda and Uk.is_contiguous() and Uk.dim() == 3
+        assert Uk.shape[0] == k.shape[0]
+        nb1 = Uk.shape[2]
+        self._check(self._lib.phoebe_elph_set_k_batch(self._ctx, k.shape[0], k.ctypes.data, Uk.data_ptr(), nb1),
+                    "phoebe_elph_set_k_batch")
+        self.nb1 = nb1
+
+    def set_k_batch_host(self, k, Uk):
+        import numpy as np
+        k = np.ascontiguousarray(k, dtype=np.float64)
+        Uk = np.ascontiguousarray(Uk, dtype=np.complex128)
+        assert k.ndim == 2 and k.shape[1] == 3 and Uk.ndim == 3 and Uk.shape[0] == k.shape[0]
+        nb1 = Uk.shape[2]
+        self._check(self._lib.phoebe_elph_set_k_batch_host(self._ctx, k.shape[0], k.ctypes.data, Uk.ctypes.data, nb1),
+                    "phoebe_elph_set_k_batch_host")
+        self.nb1 = nb1
+
+    def select_k(self, i: int):
+        self._check(self._lib.phoebe_elph_select_k(self._ctx, int(i)), "phoebe_elph_select_k")
 
     def q_batch(self, q, Ukq, ev, omega, out=None):
         """All CUDA tensors: q [nq][3] f64, Ukq [nq][nw][nb2] c128, ev [nq][nm][nm] c128, omega [nq][nm] f64.

@@ -20,7 +20,8 @@ namespace {
 constexpr int kSMs = 148;                 // B200
 constexpr size_t kAlign = 256;
 constexpr int kQPad = 128;                // q columns of Pt are padded to this (largest BM)
-constexpr int kBNMax = 128;               // over-read slack behind g1' (largest BN)
+constexpr int kKBatchMax = 32;            // most k-points per set_k_batch (largest BM of the a1 GEMM)
+constexpr size_t kCBytesCap = 9000000000ull;   // C + Pt of one q sub-batch (whole batch whenever it fits)
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 int ceil_div(int a, int b) { return (a + b - 1) / b; }
@@ -45,16 +46,17 @@ int setk_auto_split(int nRe, int nRp, int X)
 
 // ---- workspace layout ---------------------------------------------------------
 struct Layout {
-    int Kpad = 0, ldq = 0, nq_sub = 0, S_alloc = 0;
-    size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_Tpart = 0, off_g1 = 0, off_Pt = 0,
-           off_C = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+    int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
+    size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
+    size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
+           off_g1 = 0, off_Pt = 0, off_C = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
 };
 
 int default_nq_sub(const phoebe_elph_dims& d, int nq_max)
 {
     const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
-    const size_t per_q = 16 * (N + (size_t)d.nRp);
-    long n = (long)((64ull << 20) / per_q);
+    const size_t per_q = 16 * (N + (size_t)d.nRp + 4);
+    long n = (long)(kCBytesCap / per_q);
     n = n / kQPad * kQPad;
     n = std::max<long>(n, kQPad);
     n = std::min<long>(n, (long)align_up((size_t)nq_max, kQPad));
@@ -67,6 +69,9 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     const size_t X = (size_t)d.nw * d.nw * d.nmodes;
     const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
     L.Kpad = (int)align_up((size_t)d.nRp, 4);
+    L.KpadE = (int)align_up((size_t)d.nRe, 4);
+    L.nk_slots = std::max(1, d.nk_max);
+    L.g1_stride = align_up((size_t)d.nRp * N, 16);
     L.nq_sub = default_nq_sub(d, nq_max);
     L.ldq = L.nq_sub;
     const int S_auto = setk_auto_split(d.nRe, d.nRp, (int)X);
@@ -78,9 +83,11 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_Rp = take((size_t)d.nRp * 3 * 8);
     L.off_dege = take((size_t)d.nRe * 8);
     L.off_degp = take((size_t)d.nRp * 8);
-    L.off_Uk = take((size_t)d.nw * d.nb1_max * 16);
-    L.off_Tpart = take((size_t)L.S_alloc * d.nRp * X * 16);
-    L.off_g1 = take(((size_t)L.Kpad * N + kBNMax) * 16);
+    L.off_Uk = take((size_t)L.nk_slots * d.nw * d.nb1_max * 16);
+    L.off_kdev = take((size_t)kKBatchMax * 3 * 8);
+    L.off_Ptk = take((size_t)L.KpadE * kKBatchMax * 16);
+    L.off_Tpart = take((size_t)std::max(L.S_alloc, L.nk_slots) * d.nRp * X * 16);
+    L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_C = take((size_t)L.nq_sub * N * 16);
     // staging for the host-buffer entry points
@@ -98,6 +105,7 @@ bool dims_ok(const phoebe_elph_dims* d, bool need_nq)
     if (d->nRe <= 0 || d->nRp <= 0 || d->nw <= 0 || d->nmodes <= 0) return false;
     if (d->nb1_max <= 0 || d->nb1_max > d->nw || d->nb2_max <= 0 || d->nb2_max > d->nw) return false;
     if (d->nq_max < 0 || (need_nq && d->nq_max == 0)) return false;
+    if (d->nk_max < 0 || d->nk_max > kKBatchMax) return false;
     if (d->nRp > 65535) return false;                       // grid.z / grid.y limits of the kernels
     if ((long)d->nw * d->nw * d->nmodes > (1L << 24)) return false;
     return true;
@@ -115,11 +123,13 @@ struct phoebe_elph_ctx {
     size_t ws_bytes = 0;
     Layout L;
     double *Re = nullptr, *Rp = nullptr, *deg_e = nullptr, *deg_p = nullptr;
-    double2 *Uk = nullptr, *Tpart = nullptr, *g1 = nullptr, *Pt = nullptr, *C = nullptr;
+    double *kdev = nullptr;
+    double2 *Uk = nullptr, *Ptk = nullptr, *Tpart = nullptr, *g1_base = nullptr, *g1 = nullptr, *Pt = nullptr, *C = nullptr;
     int nb1 = 0;
+    int nk_have = 0;        // k slots filled by the last set_k / set_k_batch
     bool have_k = false;
     int nq_sub = 0, s_split = 0;
-    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0};
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0};
     bool prof = false;
     std::vector<EventPair> evs;
     std::vector<cudaEvent_t> ev_pool;
@@ -165,9 +175,13 @@ struct LaunchScope {          // counts the launch and, when profiling, brackets
     ~LaunchScope() { if (b) cudaEventRecord(b, c->stream); }
 };
 
-// ---- contraction launcher -------------------------------------------------------
+// ---- batched complex GEMM launcher (a4 and multi-k a1) ------------------------------
+struct GemmArgs {
+    const double2* At; int lda; const double2* B; int ldb; long long strideB;
+    double2* C; long long ldc; long long strideC; int M, N, K, Kpad, batch;
+};
 template <int BM, int BN, int WM, int WN, int KC, int ST>
-cudaError_t launch_contract(phoebe_elph_ctx* c, int nq, int N)
+cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g)
 {
     using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
     auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST>;
@@ -177,15 +191,36 @@ cudaError_t launch_contract(phoebe_elph_ctx* c, int nq, int N)
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    dim3 grid(ceil_div(N, BN), ceil_div(nq, BM));
-    kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, c->stream>>>(c->Pt, c->L.ldq, c->g1, N, c->C, N, nq, N, c->L.Kpad);
+    dim3 grid(ceil_div(g.N, BN), ceil_div(g.M, BM), g.batch);
+    kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(g.At, g.lda, g.B, g.ldb, g.strideB, g.C, g.ldc, g.strideC,
+                                                           g.M, g.N, g.K, g.Kpad);
     return cudaGetLastError();
+}
+
+int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double2* Uk_dev, int nb1, double2* g1)
+{
+    const phoebe_elph_dims& d = c->dims;
+    const int Y = d.nw * d.nmodes, N = nb1 * Y;
+    LaunchScope ls(c, PHOEBE_ELPH_K_SETK_ROTATE);
+    const int TR = 128;
+    if (nb1 <= 4) {
+        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 4));
+        pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+    } else if (nb1 <= 8) {
+        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 8));
+        pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+    } else {
+        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 16));
+        pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+    }
+    PE_CUDA(c, cudaGetLastError());
+    return PHOEBE_ELPH_OK;
 }
 
 int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb1)
 {
     const phoebe_elph_dims& d = c->dims;
-    const int X = d.nw * d.nw * d.nmodes, Y = d.nw * d.nmodes, N = nb1 * Y;
+    const int X = d.nw * d.nw * d.nmodes;
     const int T = setk_threads(X);
     int S = c->s_split > 0 ? c->s_split : setk_auto_split(d.nRe, d.nRp, X);
     S = std::min(S, c->L.S_alloc);
@@ -198,28 +233,46 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
                                                                     d.nRp, X, epc, c->Tpart);
         PE_CUDA(c, cudaGetLastError());
     }
-    // zero the K-padding rows of g1' for this N (rows nRp..Kpad-1)
-    if (c->L.Kpad > d.nRp)
-        PE_CUDA(c, cudaMemsetAsync(c->g1 + (size_t)d.nRp * N, 0, (size_t)(c->L.Kpad - d.nRp) * N * 16, c->stream));
+    int rc = launch_setk_rotate(c, c->Tpart, S, Uk_dev, nb1, c->g1_base);
+    if (rc) return rc;
+    c->nb1 = nb1;
+    c->nk_have = 1;
+    c->g1 = c->g1_base;
+    c->have_k = true;
+    return PHOEBE_ELPH_OK;
+}
+
+// a1 for a batch of k-points in ONE pass over g_W: per phonon vector p a
+// [nk x nRe].[nRe x X] complex GEMM on the FP64 tensor cores, then a2 per k.
+int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const double2* Uk_dev, int nb1)
+{
+    const phoebe_elph_dims& d = c->dims;
+    const int X = d.nw * d.nw * d.nmodes;
+    PE_CUDA(c, cudaMemcpyAsync(c->kdev, k_host, (size_t)nk * 24, cudaMemcpyHostToDevice, c->stream));
     {
-        LaunchScope ls(c, PHOEBE_ELPH_K_SETK_ROTATE);
-        const int TR = 128;
-        if (nb1 <= 4) {
-            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 4));
-            pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y, nb1,
-                                                                                 c->g1, N);
-        } else if (nb1 <= 8) {
-            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 8));
-            pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y, nb1,
-                                                                                 c->g1, N);
-        } else {
-            dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 16));
-            pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(c->Tpart, Uk_dev, S, d.nRp, d.nw, Y,
-                                                                                   nb1, c->g1, N);
-        }
+        LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
+        dim3 grid(1, std::min(c->L.KpadE, 256));
+        pe::k_qphase<<<grid, 32, 0, c->stream>>>(c->kdev, c->Re, c->deg_e, nk, d.nRe, c->L.KpadE, kKBatchMax, c->Ptk);
         PE_CUDA(c, cudaGetLastError());
     }
+    {
+        LaunchScope ls(c, PHOEBE_ELPH_K_SETK_GEMM);
+        GemmArgs g{c->Ptk, kKBatchMax, c->gW, X, (long long)d.nRe * X, c->Tpart, (long long)d.nRp * X, (long long)X,
+                   nk, X, d.nRe, c->L.KpadE, d.nRp};
+        cudaError_t e;
+        if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4>(c->stream, g);
+        else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4>(c->stream, g);
+        else e = launch_contract<32, 128, 1, 4, 8, 4>(c->stream, g);
+        PE_CUDA(c, e);
+    }
+    for (int i = 0; i < nk; ++i) {
+        int rc = launch_setk_rotate(c, c->Tpart + (size_t)i * d.nRp * X, 1, Uk_dev + (size_t)i * d.nw * nb1, nb1,
+                                    c->g1_base + (size_t)i * c->L.g1_stride);
+        if (rc) return rc;
+    }
     c->nb1 = nb1;
+    c->nk_have = nk;
+    c->g1 = c->g1_base;
     c->have_k = true;
     return PHOEBE_ELPH_OK;
 }
@@ -256,7 +309,8 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_CONTRACT);
-            PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3>(c, nqs, N)));
+            GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, (long long)N, 0, nqs, N, d.nRp, c->L.Kpad, 1};
+            PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3>(c->stream, g)));
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
@@ -327,7 +381,10 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     c->deg_p = reinterpret_cast<double*>(c->ws + L.off_degp);
     c->Uk = reinterpret_cast<double2*>(c->ws + L.off_Uk);
     c->Tpart = reinterpret_cast<double2*>(c->ws + L.off_Tpart);
-    c->g1 = reinterpret_cast<double2*>(c->ws + L.off_g1);
+    c->g1_base = reinterpret_cast<double2*>(c->ws + L.off_g1);
+    c->g1 = c->g1_base;
+    c->kdev = reinterpret_cast<double*>(c->ws + L.off_kdev);
+    c->Ptk = reinterpret_cast<double2*>(c->ws + L.off_Ptk);
     c->Pt = reinterpret_cast<double2*>(c->ws + L.off_Pt);
     c->C = reinterpret_cast<double2*>(c->ws + L.off_C);
 
@@ -340,7 +397,6 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     up(c->Rp, Rp_host, (size_t)dims->nRp * 24);
     up(c->deg_e, deg_e_host ? deg_e_host : ones.data(), (size_t)dims->nRe * 8);
     up(c->deg_p, deg_p_host ? deg_p_host : ones.data(), (size_t)dims->nRp * 8);
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->g1, 0, L.off_Pt - L.off_g1, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { delete c; return PHOEBE_ELPH_E_CUDA; }
     *ctx_out = c;
@@ -363,6 +419,35 @@ int phoebe_elph_set_k_host(phoebe_elph_ctx* c, const double* k_host, const void*
     if (nb1 <= 0 || nb1 > c->dims.nb1_max) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_host: nb1 out of range");
     PE_CUDA(c, cudaMemcpyAsync(c->Uk, Uk_host, (size_t)c->dims.nw * nb1 * 16, cudaMemcpyHostToDevice, c->stream));
     return run_set_k(c, k_host, c->Uk, nb1);
+}
+
+int phoebe_elph_set_k_batch(phoebe_elph_ctx* c, int32_t nk, const double* k_host, const void* Uk_dev, int32_t nb1)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!k_host || !Uk_dev) return fail(c, PHOEBE_ELPH_E_NULL, "set_k_batch: null pointer");
+    if (nk <= 0 || nk > c->L.nk_slots) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_batch: nk out of range (dims.nk_max)");
+    if (nb1 <= 0 || nb1 > c->dims.nb1_max) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_batch: nb1 out of range");
+    if (!aligned16(Uk_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "set_k_batch: Uk not 16-byte aligned");
+    return run_set_k_batch(c, nk, k_host, static_cast<const double2*>(Uk_dev), nb1);
+}
+
+int phoebe_elph_set_k_batch_host(phoebe_elph_ctx* c, int32_t nk, const double* k_host, const void* Uk_host, int32_t nb1)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!k_host || !Uk_host) return fail(c, PHOEBE_ELPH_E_NULL, "set_k_batch_host: null pointer");
+    if (nk <= 0 || nk > c->L.nk_slots) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_batch_host: nk out of range (dims.nk_max)");
+    if (nb1 <= 0 || nb1 > c->dims.nb1_max) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k_batch_host: nb1 out of range");
+    PE_CUDA(c, cudaMemcpyAsync(c->Uk, Uk_host, (size_t)nk * c->dims.nw * nb1 * 16, cudaMemcpyHostToDevice, c->stream));
+    return run_set_k_batch(c, nk, k_host, c->Uk, nb1);
+}
+
+int phoebe_elph_select_k(phoebe_elph_ctx* c, int32_t i)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "select_k before set_k / set_k_batch");
+    if (i < 0 || i >= c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "select_k: index out of range");
+    c->g1 = c->g1_base + (size_t)i * c->L.g1_stride;
+    return PHOEBE_ELPH_OK;
 }
 
 int phoebe_elph_q_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_dev, const void* Ukq_dev,

@@ -38,13 +38,21 @@ k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------
-// a4: C[q][n] = sum_k Pt[k][q] * B[k][n]   (complex128, K = Kpad rows, zero padded)
+// a4 (and the multi-k form of a1): batched complex128 GEMM on the FP64 tensor cores
+//     C_z[m][n] = sum_{k<K} At[k][m] * B_z[k][n]          z = blockIdx.z
+// At is [Kpad][lda] (k-major, rows K..Kpad-1 and columns >= M zero), shared by all z;
+// B_z = B + z*strideB is [K][ldb] (k-major); C_z = C + z*strideC is [M][ldc].
+//   a4:  At = Pt (phases of the q batch), B = g1' (K = nRp, N = nb1*nw*nm), C = C[q][n]
+//   a1:  At = phases of a k batch, B_z = g_W[p=z] (K = nRe, N = nw*nw*nm), C_z = T[k][p][x]
 //
-// Warp-specialised: one producer warp streams [KC x BM] tiles of Pt and [KC x BN]
-// tiles of g1' into a STAGES-deep shared-memory ring with TMA 1-D bulk copies
+// Warp-specialised: one producer warp streams [KC x BM] tiles of At and [KC x BN]
+// tiles of B into a STAGES-deep shared-memory ring with TMA 1-D bulk copies
 // (one per tile row, completion on an mbarrier); WARPS_M x WARPS_N consumer warps
 // run FP64 tensor-core tiles (mma.sync m8n8k4 -> SASS DMMA.8x8x4):
-//     Cr += Pr*Br + (-Pi)*Bi ,   Ci += Pr*Bi + Pi*Br          (4 DMMA per 8x8 complex tile per k4)
+//     Cr += Ar*Br + (-Ai)*Bi ,   Ci += Ar*Bi + Ai*Br          (4 DMMA per 8x8 complex tile per k4)
+// Only valid data are copied (rows < K, columns < N); the ring is zeroed once so
+// that what the padded k-steps / ragged columns read is finite and multiplies
+// into discarded outputs or against the zero rows of At.
 // Shared rows are padded by 2 complex so that the per-lane fragment loads
 // (LDS.128 at [k0+t][.. + g]) are bank-conflict free.
 // ---------------------------------------------------------------------------
@@ -56,16 +64,16 @@ struct ContractCfg {
     static constexpr int TN = BN / WARPS_N / 8;
     static constexpr int LDA = BM + 2;     // complex elements per shared row
     static constexpr int LDB = BN + 2;
-    static constexpr size_t kSmemBytes =
-        (size_t)STAGES * KC * (LDA + LDB) * sizeof(double2) + 2 * STAGES * sizeof(uint64_t);
+    static constexpr size_t kRingBytes = (size_t)STAGES * KC * (LDA + LDB) * sizeof(double2);
+    static constexpr size_t kSmemBytes = kRingBytes + 2 * STAGES * sizeof(uint64_t);
     static_assert(BM % (WARPS_M * 8) == 0 && BN % (WARPS_N * 8) == 0, "tile/warp mismatch");
     static_assert(KC % 4 == 0 && KC <= 32, "KC rows are issued by the 32 producer lanes");
 };
 
 template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES>
 __global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32)
-k_contract(const double2* __restrict__ Pt, int ldq, const double2* __restrict__ B, int ldb,
-           double2* __restrict__ C, int ldc, int nq, int N, int Kpad)
+k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ B, int ldb, long long strideB,
+           double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad)
 {
     using Cfg = ContractCfg<BM, BN, WARPS_M, WARPS_N, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, LDA = Cfg::LDA, LDB = Cfg::LDB;
@@ -76,32 +84,40 @@ k_contract(const double2* __restrict__ Pt, int ldq, const double2* __restrict__ 
     uint64_t* empty = full + STAGES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * BN, q0 = blockIdx.y * BM;
+    const int n0 = blockIdx.x * BN, m0 = blockIdx.y * BM;
+    B += (size_t)blockIdx.z * strideB;
+    C += (size_t)blockIdx.z * strideC;
+    for (int i = threadIdx.x; i < (int)(Cfg::kRingBytes / sizeof(double2)); i += Cfg::kThreads)
+        As[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, Cfg::kConsumerWarps); }
         mbar_fence_init();
     }
+    fence_proxy_async();      // generic-proxy zero fill ordered before the async-proxy (TMA) writes
     __syncthreads();
     const int nchunks = (Kpad + KC - 1) / KC;
 
     if (warp == Cfg::kConsumerWarps) {
         // ---------------- producer warp ----------------
-        const double2* a_src = Pt + q0;
+        const double2* a_src = At + m0;
         const double2* b_src = B + n0;
+        const int bn = min(BN, N - n0);                     // valid columns of this tile
         for (int c = 0; c < nchunks; ++c) {
             const int s = c % STAGES;
             const uint32_t use = (uint32_t)(c / STAGES);
             mbar_wait(empty + s, (use & 1u) ^ 1u);
             const int k0 = c * KC;
-            const int rows = min(KC, Kpad - k0);
-            if (lane == 0) mbar_arrive_expect_tx(full + s, (uint32_t)(rows * (BM + BN) * sizeof(double2)));
+            const int rows_a = min(KC, Kpad - k0);
+            const int rows_b = max(0, min(KC, K - k0));
+            if (lane == 0)
+                mbar_arrive_expect_tx(full + s, (uint32_t)((rows_a * BM + rows_b * bn) * sizeof(double2)));
             __syncwarp();
-            if (lane < rows) {
-                bulk_g2s(As + ((size_t)s * KC + lane) * LDA, a_src + (size_t)(k0 + lane) * ldq,
+            if (lane < rows_a)
+                bulk_g2s(As + ((size_t)s * KC + lane) * LDA, a_src + (size_t)(k0 + lane) * lda,
                          BM * sizeof(double2), full + s);
+            if (lane < rows_b)
                 bulk_g2s(Bs + ((size_t)s * KC + lane) * LDB, b_src + (size_t)(k0 + lane) * ldb,
-                         BN * sizeof(double2), full + s);
-            }
+                         bn * sizeof(double2), full + s);
         }
         return;
     }
@@ -150,12 +166,12 @@ k_contract(const double2* __restrict__ Pt, int ldq, const double2* __restrict__ 
     // ---------------- store C (complex interleaved) ----------------
 #pragma unroll
     for (int i = 0; i < TM; ++i) {
-        const int qq = q0 + wm * TM * 8 + i * 8 + g;
-        if (qq >= nq) continue;
+        const int mm = m0 + wm * TM * 8 + i * 8 + g;
+        if (mm >= M) continue;
 #pragma unroll
         for (int j = 0; j < TN; ++j) {
             const int n = n0 + wn * TN * 8 + j * 8 + 2 * t;
-            double2* dst = C + (size_t)qq * ldc + n;
+            double2* dst = C + (size_t)mm * ldc + n;
             if (n < N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
             if (n + 1 < N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
         }

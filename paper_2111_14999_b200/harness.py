@@ -60,10 +60,10 @@ def upload_gW(w: wl.Workload, device="cuda:0", threads: int | None = None):
 
 
 def make_context(w: wl.Workload, gW, *, nq_max=None, deg_e=None, deg_p=None, hbm_budget_bytes=None,
-                 nb1_max=None, nb2_max=None) -> binding.ElphContext:
+                 nb1_max=None, nb2_max=None, nk_max=0) -> binding.ElphContext:
     return binding.ElphContext(gW, wl.Re_vectors(w), wl.Rp_vectors(w), deg_e, deg_p,
                                nb1_max=nb1_max or w.nb1, nb2_max=nb2_max or w.nb2,
-                               nq_max=nq_max or w.nq, hbm_budget_bytes=hbm_budget_bytes)
+                               nq_max=nq_max or w.nq, nk_max=nk_max, hbm_budget_bytes=hbm_budget_bytes)
 
 
 def to_device(arrs, device="cuda:0"):
@@ -80,6 +80,7 @@ def algorithmic_counts(w: wl.Workload, nq: int | None = None):
         "setk_bytes": 16 * w.nRp * (w.nRe * X + N),
         "setk_stream_bytes": 16 * w.nRp * w.nRe * X,
         "setk_flop": 8 * w.nRp * w.nRe * X + 8 * w.nRp * w.nw * w.nb1 * Y,
+        "setk_stream_flop": 8 * w.nRp * w.nRe * X,
         # a4: 8 flop per complex MAC
         "contract_flop": 8 * nq * w.nRp * N,
         # a5-a7 per batch

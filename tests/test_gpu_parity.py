@@ -146,6 +146,71 @@ def test_band_windows_change_between_calls_and_errors(env):
     ctx.close()
 
 
+KBATCH = [
+    # nw nb1 nb2 nm  grid_e     grid_p    nk  nq
+    (3, 2, 3, 2, (5, 1, 1), (3, 1, 1), 1, 5),        # nRe = 5 (k padding), X = 18 (one ragged column tile)
+    (4, 4, 4, 3, (3, 3, 3), (2, 2, 2), 9, 40),       # BM = 16, ragged rows
+    (6, 5, 6, 4, (2, 3, 3), (3, 3, 1), 20, 33),      # BM = 32, X = 144 (128 + ragged 16)
+    (8, 8, 8, 6, (3, 3, 3), (3, 3, 3), 8, 70),       # BM = 8 exactly, X = 384 = 3 tiles
+    (5, 3, 2, 9, (4, 2, 3), (1, 1, 2), 32, 7),       # the most k a batch takes
+]
+
+
+@pytest.mark.parametrize("case", KBATCH, ids=lambda c: "nw%d_nk%d" % (c[0], c[6]))
+@pytest.mark.parametrize("host", [False, True], ids=["dev", "host"])
+def test_set_k_batch_matches_oracle_per_k(env, case, host):
+    """one pass over g_W for nk k-points == nk independent Eq. 71 precomputes."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    nw, nb1, nb2, nm, ge, gp, nk, nq = case
+    w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=ge, grid_p=gp, nk=nk, nq=nq, cfg_id=60 + nw)
+    gW_np, Re, Rp = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w)
+    rng = np.random.default_rng(nk)
+    deg_e = rng.integers(1, 4, w.nRe).astype(np.float64)
+    deg_p = rng.integers(1, 4, w.nRp).astype(np.float64)
+    ks = wl.k_points(w)
+    Uks = np.stack([wl.U_k(w, ik) for ik in range(nk)])
+    gW = torch.from_numpy(gW_np).cuda()
+    ctx = harness.make_context(w, gW, nq_max=nq, nk_max=nk, deg_e=deg_e, deg_p=deg_p)
+    if host:
+        ctx.set_k_batch_host(ks, Uks)
+    else:
+        ctx.set_k_batch(ks, harness.to_device([Uks])[0])
+    worst = 0.0
+    for ik in reversed(range(nk)):
+        ctx.select_k(ik)
+        g1 = ctx.copy_g1().cpu().numpy()
+        g1_ref = oracle.setk(gW_np, Re, deg_e, ks[ik], Uks[ik])
+        assert _relerr(g1, g1_ref) < 1e-12
+        q, Ukq, ev, om = wl.q_inputs(w, ik)
+        out = ctx.q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
+        ref = oracle.qbatch(g1_ref, Rp, deg_p, q, Ukq, ev, om)
+        worst = max(worst, _relerr(out, ref))
+    assert worst <= TOL
+    n = ctx.launch_counts()
+    assert n["setk_gemm"] == 1 and n["setk_stream"] == 0 and n["setk_rotate"] == nk
+    with pytest.raises(env["binding"].PhoebeElphError) as e:
+        ctx.select_k(nk)
+    assert e.value.code == -2
+    # a plain set_k afterwards overwrites slot 0 and is what q_batch then uses
+    ctx.set_k(ks[nk - 1], harness.to_device([Uks[nk - 1]])[0])
+    q, Ukq, ev, om = wl.q_inputs(w, nk - 1)
+    out = ctx.q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
+    ref = oracle.elph(gW_np, Re, Rp, deg_e, deg_p, ks[nk - 1], Uks[nk - 1], q, Ukq, ev, om)
+    assert _relerr(out, ref) <= TOL
+    ctx.close()
+
+
+def test_set_k_batch_needs_nk_max(env):
+    wl, torch, harness, binding = env["wl"], env["torch"], env["harness"], env["binding"]
+    w = wl.custom(nw=2, nm=3, grid_e=(3, 1, 1), nk=2, nq=4, cfg_id=61)
+    ctx = harness.make_context(w, torch.from_numpy(wl.gW_full(w)).cuda(), nq_max=4)      # nk_max = 0
+    Uks = np.stack([wl.U_k(w, i) for i in range(2)])
+    with pytest.raises(binding.PhoebeElphError) as e:
+        ctx.set_k_batch(wl.k_points(w), harness.to_device([Uks])[0])
+    assert e.value.code == -2
+    ctx.close()
+
+
 def test_periodicity_on_gpu(env):
     """Eq. 87: out(k, q+G) = out(k, q) for integer G -- a property that holds at any size."""
     wl, torch, harness = env["wl"], env["torch"], env["harness"]

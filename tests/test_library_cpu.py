@@ -58,6 +58,7 @@ def test_large_config_fits_180GB(lib):
 @pytest.mark.parametrize("bad", [
     (0, 343, 8, 6, 8, 8, 16), (343, 0, 8, 6, 8, 8, 16), (343, 343, 8, 6, 9, 8, 16),
     (343, 343, 8, 6, 8, 0, 16), (343, 343, 8, 0, 8, 8, 16), (343, 343, 8, 6, 8, 8, -1),
+    (343, 343, 8, 6, 8, 8, 16, 33), (343, 343, 8, 6, 8, 8, 16, -1),
 ])
 def test_bad_dims_rejected(lib, bad):
     with pytest.raises(binding.PhoebeElphError) as e:
