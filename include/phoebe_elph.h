@@ -165,8 +165,13 @@ int phoebe_elph_profile(phoebe_elph_ctx* ctx, int32_t enable);
 int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches);
 
 /* Tuning knobs (integers); unknown key -> E_DIMS.  Keys:
- *   "nq_sub"  q sub-batch kept L2-resident between the contraction and the rotation kernel
- *   "s_split" number of Re chunks in the set_k stream (0 = automatic)                       */
+ *   "nq_sub"    q-points per contraction / rotation launch (default: the whole batch when C fits)
+ *   "s_split"   number of Re chunks in the set_k stream (0 = automatic)
+ *   "m3"        1 (default) = three-multiply complex product in the two GEMMs (T1 = Ar.Br, T2 = Ai.Bi,
+ *               T3 = (Ar+Ai).(Br+Bi); Re = T1-T2, Im = T3-T1-T2: 6 instead of 8 real flop per complex MAC,
+ *               normwise FP64-accurate); 0 = the four-multiply product
+ *   "tile"      contraction CTA tile: 0 = automatic (cost model), 32 or 64
+ *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)           */
 int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
 int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);
 

@@ -26,6 +26,8 @@ def nvcc_cmd(verbose: bool = False):
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC",
            "-o", LIB, SRC]
+    extra = os.environ.get("PHOEBE_ELPH_NVCC_FLAGS", "").split()      # e.g. -D switches of kernel experiments
+    cmd[1:1] = extra
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     return cmd

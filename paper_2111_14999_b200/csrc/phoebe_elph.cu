@@ -129,6 +129,9 @@ struct phoebe_elph_ctx {
     int nk_have = 0;        // k slots filled by the last set_k / set_k_batch
     bool have_k = false;
     int nq_sub = 0, s_split = 0;
+    bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
+    int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
+    bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0};
     bool prof = false;
     std::vector<EventPair> evs;
@@ -180,11 +183,11 @@ struct GemmArgs {
     const double2* At; int lda; const double2* B; int ldb; long long strideB;
     double2* C; long long ldc; long long strideC; int M, N, K, Kpad, batch;
 };
-template <int BM, int BN, int WM, int WN, int KC, int ST>
+template <int BM, int BN, int WM, int WN, int KC, int ST, bool M3>
 cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g)
 {
     using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
-    auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST>;
+    auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST, M3>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
@@ -197,21 +200,28 @@ cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g)
     return cudaGetLastError();
 }
 
-int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double2* Uk_dev, int nb1, double2* g1)
+int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double2* Uk_dev, int nb1, double2* g1,
+                       int nk, long long strideT, long long strideG)
 {
     const phoebe_elph_dims& d = c->dims;
     const int Y = d.nw * d.nmodes, N = nb1 * Y;
     LaunchScope ls(c, PHOEBE_ELPH_K_SETK_ROTATE);
     const int TR = 128;
     if (nb1 <= 4) {
-        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 4));
-        pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+        const int ng = ceil_div(nb1, 4);
+        dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
+        pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N, ng,
+                                                                             strideT, strideG);
     } else if (nb1 <= 8) {
-        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 8));
-        pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+        const int ng = ceil_div(nb1, 8);
+        dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
+        pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N, ng,
+                                                                             strideT, strideG);
     } else {
-        dim3 grid(ceil_div(Y, TR), d.nRp, ceil_div(nb1, 16));
-        pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N);
+        const int ng = ceil_div(nb1, 16);
+        dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
+        pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N,
+                                                                               ng, strideT, strideG);
     }
     PE_CUDA(c, cudaGetLastError());
     return PHOEBE_ELPH_OK;
@@ -233,7 +243,7 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
                                                                     d.nRp, X, epc, c->Tpart);
         PE_CUDA(c, cudaGetLastError());
     }
-    int rc = launch_setk_rotate(c, c->Tpart, S, Uk_dev, nb1, c->g1_base);
+    int rc = launch_setk_rotate(c, c->Tpart, S, Uk_dev, nb1, c->g1_base, 1, 0, 0);
     if (rc) return rc;
     c->nb1 = nb1;
     c->nk_have = 1;
@@ -260,14 +270,20 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
         GemmArgs g{c->Ptk, kKBatchMax, c->gW, X, (long long)d.nRe * X, c->Tpart, (long long)d.nRp * X, (long long)X,
                    nk, X, d.nRe, c->L.KpadE, d.nRp};
         cudaError_t e;
-        if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4>(c->stream, g);
-        else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4>(c->stream, g);
-        else e = launch_contract<32, 128, 1, 4, 8, 4>(c->stream, g);
+        if (c->m3) {
+            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, true>(c->stream, g);
+            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, true>(c->stream, g);
+            else e = launch_contract<32, 128, 1, 8, 8, 4, true>(c->stream, g);
+        } else {
+            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, false>(c->stream, g);
+            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, false>(c->stream, g);
+            else e = launch_contract<32, 128, 1, 4, 8, 4, false>(c->stream, g);
+        }
         PE_CUDA(c, e);
     }
-    for (int i = 0; i < nk; ++i) {
-        int rc = launch_setk_rotate(c, c->Tpart + (size_t)i * d.nRp * X, 1, Uk_dev + (size_t)i * d.nw * nb1, nb1,
-                                    c->g1_base + (size_t)i * c->L.g1_stride);
+    {
+        int rc = launch_setk_rotate(c, c->Tpart, 1, Uk_dev, nb1, c->g1_base, nk, (long long)d.nRp * X,
+                                    (long long)c->L.g1_stride);
         if (rc) return rc;
     }
     c->nb1 = nb1;
@@ -283,19 +299,55 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     const phoebe_elph_dims& d = c->dims;
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
     const int nq_sub = std::min(c->nq_sub, c->L.nq_sub);
-    // rotation kernel geometry: as many b1 per CTA as fit in ~96 KB of shared memory
-    const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;
-    const size_t per_b1 = ((size_t)Y + (size_t)nb2 * d.nmodes) * 16;
-    int gb1 = (int)std::max<size_t>(1, std::min<size_t>((size_t)nb1, ((96u << 10) - std::min<size_t>(fixed, 90u << 10)) / per_b1));
-    const size_t rot_smem = fixed + per_b1 * gb1;
-    if (rot_smem > (200u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
-    static size_t rot_attr = 0;
-    if (rot_smem > (48u << 10) && rot_smem > rot_attr) {
-        PE_CUDA(c, cudaFuncSetAttribute(pe::k_rotate_epilogue, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
-        rot_attr = rot_smem;
+    // rotation kernel geometry
+    const int NT = ceil_div(d.nmodes, 8);
+    const bool use_mma = NT <= 6 && !c->rot_plain;
+    int gb1, rot_threads;
+    size_t rot_smem;
+    int QG = 1;
+    if (use_mma) {
+        const int nwp = (d.nw + 3) & ~3, MT = ceil_div(nb2, 8);
+        const size_t slack = (size_t)(4 * d.nmodes + 8) * 16;
+        const size_t fixed_q = (size_t)8 * NT * 8 + ((size_t)nwp * (MT * 8 + 2) + (size_t)8 * NT * (NT * 8 + 1)) * 16;
+        const size_t per_b1 = (size_t)Y * 16;
+        const size_t whole_q = fixed_q + per_b1 * nb1 + slack;
+        const size_t budget = 100u << 10;
+        if (whole_q <= (64u << 10)) {
+            // small cell: every b1 of a q at once, several q per CTA (amortises the CTA prologue), but keep
+            // at least ~4 CTAs per SM in the grid
+            gb1 = nb1;
+            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (64u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
+            rot_smem = 16 + whole_q * QG;
+        } else {
+            if (fixed_q + 2 * (per_b1 + slack) > (200u << 10))
+                return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+            const size_t room = budget > fixed_q + 2 * slack ? budget - fixed_q - 2 * slack : 0;
+            gb1 = (int)std::max<size_t>(1, std::min<size_t>((size_t)nb1, room / (2 * per_b1)));
+            rot_smem = 16 + fixed_q + 2 * (per_b1 * gb1 + slack);
+        }
+        rot_threads = 128;
+    } else {
+        const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;
+        const size_t per_b1 = ((size_t)Y + (size_t)nb2 * d.nmodes) * 16;
+        gb1 = (int)std::max<size_t>(1, std::min<size_t>((size_t)nb1, ((96u << 10) - std::min<size_t>(fixed, 90u << 10)) / per_b1));
+        rot_smem = fixed + per_b1 * gb1;
+        if (rot_smem > (200u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+        const int work = gb1 * nb2 * d.nmodes;
+        rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
     }
-    const int work = gb1 * nb2 * d.nmodes;
-    const int rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
+    auto rot_kernel = [&]() -> const void* {
+        if (!use_mma) return (const void*)pe::k_rotate_epilogue;
+        switch (NT) {
+            case 1: return (const void*)pe::k_rotate_epilogue_mma<1>;
+            case 2: return (const void*)pe::k_rotate_epilogue_mma<2>;
+            case 3: return (const void*)pe::k_rotate_epilogue_mma<3>;
+            case 4: return (const void*)pe::k_rotate_epilogue_mma<4>;
+            case 5: return (const void*)pe::k_rotate_epilogue_mma<5>;
+            default: return (const void*)pe::k_rotate_epilogue_mma<6>;
+        }
+    }();
+    if (rot_smem > (48u << 10))
+        PE_CUDA(c, cudaFuncSetAttribute(rot_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
 
     for (int qs = 0; qs < nq; qs += nq_sub) {
         const int nqs = std::min(nq_sub, nq - qs);
@@ -310,15 +362,36 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_CONTRACT);
             GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, (long long)N, 0, nqs, N, d.nRp, c->L.Kpad, 1};
-            PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3>(c->stream, g)));
+            // tile choice: 64x64 unless that leaves the 148 SMs with a long ragged tail (few tiles);
+            // cost model = rounds of tiles per SM x tile area (+5 % for the smaller tile's extra operand traffic)
+            const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64;
+            const double cost32 = (double)ceil_div(ceil_div(nqs, 32) * ceil_div(N, 32), kSMs) * 32 * 32 * 1.05;
+            const int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
+            if (c->m3) {
+                if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
+#ifdef EXP_M3_TILE
+                else PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true>(c->stream, g)));
+#else
+                else PE_CUDA(c, (launch_contract<64, 64, 2, 4, 16, 4, true>(c->stream, g)));
+#endif
+            } else {
+                if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, false>(c->stream, g)));
+                else PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3, false>(c->stream, g)));
+            }
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
-            dim3 grid(ceil_div(nb1, gb1), nqs);
-            pe::k_rotate_epilogue<<<grid, rot_threads, rot_smem, c->stream>>>(
-                c->C, N, Ukq + (size_t)qs * d.nw * nb2, ev + (size_t)qs * d.nmodes * d.nmodes,
-                omega + (size_t)qs * d.nmodes, out + (size_t)qs * nb1 * nb2 * d.nmodes, d.nw, d.nmodes, nb1, nb2, gb1);
-            PE_CUDA(c, cudaGetLastError());
+            dim3 grid = use_mma ? dim3(ceil_div(nqs, QG)) : dim3(ceil_div(nb1, gb1), nqs);
+            const double2* Cp = c->C; long long ldc = N; int ldc_i = N;
+            const double2* Up = Ukq + (size_t)qs * d.nw * nb2;
+            const double2* Zp = ev + (size_t)qs * d.nmodes * d.nmodes;
+            const double* wp = omega + (size_t)qs * d.nmodes;
+            double* op = out + (size_t)qs * nb1 * nb2 * d.nmodes;
+            int nw_ = d.nw, nm_ = d.nmodes, nb1_ = nb1, nb2_ = nb2, gb1_ = gb1, nqs_ = nqs, QG_ = QG;
+            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_};
+            void* args_pl[] = {&Cp, &ldc_i, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_};
+            PE_CUDA(c, cudaLaunchKernel(rot_kernel, grid, dim3(rot_threads), use_mma ? args_mma : args_pl, rot_smem,
+                                        c->stream));
         }
     }
     return PHOEBE_ELPH_OK;
@@ -542,6 +615,13 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         c->nq_sub = (int)std::min<int64_t>(value, c->L.nq_sub);
         return PHOEBE_ELPH_OK;
     }
+    if (!strcmp(key, "tile")) {
+        if (value != 0 && value != 32 && value != 64) return fail(c, PHOEBE_ELPH_E_DIMS, "tile must be 0, 32 or 64");
+        c->tile = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
+    if (!strcmp(key, "m3")) { c->m3 = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "s_split")) {
         if (value < 0 || value > c->L.S_alloc) return fail(c, PHOEBE_ELPH_E_DIMS, "s_split out of range");
         c->s_split = (int)value;
@@ -554,6 +634,7 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
 {
     if (!c || !key || !value) return PHOEBE_ELPH_E_NULL;
     if (!strcmp(key, "nq_sub")) { *value = c->nq_sub; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "m3")) { *value = c->m3 ? 1 : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "s_split")) {
         *value = c->s_split > 0 ? c->s_split
                                 : setk_auto_split(c->dims.nRe, c->dims.nRp, c->dims.nw * c->dims.nw * c->dims.nmodes);

@@ -70,7 +70,7 @@ struct ContractCfg {
     static_assert(KC % 4 == 0 && KC <= 32, "KC rows are issued by the 32 producer lanes");
 };
 
-template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES>
+template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES, bool M3>
 __global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32)
 k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ B, int ldb, long long strideB,
            double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad)
@@ -125,11 +125,18 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
     // ---------------- consumer warps ----------------
     const int wm = warp / WARPS_N, wn = warp % WARPS_N;
     const int g = lane >> 2, t = lane & 3;
-    double cr[TM][TN][2], ci[TM][TN][2];
+    // M3 = false: cr = Re C, ci = Im C (4 DMMA per tile and k-step).
+    // M3 = true : the three-multiply complex product (3 DMMA per tile and k-step):
+    //     cr = T1 = sum Ar*Br,  ci = T2 = sum Ai*Bi,  cs = T3 = sum (Ar+Ai)*(Br+Bi)
+    //     Re C = T1 - T2,  Im C = T3 - T1 - T2     (formed once, after the k loop)
+    double cr[TM][TN][2], ci[TM][TN][2], cs[M3 ? TM : 1][M3 ? TN : 1][2];
 #pragma unroll
     for (int i = 0; i < TM; ++i)
 #pragma unroll
-        for (int j = 0; j < TN; ++j) { cr[i][j][0] = cr[i][j][1] = 0.0; ci[i][j][0] = ci[i][j][1] = 0.0; }
+        for (int j = 0; j < TN; ++j) {
+            cr[i][j][0] = cr[i][j][1] = 0.0; ci[i][j][0] = ci[i][j][1] = 0.0;
+            if (M3) cs[i][j][0] = cs[i][j][1] = 0.0;
+        }
 
     for (int c = 0; c < nchunks; ++c) {
         const int s = c % STAGES;
@@ -146,21 +153,55 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
                 for (int i = 0; i < TM; ++i) a[i] = a_base[(size_t)k4 * 4 * LDA + i * 8];
 #pragma unroll
                 for (int j = 0; j < TN; ++j) b[j] = b_base[(size_t)k4 * 4 * LDB + j * 8];
+                if (M3) {
+                    double as[TM], bs[TN];
 #pragma unroll
-                for (int i = 0; i < TM; ++i) {
-                    const double npi = neg(a[i].y);
+#ifdef EXP_NO_DADD
+                    for (int i = 0; i < TM; ++i) as[i] = a[i].x;
 #pragma unroll
-                    for (int j = 0; j < TN; ++j) {
-                        dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-                        dmma884(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
-                        dmma884(cr[i][j][0], cr[i][j][1], npi, b[j].y);
-                        dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
+                    for (int j = 0; j < TN; ++j) bs[j] = b[j].x;
+#else
+                    for (int i = 0; i < TM; ++i) as[i] = a[i].x + a[i].y;
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) bs[j] = b[j].x + b[j].y;
+#endif
+#pragma unroll
+                    for (int i = 0; i < TM; ++i)
+#pragma unroll
+                        for (int j = 0; j < TN; ++j) {
+                            dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+                            dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].y);
+                            dmma884(cs[i][j][0], cs[i][j][1], as[i], bs[j]);
+                        }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < TM; ++i) {
+                        const double npi = neg(a[i].y);
+#pragma unroll
+                        for (int j = 0; j < TN; ++j) {
+                            dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
+                            dmma884(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
+                            dmma884(cr[i][j][0], cr[i][j][1], npi, b[j].y);
+                            dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
+                        }
                     }
                 }
             }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + s);
+    }
+    if (M3) {
+#pragma unroll
+        for (int i = 0; i < TM; ++i)
+#pragma unroll
+            for (int j = 0; j < TN; ++j)
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const double t1 = cr[i][j][h], t2 = ci[i][j][h];
+                    cr[i][j][h] = t1 - t2;
+                    ci[i][j][h] = cs[i][j][h] - t1 - t2;
+                }
     }
 
     // ---------------- store C (complex interleaved) ----------------
@@ -179,8 +220,141 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------
+// a5..a7 on the FP64 tensor cores, chained in registers.  A warp takes work items (q, b1, mt)
+// with mt an 8-row tile of b2:
+//   a5  D[b2][ka] = sum_w2 Uh[b2][w2] C[b1][w2][ka]      A = Uh (8x4 per k-step), B = C panel, K = nw
+//   a6  E[b2][nu] = sum_ka D[b2][ka] Z[ka][nu]            A = D straight from the a5 accumulators
+//   a7  out = |E|^2 * 1/(2 omega)
+// The DMMA accumulator of lane (g,t) holds D[g][2t], D[g][2t+1]; as the A operand of the next
+// product it must hold A[g][k-slot t].  The sum over ka may run in any order, so k-step (j,s) of
+// a6 is DEFINED to cover ka = 8j + 2t + s (t = 0..3): the accumulator registers are then the A
+// fragments as they stand and the B fragment is Z[8j + 2t + s][8n + g] -- no shuffles, no
+// shared-memory round trip.
+// Shared memory: Us[nwp][ldu] = conj(Ukq) zero padded (ldu = 2 mod 8 complex: conflict-free A
+// loads), Zs[8NT][ldz] zero padded (ldz = 1 mod 4), inv2w[8NT], Cs = the contiguous C panel of
+// a (q, b1 group) brought in by ONE TMA bulk copy, followed by zeroed slack so that the padded
+// k-steps / columns read finite values (they multiply zero rows of Us / Zs).
+// NT = ceil(nm / 8) <= 6.
+// ---------------------------------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(128)
+k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
+                      const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
+                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG)
+{
+    // One CTA = QG consecutive q-points; it walks the b1 groups (gb1 values of b1 each) with the C panels
+    // double-buffered: the TMA bulk copy of group i+1 runs while the warps do the DMMAs of group i.
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int nwp = (nw + 3) & ~3, MT = (nb2 + 7) >> 3;
+    const int ldu = MT * 8 + 2, ldz = NT * 8 + 1, Y = nw * nm;
+    const int slack = 4 * nm + 8;
+    const size_t panel = (size_t)gb1 * Y + slack;                       // complex elements of one (q, group) buffer
+    const int ngroups = (nb1 + gb1 - 1) / gb1;
+    const int nbuf = ngroups > 1 ? 2 : 1;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);                               // [2]
+    double* inv2w = reinterpret_cast<double*>(smem_raw + 16);                            // [QG][8 NT]
+    double2* Us = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)QG * 8 * NT * sizeof(double));   // [QG][nwp][ldu]
+    double2* Zs = Us + (size_t)QG * nwp * ldu;                                           // [QG][8 NT][ldz]
+    double2* Cs = Zs + (size_t)QG * 8 * NT * ldz;                                        // [nbuf][QG][panel]
+    const int q0 = blockIdx.x * QG;
+    const int nql = min(QG, nq - q0);
+    if (threadIdx.x == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); mbar_fence_init(); }
+    __syncthreads();
+    auto issue = [&](int grp) {             // thread 0: bring the C panels of group grp (all nql q-points) in
+        const int b10 = grp * gb1;
+        const int nb1l = min(gb1, nb1 - b10);
+        const uint32_t bytes = (uint32_t)((size_t)nb1l * Y * sizeof(double2));
+        uint64_t* fb = bar + (grp & 1);
+        mbar_arrive_expect_tx(fb, bytes * (uint32_t)nql);
+        for (int ql = 0; ql < nql; ++ql)
+            bulk_g2s(Cs + ((size_t)(grp & (nbuf - 1)) * QG + ql) * panel,
+                     C + (size_t)(q0 + ql) * ldc + (size_t)b10 * Y, bytes, fb);
+    };
+    if (threadIdx.x == 0) issue(0);
+    // while the first panels are in flight: conj(Ukq) -> Us, ev -> Zs, 1/(2 omega), zero padding / slack
+    for (int i = threadIdx.x; i < nql * nwp * ldu; i += blockDim.x) {
+        const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
+        const int w2 = r / ldu, b2 = r - w2 * ldu;
+        double2 u = make_double2(0.0, 0.0);
+        if (w2 < nw && b2 < nb2) { u = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2]; u.y = -u.y; }
+        Us[i] = u;
+    }
+    for (int i = threadIdx.x; i < nql * 8 * NT * ldz; i += blockDim.x) {
+        const int ql = i / (8 * NT * ldz), r = i - ql * 8 * NT * ldz;
+        const int ka = r / ldz, nu = r - ka * ldz;
+        Zs[i] = (ka < nm && nu < nm) ? ev[((size_t)(q0 + ql) * nm + ka) * nm + nu] : make_double2(0.0, 0.0);
+    }
+    for (int i = threadIdx.x; i < nql * 8 * NT; i += blockDim.x) {
+        const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
+        const double w = (nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
+        inv2w[i] = (w > 0.0) ? 0.5 / w : 0.0;
+    }
+    for (int i = threadIdx.x; i < nbuf * QG * slack; i += blockDim.x) {
+        const int bq = i / slack, r = i - bq * slack;
+        Cs[(size_t)bq * panel + (size_t)gb1 * Y + r] = make_double2(0.0, 0.0);
+    }
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const int g = lane >> 2, t = lane & 3;
+    const int nks = nwp >> 2;
+    for (int grp = 0; grp < ngroups; ++grp) {
+        __syncthreads();                    // everyone is done with the buffer group grp+1 will overwrite (and with the fills)
+        if (threadIdx.x == 0 && grp + 1 < ngroups) issue(grp + 1);
+        mbar_wait(bar + (grp & 1), (uint32_t)(grp >> 1) & 1u);
+        const int b10 = grp * gb1;
+        const int nb1l = min(gb1, nb1 - b10);
+        const int per_q = nb1l * MT;
+        for (int item = warp; item < nql * per_q; item += nwarps) {
+            const int ql = item / per_q, r = item - ql * per_q;
+            const int b1 = r / MT, mt = r - b1 * MT;
+            double dr[NT][2], di[NT][2];
+#pragma unroll
+            for (int j = 0; j < NT; ++j) { dr[j][0] = dr[j][1] = 0.0; di[j][0] = di[j][1] = 0.0; }
+            const double2* ua = Us + ((size_t)ql * nwp + t) * ldu + mt * 8 + g;
+            const double2* cb = Cs + ((size_t)(grp & (nbuf - 1)) * QG + ql) * panel + (size_t)b1 * Y + (size_t)t * nm + g;
+            for (int ks = 0; ks < nks; ++ks) {
+                const double2 a = ua[(size_t)ks * 4 * ldu];
+                const double nai = neg(a.y);
+#pragma unroll
+                for (int j = 0; j < NT; ++j) {
+                    const double2 b = cb[(size_t)ks * 4 * nm + j * 8];
+                    dmma884(dr[j][0], dr[j][1], a.x, b.x);
+                    dmma884(di[j][0], di[j][1], a.x, b.y);
+                    dmma884(dr[j][0], dr[j][1], nai, b.y);
+                    dmma884(di[j][0], di[j][1], a.y, b.x);
+                }
+            }
+            const int b2 = mt * 8 + g;
+            double* orow = out + (((size_t)(q0 + ql) * nb1 + b10 + b1) * nb2 + b2) * nm;
+            const double2* zq = Zs + (size_t)ql * 8 * NT * ldz;
+            const double* iw = inv2w + ql * 8 * NT;
+#pragma unroll 1
+            for (int n = 0; n < NT; ++n) {       // not unrolled: keeps at most 2 NT fragments of Z in registers
+                double er[2] = {0.0, 0.0}, ei[2] = {0.0, 0.0};
+#pragma unroll
+                for (int j = 0; j < NT; ++j)
+#pragma unroll
+                    for (int sl = 0; sl < 2; ++sl) {
+                        const double2 z = zq[(size_t)(8 * j + 2 * t + sl) * ldz + 8 * n + g];
+                        const double ar = dr[j][sl], ai = di[j][sl];
+                        dmma884(er[0], er[1], ar, z.x);
+                        dmma884(ei[0], ei[1], ar, z.y);
+                        dmma884(er[0], er[1], neg(ai), z.y);
+                        dmma884(ei[0], ei[1], ai, z.x);
+                    }
+                const int nu = 8 * n + 2 * t;
+                if (b2 < nb2) {
+                    if (nu < nm) orow[nu] = (er[0] * er[0] + ei[0] * ei[0]) * iw[nu];
+                    if (nu + 1 < nm) orow[nu + 1] = (er[1] * er[1] + ei[1] * ei[1]) * iw[nu + 1];
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
 // a5..a7: per (q, group of b1): rotate by conj(Ukq), by ev, square, scale.
-// First, plain shared-memory version (DFMA).
+// Plain shared-memory DFMA version: the fallback for nm > 48 (NT > 6).
 // smem: Uc[nw][nb2] (already conjugated), Z[nm][nm], Cs[gb1][nw*nm], Ds[gb1][nb2*nm]
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)

@@ -60,15 +60,22 @@ k_setk_stream(const double2* __restrict__ gW, const double* __restrict__ Re, con
     Tpart[((size_t)s * nRp + p) * (size_t)X + col] = make_double2(ar, ai);
 }
 
-// a2: one thread per (p, y), NBT values of b1 per thread (blockIdx.z picks the b1 group).
+// a2: one thread per (p, y), NBT values of b1 per thread.  blockIdx.z = ik * ngroups + (b1 group):
+// a batch of k-points (set_k_batch) is rotated by one launch; k-point ik reads Tpart + ik*strideT,
+// Uk + ik*nw*nb1 and writes g1 + ik*strideG.
 template <int NBT>
 __global__ void __launch_bounds__(128)
-k_setk_rotate(const double2* __restrict__ Tpart, const double2* __restrict__ Uk /* [nw][nb1] */,
-              int S, int nRp, int nw, int Y, int nb1, double2* __restrict__ g1 /* [nRp][nb1][Y] */, int ldg)
+k_setk_rotate(const double2* __restrict__ Tpart, const double2* __restrict__ Uk /* [nk][nw][nb1] */,
+              int S, int nRp, int nw, int Y, int nb1, double2* __restrict__ g1 /* [nk][nRp][nb1][Y] */, int ldg,
+              int ngroups, long long strideT, long long strideG)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* U = reinterpret_cast<double2*>(smem_raw);           // [nw][NBT]
-    const int b0 = blockIdx.z * NBT;
+    const int ik = blockIdx.z / ngroups;
+    const int b0 = (blockIdx.z - ik * ngroups) * NBT;
+    Tpart += (size_t)ik * strideT;
+    Uk += (size_t)ik * nw * nb1;
+    g1 += (size_t)ik * strideG;
     for (int i = threadIdx.x; i < nw * NBT; i += blockDim.x) {
         int w1 = i / NBT, b = i % NBT;
         U[i] = (b0 + b < nb1) ? Uk[(size_t)w1 * nb1 + b0 + b] : make_double2(0.0, 0.0);

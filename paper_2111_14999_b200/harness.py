@@ -71,9 +71,12 @@ def to_device(arrs, device="cuda:0"):
     return [torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in arrs]
 
 
-def algorithmic_counts(w: wl.Workload, nq: int | None = None):
-    """Algorithmic flop / byte counts of SURVEY 8(d), per k-point and per q-batch of nq."""
+def algorithmic_counts(w: wl.Workload, nq: int | None = None, m3: bool = False):
+    """Flop / byte counts of SURVEY 8(d), per k-point and per q-batch of nq.  The two GEMMs count the flops they
+    EXECUTE: 8 real flop per complex MAC with the four-multiply product, 6 with the three-multiply product (m3;
+    its few extra additions -- 2 per operand element loaded, 3 per output -- are not counted)."""
     nq = w.nq if nq is None else nq
+    fpc = 6 if m3 else 8
     X, N, Y = w.X, w.N, w.nw * w.nm
     return {
         # a1+a2: bytes = |g_W| + |g1'| ; flop = Fourier sum + rotation
@@ -81,8 +84,11 @@ def algorithmic_counts(w: wl.Workload, nq: int | None = None):
         "setk_stream_bytes": 16 * w.nRp * w.nRe * X,
         "setk_flop": 8 * w.nRp * w.nRe * X + 8 * w.nRp * w.nw * w.nb1 * Y,
         "setk_stream_flop": 8 * w.nRp * w.nRe * X,
+        "setk_gemm_flop": fpc * w.nRp * w.nRe * X,
         # a4: 8 flop per complex MAC
-        "contract_flop": 8 * nq * w.nRp * N,
+        "contract_flop": fpc * nq * w.nRp * N,
+        "contract_flop_4m": 8 * nq * w.nRp * N,
+        "flop_per_complex_mac": fpc,
         # a5-a7 per batch
         "rotate_flop": nq * (8 * w.nb1 * w.nb2 * w.nm * (w.nw + w.nm) + 4 * w.nb1 * w.nb2 * w.nm),
         "rotate_bytes": nq * (16 * N + 8 * w.nb1 * w.nb2 * w.nm + 16 * w.nw * w.nb2 + 16 * w.nm * w.nm + 8 * w.nm),

@@ -75,6 +75,10 @@ RAGGED = [
     (1, 1, 1, 1, (1, 1, 1), (1, 1, 2), 3),
     (8, 4, 4, 6, (3, 3, 3), (3, 3, 3), 200),
     (6, 6, 5, 9, (4, 3, 2), (3, 2, 5), 96),
+    (7, 7, 7, 15, (2, 2, 1), (2, 3, 1), 40),      # NT = 2, nw % 4 = 3
+    (9, 9, 10 - 1, 30, (2, 1, 1), (3, 1, 1), 20),  # NT = 4 (the "large" cell's mode count)
+    (3, 3, 3, 45, (2, 1, 1), (1, 2, 1), 6),       # NT = 6
+    (2, 2, 2, 51, (2, 1, 1), (2, 1, 1), 9),       # nm > 48: plain DFMA rotation fallback
 ]
 
 
@@ -94,6 +98,26 @@ def test_ragged_small_cases(env, case, host):
     ref = oracle.qbatch(g1_ref, a["Rp"], deg_p, a["q"], a["Ukq"], a["ev"], a["om"])
     assert out.shape == ref.shape
     assert _relerr(out, ref) <= TOL
+
+
+@pytest.mark.parametrize("knob", [{"tile": 32, "m3": 0}, {"tile": 64, "m3": 0}, {"tile": 32, "m3": 1},
+                                  {"tile": 64, "m3": 1}, {"rot_plain": 1}],
+                         ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
+def test_forced_kernel_variants(env, knob):
+    """Every kernel variant the dispatcher can pick is parity-checked on the same input."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=6, nb1=5, nb2=6, nm=9, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nq=150, cfg_id=84)
+    a = _inputs(wl, w)
+    ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=150)
+    for key, val in knob.items():
+        ctx.set_tuning(key, val)
+        if key == "m3":
+            assert ctx.get_tuning(key) == val
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    out = ctx.q_batch(*harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])).cpu().numpy()
+    assert _relerr(out, ref) <= TOL
+    ctx.close()
 
 
 def test_nonpositive_omega_and_sub_batches(env):
@@ -157,7 +181,7 @@ KBATCH = [
 
 
 @pytest.mark.parametrize("case", KBATCH, ids=lambda c: "nw%d_nk%d" % (c[0], c[6]))
-@pytest.mark.parametrize("host", [False, True], ids=["dev", "host"])
+@pytest.mark.parametrize("host", [False, True], ids=["dev_m3", "host_4m"])
 def test_set_k_batch_matches_oracle_per_k(env, case, host):
     """one pass over g_W for nk k-points == nk independent Eq. 71 precomputes."""
     wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
@@ -171,6 +195,7 @@ def test_set_k_batch_matches_oracle_per_k(env, case, host):
     Uks = np.stack([wl.U_k(w, ik) for ik in range(nk)])
     gW = torch.from_numpy(gW_np).cuda()
     ctx = harness.make_context(w, gW, nq_max=nq, nk_max=nk, deg_e=deg_e, deg_p=deg_p)
+    ctx.set_tuning("m3", 0 if host else 1)      # host leg: four-multiply product; device leg: three-multiply
     if host:
         ctx.set_k_batch_host(ks, Uks)
     else:
@@ -187,7 +212,7 @@ def test_set_k_batch_matches_oracle_per_k(env, case, host):
         worst = max(worst, _relerr(out, ref))
     assert worst <= TOL
     n = ctx.launch_counts()
-    assert n["setk_gemm"] == 1 and n["setk_stream"] == 0 and n["setk_rotate"] == nk
+    assert n["setk_gemm"] == 1 and n["setk_stream"] == 0 and n["setk_rotate"] == 1
     with pytest.raises(env["binding"].PhoebeElphError) as e:
         ctx.select_k(nk)
     assert e.value.code == -2
