@@ -234,6 +234,8 @@ def run_ours(args):
     kb = max(1, min(args.k_batch, 32, len(host_inputs)))
     ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0)
     ctx.set_tuning("m3", args.m3)
+    if args.tile:
+        ctx.set_tuning("tile", args.tile)
     out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
     # k-points grouped into batches of kb: one pass over g_W per batch (set_k_batch)
     groups = [list(range(i, min(i + kb, len(host_inputs)))) for i in range(0, len(host_inputs), kb)]
@@ -410,6 +412,7 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(wl.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--m3", type=int, default=1, help="1 = three-multiply complex product in the GEMMs (default), 0 = four")
+    ap.add_argument("--tile", type=int, default=0, help="force the contraction CTA tile (0 = automatic)")
     ap.add_argument("--k-batch", type=int, default=16,
                     help="k-points per pass over g_W (phoebe_elph_set_k_batch); 1 = one set_k per k")
     args = ap.parse_args()

@@ -105,3 +105,43 @@ def qbatch(g1, Rp, deg_p, q, Ukq, ev, omega):
 def elph(gW, Re, Rp, deg_e, deg_p, k, Uk, q, Ukq, ev, omega):
     """setk followed by qbatch (the factorised two-step form, Eq. 71 then Eq. 70)."""
     return qbatch(setk(gW, Re, deg_e, k, Uk), Rp, deg_p, q, Ukq, ev, omega)
+
+
+# ---- SURVEY 8(f) f2: linewidths from |g|^2 (Eq. 29 + Eq. 61) -------------------------------
+def _dbl(name, nargs):
+    f = getattr(_load(), name)
+    f.restype = ctypes.c_double
+    f.argtypes = [ctypes.c_double] * nargs
+    return f
+
+
+def fermi(eps, mu, kT):
+    return float(_dbl("oracle_fermi", 3)(eps, mu, kT))
+
+
+def bose(omega, kT):
+    return float(_dbl("oracle_bose", 2)(omega, kT))
+
+
+def delta_gauss(x, sigma):
+    """Eq. 61: exp(-x^2/sigma^2)/(sqrt(pi) sigma)."""
+    return float(_dbl("oracle_delta_gauss", 2)(x, sigma))
+
+
+def rate_weight(eps_kb, eps_kqb, omega, kT, mu, sigma):
+    """The square bracket of Eq. 29 for one (b, b', nu) term."""
+    return float(_dbl("oracle_rate_weight", 6)(eps_kb, eps_kqb, omega, kT, mu, sigma))
+
+
+def rates(out, eps_k, eps_kq, omega, kT, mu, sigma, pref, rate=None):
+    """rate[b1] (+)= pref * sum_{q,b2,nu} out[q][b1][b2][nu] * W   (Eq. 29 with the Gaussian delta of Eq. 61)."""
+    nq, nb1, nb2, nm = out.shape
+    out = _c(out, np.float64); eps_k = _c(eps_k, np.float64, (nb1,)); eps_kq = _c(eps_kq, np.float64, (nq, nb2))
+    omega = _c(omega, np.float64, (nq, nm))
+    rate = np.zeros(nb1) if rate is None else rate
+    assert rate.dtype == np.float64 and rate.shape == (nb1,) and rate.flags.c_contiguous
+    f = _load().oracle_rates
+    f.argtypes = [ctypes.c_int] * 4 + [ctypes.c_void_p] * 4 + [ctypes.c_double] * 4 + [ctypes.c_void_p]
+    rc = f(nq, nb1, nb2, nm, _p(out), _p(eps_k), _p(eps_kq), _p(omega), kT, mu, sigma, pref, _p(rate))
+    assert rc == 0
+    return rate

@@ -207,3 +207,60 @@ int oracle_qbatch(int nRp, int nw, int nm, int nb1, int nb2, int nq,
     }
     return rc;
 }
+
+/* ========================================================================
+ * electron linewidths from |g|^2 (Eq. 29)
+ * with the Gaussian approximation of the Dirac delta (Eq. 61).
+ *
+ *   1/tau_{k b} = (2 pi / (N_k V)) sum_{k' b' q nu} |g_{b b' nu}(k,k')|^2
+ *        [ (1 - f_{k'b'} + n_{q nu}) delta(eps_{kb} - hbar omega_{q nu} - eps_{k'b'})
+ *        + (    f_{k'b'} + n_{q nu}) delta(eps_{kb} + hbar omega_{q nu} - eps_{k'b'}) ] delta(k - k' + q)
+ *   delta(x) ~ exp(-x^2 / sigma^2) / (sqrt(pi) sigma)                              (Eq. 61)
+ *   f(eps) = 1 / (e^{(eps - mu)/k_B T} + 1)   (L212),   n(omega) = 1 / (e^{omega/k_B T} - 1)
+ *
+ * Readings (R16-R18):
+ *   R16 delta(k - k' + q) selects k' = k + q: the sum runs over the q list only; b = b1 (band at k),
+ *       b' = b2 (band at k+q), so |g_{b b' nu}|^2 = out[q][b1][b2][nu] of Eq. 7/13.
+ *   R17 the prefactor 2 pi/(N_k V) (and any unit conversion) is the caller's `pref`; hbar = 1 (R8).
+ *   R18 modes with omega <= 0 contribute nothing (their |g|^2 is 0 by R7; n is not evaluated).
+ *
+ *   rate[b1] += pref * sum_{q, b2, nu} out[q][b1][b2][nu] * W(eps_k[b1], eps_kq[q][b2], omega[q][nu])
+ *
+ * Plain loops, long double accumulation.
+ * ====================================================================== */
+double oracle_fermi(double eps, double mu, double kT) { return 1.0 / (exp((eps - mu) / kT) + 1.0); }
+
+double oracle_bose(double omega, double kT) { return 1.0 / (exp(omega / kT) - 1.0); }
+
+double oracle_delta_gauss(double x, double sigma)
+{
+    return exp(-(x * x) / (sigma * sigma)) / (sqrt(ORACLE_PI) * sigma);
+}
+
+/* the square bracket of Eq. 29 for one (b, b', nu) term */
+double oracle_rate_weight(double eps_kb, double eps_kqb, double omega, double kT, double mu, double sigma)
+{
+    if (!(omega > 0.0)) return 0.0;
+    double f = oracle_fermi(eps_kqb, mu, kT), n = oracle_bose(omega, kT);
+    return (1.0 - f + n) * oracle_delta_gauss(eps_kb - omega - eps_kqb, sigma) +
+           (f + n) * oracle_delta_gauss(eps_kb + omega - eps_kqb, sigma);
+}
+
+int oracle_rates(int nq, int nb1, int nb2, int nm, const double *out /* [nq][nb1][nb2][nm] */,
+                 const double *eps_k /* [nb1] */, const double *eps_kq /* [nq][nb2] */,
+                 const double *omega /* [nq][nm] */, double kT, double mu, double sigma, double pref,
+                 double *rate /* [nb1], accumulated into */)
+{
+    for (int b1 = 0; b1 < nb1; ++b1) {
+        long double s = 0.0L;
+        for (int iq = 0; iq < nq; ++iq)
+            for (int b2 = 0; b2 < nb2; ++b2)
+                for (int nu = 0; nu < nm; ++nu) {
+                    double w = oracle_rate_weight(eps_k[b1], eps_kq[(size_t)iq * nb2 + b2],
+                                                  omega[(size_t)iq * nm + nu], kT, mu, sigma);
+                    s += (long double)out[(((size_t)iq * nb1 + b1) * nb2 + b2) * nm + nu] * (long double)w;
+                }
+        rate[b1] += (double)((long double)pref * s);
+    }
+    return 0;
+}

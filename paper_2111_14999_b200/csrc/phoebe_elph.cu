@@ -20,6 +20,7 @@ namespace {
 constexpr int kSMs = 148;                 // B200
 constexpr size_t kAlign = 256;
 constexpr int kQPad = 128;                // q columns of Pt are padded to this (largest BM)
+constexpr int kKPad = 16;                 // phase matrices are zero padded to this many rows (largest KC)
 constexpr int kKBatchMax = 32;            // most k-points per set_k_batch (largest BM of the a1 GEMM)
 constexpr size_t kCBytesCap = 9000000000ull;   // C + Pt of one q sub-batch (whole batch whenever it fits)
 
@@ -68,8 +69,8 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     Layout L;
     const size_t X = (size_t)d.nw * d.nw * d.nmodes;
     const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
-    L.Kpad = (int)align_up((size_t)d.nRp, 4);
-    L.KpadE = (int)align_up((size_t)d.nRe, 4);
+    L.Kpad = (int)align_up((size_t)d.nRp, kKPad);     // k_contract: Kpad % KC == 0 for every KC in use
+    L.KpadE = (int)align_up((size_t)d.nRe, kKPad);
     L.nk_slots = std::max(1, d.nk_max);
     L.g1_stride = align_up((size_t)d.nRp * N, 16);
     L.nq_sub = default_nq_sub(d, nq_max);
@@ -183,20 +184,28 @@ struct GemmArgs {
     const double2* At; int lda; const double2* B; int ldb; long long strideB;
     double2* C; long long ldc; long long strideC; int M, N, K, Kpad, batch;
 };
-template <int BM, int BN, int WM, int WN, int KC, int ST, bool M3>
-cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g)
+template <int BM, int BN, int WM, int WN, int KC, int ST, bool M3, int MINB = 1>
+cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persistent = true)
 {
     using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
-    auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST, M3>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST, M3, MINB>;
+    static int ctas_per_sm = 0;          // per instantiation; set once
+    if (ctas_per_sm == 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        int nb = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, Cfg::kThreads, Cfg::kSmemBytes);
+        if (e != cudaSuccess) return e;
+        ctas_per_sm = std::max(1, nb);
     }
-    dim3 grid(ceil_div(g.N, BN), ceil_div(g.M, BM), g.batch);
+    // persistent grid: one CTA per resident slot, each walks the tile list with stride gridDim.x
+    const long long ntiles = (long long)ceil_div(g.N, BN) * ceil_div(g.M, BM) * g.batch;
+    // (the HBM-streaming multi-k a1 GEMM measured faster with one tile per CTA: the next CTA's prologue keeps
+    //  loads in flight while this one stores; it passes persistent = false)
+    if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int grid = persistent ? (int)std::min<long long>(ntiles, (long long)kSMs * ctas_per_sm) : (int)ntiles;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(g.At, g.lda, g.B, g.ldb, g.strideB, g.C, g.ldc, g.strideC,
-                                                           g.M, g.N, g.K, g.Kpad);
+                                                           g.M, g.N, g.K, g.Kpad, g.batch);
     return cudaGetLastError();
 }
 
@@ -271,13 +280,13 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
                    nk, X, d.nRe, c->L.KpadE, d.nRp};
         cudaError_t e;
         if (c->m3) {
-            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, true>(c->stream, g);
-            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, true>(c->stream, g);
-            else e = launch_contract<32, 128, 1, 8, 8, 4, true>(c->stream, g);
+            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, true>(c->stream, g, false);
+            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, true>(c->stream, g, false);
+            else e = launch_contract<32, 128, 1, 8, 8, 4, true>(c->stream, g, false);
         } else {
-            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, false>(c->stream, g);
-            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, false>(c->stream, g);
-            else e = launch_contract<32, 128, 1, 4, 8, 4, false>(c->stream, g);
+            if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, false>(c->stream, g, false);
+            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, false>(c->stream, g, false);
+            else e = launch_contract<32, 128, 1, 4, 8, 4, false>(c->stream, g, false);
         }
         PE_CUDA(c, e);
     }
@@ -369,14 +378,11 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             const int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
             if (c->m3) {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
-#ifdef EXP_M3_TILE
-                else PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true>(c->stream, g)));
-#else
+                else if (tile == 6432) PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true, 2>(c->stream, g)));
                 else PE_CUDA(c, (launch_contract<64, 64, 2, 4, 16, 4, true>(c->stream, g)));
-#endif
             } else {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, false>(c->stream, g)));
-                else PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3, false>(c->stream, g)));
+                else PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3, false, 2>(c->stream, g)));
             }
         }
         {
@@ -616,7 +622,8 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "tile")) {
-        if (value != 0 && value != 32 && value != 64) return fail(c, PHOEBE_ELPH_E_DIMS, "tile must be 0, 32 or 64");
+        if (value != 0 && value != 32 && value != 64 && value != 6432)
+            return fail(c, PHOEBE_ELPH_E_DIMS, "tile must be 0, 32, 64 or 6432");
         c->tile = (int)value;
         return PHOEBE_ELPH_OK;
     }

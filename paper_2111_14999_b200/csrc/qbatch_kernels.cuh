@@ -40,7 +40,7 @@ k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ 
 // ---------------------------------------------------------------------------
 // a4 (and the multi-k form of a1): batched complex128 GEMM on the FP64 tensor cores
 //     C_z[m][n] = sum_{k<K} At[k][m] * B_z[k][n]          z = blockIdx.z
-// At is [Kpad][lda] (k-major, rows K..Kpad-1 and columns >= M zero), shared by all z;
+// At is [Kpad][lda] (k-major, Kpad a multiple of KC, rows K..Kpad-1 and columns >= M zero), shared by all z;
 // B_z = B + z*strideB is [K][ldb] (k-major); C_z = C + z*strideC is [M][ldc].
 //   a4:  At = Pt (phases of the q batch), B = g1' (K = nRp, N = nb1*nw*nm), C = C[q][n]
 //   a1:  At = phases of a k batch, B_z = g_W[p=z] (K = nRe, N = nw*nw*nm), C_z = T[k][p][x]
@@ -70,10 +70,10 @@ struct ContractCfg {
     static_assert(KC % 4 == 0 && KC <= 32, "KC rows are issued by the 32 producer lanes");
 };
 
-template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES, bool M3>
-__global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32)
+template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES, bool M3, int MINB = 1>
+__global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32, MINB)
 k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ B, int ldb, long long strideB,
-           double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad)
+           double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad, int nbatch)
 {
     using Cfg = ContractCfg<BM, BN, WARPS_M, WARPS_N, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, LDA = Cfg::LDA, LDB = Cfg::LDB;
@@ -84,9 +84,6 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
     uint64_t* empty = full + STAGES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * BN, m0 = blockIdx.y * BM;
-    B += (size_t)blockIdx.z * strideB;
-    C += (size_t)blockIdx.z * strideC;
     for (int i = threadIdx.x; i < (int)(Cfg::kRingBytes / sizeof(double2)); i += Cfg::kThreads)
         As[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
@@ -95,29 +92,38 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
     }
     fence_proxy_async();      // generic-proxy zero fill ordered before the async-proxy (TMA) writes
     __syncthreads();
-    const int nchunks = (Kpad + KC - 1) / KC;
+    const int nchunks = Kpad / KC;          // host contract: Kpad % KC == 0, rows K..Kpad-1 of At are zero
+    // PERSISTENT: the CTA walks tiles blockIdx.x, blockIdx.x + gridDim.x, ... (n fastest, then m, then batch z);
+    // the ring and its barrier phases run on across tile boundaries, so the producer is already filling the
+    // stages of the next tile while the consumers store C -- no per-tile prologue, no pipeline drain.
+    const int ntn = (N + BN - 1) / BN, ntm = (M + BM - 1) / BM;
+    const long long ntiles = (long long)ntn * ntm * nbatch;
 
     if (warp == Cfg::kConsumerWarps) {
         // ---------------- producer warp ----------------
-        const double2* a_src = At + m0;
-        const double2* b_src = B + n0;
-        const int bn = min(BN, N - n0);                     // valid columns of this tile
-        for (int c = 0; c < nchunks; ++c) {
-            const int s = c % STAGES;
-            const uint32_t use = (uint32_t)(c / STAGES);
-            mbar_wait(empty + s, (use & 1u) ^ 1u);
-            const int k0 = c * KC;
-            const int rows_a = min(KC, Kpad - k0);
-            const int rows_b = max(0, min(KC, K - k0));
-            if (lane == 0)
-                mbar_arrive_expect_tx(full + s, (uint32_t)((rows_a * BM + rows_b * bn) * sizeof(double2)));
-            __syncwarp();
-            if (lane < rows_a)
-                bulk_g2s(As + ((size_t)s * KC + lane) * LDA, a_src + (size_t)(k0 + lane) * lda,
-                         BM * sizeof(double2), full + s);
-            if (lane < rows_b)
-                bulk_g2s(Bs + ((size_t)s * KC + lane) * LDB, b_src + (size_t)(k0 + lane) * ldb,
-                         bn * sizeof(double2), full + s);
+        int s = 0; uint32_t ph = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int tn = (int)(tile % ntn), tm = (int)((tile / ntn) % ntm);
+            const long long z = tile / ((long long)ntn * ntm);
+            const int n0 = tn * BN, m0 = tm * BM;
+            const double2* a_src = At + m0;
+            const double2* b_src = B + (size_t)z * strideB + n0;
+            const int bn = min(BN, N - n0);                     // valid columns of this tile
+            for (int c = 0; c < nchunks; ++c) {
+                mbar_wait(empty + s, ph ^ 1u);
+                const int k0 = c * KC;
+                const int rows_b = max(0, min(KC, K - k0));
+                if (lane == 0)
+                    mbar_arrive_expect_tx(full + s, (uint32_t)((KC * BM + rows_b * bn) * sizeof(double2)));
+                __syncwarp();
+                if (lane < KC)
+                    bulk_g2s(As + ((size_t)s * KC + lane) * LDA, a_src + (size_t)(k0 + lane) * lda,
+                             BM * sizeof(double2), full + s);
+                if (lane < rows_b)
+                    bulk_g2s(Bs + ((size_t)s * KC + lane) * LDB, b_src + (size_t)(k0 + lane) * ldb,
+                             bn * sizeof(double2), full + s);
+                if (++s == STAGES) { s = 0; ph ^= 1u; }
+            }
         }
         return;
     }
@@ -129,6 +135,12 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
     // M3 = true : the three-multiply complex product (3 DMMA per tile and k-step):
     //     cr = T1 = sum Ar*Br,  ci = T2 = sum Ai*Bi,  cs = T3 = sum (Ar+Ai)*(Br+Bi)
     //     Re C = T1 - T2,  Im C = T3 - T1 - T2     (formed once, after the k loop)
+    constexpr int KS = KC / 4;
+    int s = 0; uint32_t ph = 0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int tn = (int)(tile % ntn), tm = (int)((tile / ntn) % ntm);
+    const long long z = tile / ((long long)ntn * ntm);
+    const int n0 = tn * BN, m0 = tm * BM;
     double cr[TM][TN][2], ci[TM][TN][2], cs[M3 ? TM : 1][M3 ? TN : 1][2];
 #pragma unroll
     for (int i = 0; i < TM; ++i)
@@ -138,58 +150,58 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
             if (M3) cs[i][j][0] = cs[i][j][1] = 0.0;
         }
 
+    // Kpad is a multiple of KC (host contract): every chunk has KC/4 full k-steps, so the k-step loop is
+    // straight-line code.  Fragments are double-buffered in registers: the LDS.128 of k-step k4+1 are issued
+    // before the DMMAs of k-step k4, so their latency hides behind 3*TM*TN (or 4*TM*TN) tensor instructions.
     for (int c = 0; c < nchunks; ++c) {
-        const int s = c % STAGES;
-        const uint32_t use = (uint32_t)(c / STAGES);
-        mbar_wait(full + s, use & 1u);
-        const int rows = min(KC, Kpad - c * KC);
+        mbar_wait(full + s, ph);
         const double2* a_base = As + ((size_t)s * KC + t) * LDA + wm * TM * 8 + g;
         const double2* b_base = Bs + ((size_t)s * KC + t) * LDB + wn * TN * 8 + g;
+        double2 a[2][TM], b[2][TN];
 #pragma unroll
-        for (int k4 = 0; k4 < KC / 4; ++k4) {
-            if (k4 * 4 < rows) {
-                double2 a[TM], b[TN];
+        for (int i = 0; i < TM; ++i) a[0][i] = a_base[i * 8];
 #pragma unroll
-                for (int i = 0; i < TM; ++i) a[i] = a_base[(size_t)k4 * 4 * LDA + i * 8];
+        for (int j = 0; j < TN; ++j) b[0][j] = b_base[j * 8];
 #pragma unroll
-                for (int j = 0; j < TN; ++j) b[j] = b_base[(size_t)k4 * 4 * LDB + j * 8];
-                if (M3) {
-                    double as[TM], bs[TN];
+        for (int k4 = 0; k4 < KS; ++k4) {
+            const int cur = k4 & 1, nxt = cur ^ 1;
+            if (k4 + 1 < KS) {
 #pragma unroll
-#ifdef EXP_NO_DADD
-                    for (int i = 0; i < TM; ++i) as[i] = a[i].x;
+                for (int i = 0; i < TM; ++i) a[nxt][i] = a_base[(size_t)(k4 + 1) * 4 * LDA + i * 8];
 #pragma unroll
-                    for (int j = 0; j < TN; ++j) bs[j] = b[j].x;
-#else
-                    for (int i = 0; i < TM; ++i) as[i] = a[i].x + a[i].y;
+                for (int j = 0; j < TN; ++j) b[nxt][j] = b_base[(size_t)(k4 + 1) * 4 * LDB + j * 8];
+            }
+            if (M3) {
+                double as[TM], bs[TN];
 #pragma unroll
-                    for (int j = 0; j < TN; ++j) bs[j] = b[j].x + b[j].y;
-#endif
+                for (int i = 0; i < TM; ++i) as[i] = a[cur][i].x + a[cur][i].y;
 #pragma unroll
-                    for (int i = 0; i < TM; ++i)
+                for (int j = 0; j < TN; ++j) bs[j] = b[cur][j].x + b[cur][j].y;
 #pragma unroll
-                        for (int j = 0; j < TN; ++j) {
-                            dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-                            dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].y);
-                            dmma884(cs[i][j][0], cs[i][j][1], as[i], bs[j]);
-                        }
-                } else {
+                for (int i = 0; i < TM; ++i)
 #pragma unroll
-                    for (int i = 0; i < TM; ++i) {
-                        const double npi = neg(a[i].y);
+                    for (int j = 0; j < TN; ++j) {
+                        dmma884(cr[i][j][0], cr[i][j][1], a[cur][i].x, b[cur][j].x);
+                        dmma884(ci[i][j][0], ci[i][j][1], a[cur][i].y, b[cur][j].y);
+                        dmma884(cs[i][j][0], cs[i][j][1], as[i], bs[j]);
+                    }
+            } else {
 #pragma unroll
-                        for (int j = 0; j < TN; ++j) {
-                            dmma884(cr[i][j][0], cr[i][j][1], a[i].x, b[j].x);
-                            dmma884(ci[i][j][0], ci[i][j][1], a[i].x, b[j].y);
-                            dmma884(cr[i][j][0], cr[i][j][1], npi, b[j].y);
-                            dmma884(ci[i][j][0], ci[i][j][1], a[i].y, b[j].x);
-                        }
+                for (int i = 0; i < TM; ++i) {
+                    const double npi = neg(a[cur][i].y);
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) {
+                        dmma884(cr[i][j][0], cr[i][j][1], a[cur][i].x, b[cur][j].x);
+                        dmma884(ci[i][j][0], ci[i][j][1], a[cur][i].x, b[cur][j].y);
+                        dmma884(cr[i][j][0], cr[i][j][1], npi, b[cur][j].y);
+                        dmma884(ci[i][j][0], ci[i][j][1], a[cur][i].y, b[cur][j].x);
                     }
                 }
             }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + s);
+        if (++s == STAGES) { s = 0; ph ^= 1u; }
     }
     if (M3) {
 #pragma unroll
@@ -212,11 +224,12 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
 #pragma unroll
         for (int j = 0; j < TN; ++j) {
             const int n = n0 + wn * TN * 8 + j * 8 + 2 * t;
-            double2* dst = C + (size_t)mm * ldc + n;
+            double2* dst = C + (size_t)z * strideC + (size_t)mm * ldc + n;
             if (n < N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
             if (n + 1 < N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
         }
     }
+    }   // tile loop
 }
 
 // ---------------------------------------------------------------------------

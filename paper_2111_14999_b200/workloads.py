@@ -220,3 +220,20 @@ def sample_indices(n: int, count: int, seed: int = 12345) -> np.ndarray:
     subsets at full size; covers every tile position with high probability)."""
     count = min(count, n)
     return np.sort(np.random.default_rng(seed).permutation(n)[:count])
+
+
+# ---- inputs of the fused linewidth accumulation (SURVEY 8(f) f2; PAPER.md Eq. 29, Eq. 61) ----------
+_T_EPS_K, _T_EPS_KQ = 7, 8
+
+#: k_B T (300 K in eV), chemical potential, Gaussian smearing sigma (Eq. 61), prefactor 2 pi/(N_k V) of Eq. 29.
+#: Energies are in eV-like units on the scale of omega (0.005 .. 0.06) so that both delta functions of
+#: Eq. 29 have support inside the band window.
+RATE_PARAMS = dict(kT=0.02585, mu=0.0, sigma=0.012, pref=2.0 * np.pi / 4096.0)
+
+
+def band_energies(w: Workload, ik: int = 0):
+    """(eps_k [nb1], eps_kq [nq][nb2]): band energies at k and at every k+q, iid uniform in
+    [-0.15, 0.15) around mu = 0 (a band window a few phonon energies wide)."""
+    eps_k = _rng(w, _T_EPS_K, ik).uniform(-0.15, 0.15, w.nb1)
+    eps_kq = _rng(w, _T_EPS_KQ, ik).uniform(-0.15, 0.15, (w.nq, w.nb2))
+    return eps_k, eps_kq
