@@ -344,22 +344,31 @@ def run_ours(args):
         pin = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (Uk, q, Ukq, ev, om)]
         pinned.append((k, pin))
     Uks_pin = [torch.from_numpy(u).pin_memory() for u in Uks_np]
-    out_host = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory()
+    out_hosts = [torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory() for _ in range(2)]
+    out_host = out_hosts[0]
     h2d = sum(sum(t.numel() * t.element_size() for t in pin) + 24 for _, pin in pinned)
     d2h = len(pinned) * out_host.numel() * 8
 
     def step_e2e():
-        if kb == 1:
-            for k, (Uk_p, q_p, Ukq_p, ev_p, om_p) in pinned:
-                ctx.set_k_host(k, Uk_p.numpy())
-                ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
-            return
+        # every k-point: inputs host->device, |g|^2 device->host (into two alternating pinned buffers, as a consumer
+        # that reads batch n while batch n+1 is computed would hold them); phoebe_elph_q_batch_host_async overlaps the
+        # copies with the kernels; the step ends when the last result is on the host (phoebe_elph_wait)
+        n = 0
         for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
-            ctx.set_k_batch_host(ks, Uk_p.numpy())
+            if kb == 1:
+                ctx.set_k_host(ks[0], Uk_p.numpy()[0])
+            else:
+                ctx.set_k_batch_host(ks, Uk_p.numpy())
             for j, i in enumerate(g):
                 ctx.select_k(j)
                 _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
-                ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
+                if args.e2e_sync:
+                    ctx.q_batch_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), out_host.numpy())
+                else:
+                    ctx.q_batch_host_async(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(),
+                                           out_hosts[n & 1].numpy())
+                n += 1
+        ctx.wait()
 
     e2e_steps = max(1, min(args.steps, 3))
     step_e2e()
@@ -372,6 +381,64 @@ def run_ours(args):
     barrier()
     ms_e2e = maxreduce(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3))
     e2e_value = pairs_per_step_all * e2e_steps / (ms_e2e * 1e-3)
+
+    # ---- the same pass with the linewidth sum (Eq. 29) fused in, |g|^2 never stored ----
+    rates = None
+    if not args.no_rates:
+        P = wl.RATE_PARAMS
+        eps_np = [wl.band_energies(w, ik) for ik in k_ids]
+        eps_d = [harness.to_device([e1, e2], dev) for e1, e2 in eps_np]
+        rate_d = torch.zeros((len(dev_inputs), w.nb1), dtype=torch.float64, device=dev)
+
+        def step_rates():
+            for g, ks, Uk_d in zip(groups, ks_np, Uks_d):
+                if kb == 1:
+                    ctx.set_k(ks[0], Uk_d[0])
+                else:
+                    ctx.set_k_batch(ks, Uk_d)
+                for j, i in enumerate(g):
+                    ctx.select_k(j)
+                    q_d, Ukq_d, ev_d, om_d = dev_inputs[i][2]
+                    ctx.q_batch_rates(q_d, Ukq_d, ev_d, om_d, eps_d[i][0], eps_d[i][1], rate_d[i], **P)
+
+        step_rates()
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            step_rates()
+        e1.record()
+        barrier()
+        ms_r = maxreduce(e0.elapsed_time(e1))
+        eps_pin = [[torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in e] for e in eps_np]
+        rate_h = np.zeros((len(dev_inputs), w.nb1))
+
+        def step_rates_e2e():
+            for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
+                if kb == 1:
+                    ctx.set_k_host(ks[0], Uk_p.numpy()[0])
+                else:
+                    ctx.set_k_batch_host(ks, Uk_p.numpy())
+                for j, i in enumerate(g):
+                    ctx.select_k(j)
+                    _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
+                    ctx.q_batch_rates_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), eps_pin[i][0].numpy(),
+                                           eps_pin[i][1].numpy(), rate_h[i], **P)
+
+        step_rates_e2e()
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(e2e_steps):
+            step_rates_e2e()
+        e1.record()
+        barrier()
+        ms_re = maxreduce(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3))
+        rates = {"what": "same pass with phoebe_elph_q_batch_rates: Eq. 29 linewidth sum fused into the |g|^2 epilogue, "
+                         "|g|^2 not stored; the result per k-point is nb1 doubles",
+                 "value": pairs_per_step_all * args.steps / (ms_r * 1e-3), "unit": UNIT,
+                 "e2e": {"value": pairs_per_step_all * e2e_steps / (ms_re * 1e-3), "unit": UNIT,
+                         "h2d_bytes_per_step": int(h2d + sum(a.numel() * 8 for e in eps_pin for a in e)),
+                         "d2h_bytes_per_step": int(len(pinned) * w.nb1 * 8)}}
 
     # ---- CPU baseline: the oracle on the host cores (rank 0, N=1 only) ----------
     cpu_baseline = None
@@ -387,12 +454,13 @@ def run_ours(args):
             "config": _with_kbatch(_config_dict(w, world), kb),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "steps": e2e_steps},
+                    "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else "q_batch_host_async + wait"},
             "gpu_launches": int(gpu_launches),
             "roofline": roofline,
             "kernels": kernels,
             "fp64_probe": fp64_probe,
             "cpu_baseline": cpu_baseline,
+            "rates_fused": rates,
             "fp64_tflops_whole_path_4m_equivalent": (counts["setk_flop"] + counts["contract_flop_4m"] + counts["rotate_flop"]) * w.nk * world
             * args.steps / (ms_total * 1e-3) / 1e12,
             "input_gen_s": round(t_gen, 1),
@@ -411,6 +479,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(wl.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-sync", action="store_true", help="end-to-end leg with the synchronous q_batch_host (no copy/compute overlap)")
+    ap.add_argument("--no-rates", action="store_true", help="skip the extra fused-linewidth (f2) measurement")
     ap.add_argument("--m3", type=int, default=1, help="1 = three-multiply complex product in the GEMMs (default), 0 = four")
     ap.add_argument("--tile", type=int, default=0, help="force the contraction CTA tile (0 = automatic)")
     ap.add_argument("--k-batch", type=int, default=16,

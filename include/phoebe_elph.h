@@ -67,7 +67,8 @@ enum {
     PHOEBE_ELPH_K_CONTRACT    = 3,  /* a4: Rp contraction (complex FP64 GEMM, DMMA)        */
     PHOEBE_ELPH_K_ROTATE_EPI  = 4,  /* a5-a7: U_kq^dagger, phonon rotation, |.|^2/(2 omega) */
     PHOEBE_ELPH_K_SETK_GEMM   = 5,  /* a1 for a batch of k: one pass over g_W (FP64 GEMM, DMMA) */
-    PHOEBE_ELPH_K_COUNT       = 6
+    PHOEBE_ELPH_K_RATE_REDUCE = 6,  /* f2: fixed-order sum of the per-CTA linewidth partials    */
+    PHOEBE_ELPH_K_COUNT       = 7
 };
 
 /* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
@@ -148,6 +149,49 @@ int phoebe_elph_q_batch(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
 int phoebe_elph_q_batch_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
                              const double* q_host, const void* Ukq_host, const void* ev_host,
                              const double* omega_host, double* out_host);
+
+/* Pipelined form of q_batch_host (the paper moves every batch of |g|^2 back to the CPU, L556 / L707; here the
+ * copies overlap the kernels): enqueues the four host->device copies on a copy-in stream, the batch on the
+ * compute stream and the device->host copy of out on a copy-out stream, chained by events, over two staging
+ * slots inside the workspace, and RETURNS WITHOUT WAITING -- the copy-in of batch n+1 and the copy-out of
+ * batch n-1 run while batch n computes.  The host buffers must be page-locked (cudaHostAlloc / pinned) for
+ * the overlap and must stay valid and unmodified (inputs) / unread (out_host) until phoebe_elph_wait returns;
+ * with pageable memory the copies are staged by the driver and the call degrades to q_batch_host's ordering.
+ * set_k / set_k_batch / select_k may be called between batches (they are ordered on the compute stream).
+ * Errors: as q_batch_host. */
+int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                                   const double* q_host, const void* Ukq_host, const void* ev_host,
+                                   const double* omega_host, double* out_host);
+
+/* Blocks until every batch enqueued by q_batch_host_async has been copied out (and the compute stream is idle).
+ * Errors: E_NULL, E_CUDA. */
+int phoebe_elph_wait(phoebe_elph_ctx* ctx);
+
+/* q_batch with the linewidth sum fused into the |g|^2 epilogue (no |g|^2 round trip
+ * to the host; the paper does this sum on the CPU, L556 / L707).  Eq. 29 (L229) with the Gaussian delta
+ * of Eq. 61 (L437), delta(k-k'+q) resolved by k' = k+q, hbar = 1:
+ *   rate[b1] += pref * sum_{q<nq, b2<nb2, nu<nmodes} out[q][b1][b2][nu] *
+ *               [ (1 - f(eps_kq[q][b2]) + n(omega[q][nu])) d(eps_k[b1] - omega[q][nu] - eps_kq[q][b2])
+ *               + (    f(eps_kq[q][b2]) + n(omega[q][nu])) d(eps_k[b1] + omega[q][nu] - eps_kq[q][b2]) ]
+ *   f(e) = 1/(exp((e - mu)/kT) + 1),  n(w) = 1/(exp(w/kT) - 1),  d(x) = exp(-x^2/sigma^2)/(sqrt(pi) sigma);
+ *   terms with omega <= 0 contribute nothing.  `pref` carries the paper's 2 pi/(N_k V) and any unit factor.
+ *   eps_k_dev DEVICE [nb1] band energies at k; eps_kq_dev DEVICE [nq][nb2] band energies at k+q;
+ *   rate_dev DEVICE [nb1], ACCUMULATED INTO (the caller zeroes it before the first batch of a k-point);
+ *   out_dev as in q_batch, or NULL: |g|^2 is then not stored at all.
+ * The sum runs in a fixed order: results are bit-reproducible for a given batch split.
+ * Errors: as q_batch, plus E_DIMS when kT <= 0 or sigma <= 0. */
+typedef struct { double kT, mu, sigma, pref; } phoebe_elph_rate_params;
+int phoebe_elph_q_batch_rates(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                              const double* q_dev, const void* Ukq_dev, const void* ev_dev, const double* omega_dev,
+                              const double* eps_k_dev, const double* eps_kq_dev, const phoebe_elph_rate_params* prm,
+                              double* rate_dev, double* out_dev);
+
+/* Same with HOST buffers (rate_host [nb1] is read, accumulated into and written back; out_host may be
+ * NULL, and then only nb1 doubles come back); SYNCHRONISES the stream before returning. */
+int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                                   const double* q_host, const void* Ukq_host, const void* ev_host,
+                                   const double* omega_host, const double* eps_k_host, const double* eps_kq_host,
+                                   const phoebe_elph_rate_params* prm, double* rate_host, double* out_host);
 
 /* Copy the current g1' (complex128 [nRp][nb1][nw][nmodes]) to dst_dev (DEVICE, >= bytes
  * nRp*nb1*nw*nmodes*16); for tests of set_k on its own.  Errors: E_NULL, E_NO_K, E_WORKSPACE, E_CUDA. */

@@ -14,13 +14,15 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libphoebe_elph.so")
 
-KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm"]
+KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm", "rate_reduce"]
 
 #: every symbol declared in include/phoebe_elph.h
 EXPORTS = [
     "phoebe_elph_workspace_bytes", "phoebe_elph_setup", "phoebe_elph_set_k", "phoebe_elph_set_k_host",
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
-    "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_copy_g1", "phoebe_elph_launch_counts",
+    "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
+    "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
+    "phoebe_elph_copy_g1", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
     "phoebe_elph_version",
@@ -34,6 +36,11 @@ class Dims(ctypes.Structure):
 
     def __init__(self, nRe=0, nRp=0, nw=0, nmodes=0, nb1_max=0, nb2_max=0, nq_max=0, nk_max=0):
         super().__init__(nRe, nRp, nw, nmodes, nb1_max, nb2_max, nq_max, nk_max)
+
+
+class RateParams(ctypes.Structure):
+    """phoebe_elph_rate_params: k_B T, chemical potential, Gaussian sigma (Eq. 61), prefactor of Eq. 29."""
+    _fields_ = [(n, c_double) for n in ("kT", "mu", "sigma", "pref")]
 
 
 class PhoebeElphError(RuntimeError):
@@ -64,6 +71,10 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_select_k.argtypes = [c_void_p, c_int32]
     lib.phoebe_elph_q_batch.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_q_batch_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_wait.argtypes = [c_void_p]
+    lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
+    lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.phoebe_elph_launch_counts.argtypes = [c_void_p, POINTER(c_int64)]
     lib.phoebe_elph_profile.argtypes = [c_void_p, c_int32]
@@ -231,6 +242,48 @@ class ElphContext:
                                                        ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
                     "phoebe_elph_q_batch_host")
         return out
+
+    def q_batch_host_async(self, q, Ukq, ev, omega, out):
+        """Pipelined q_batch_host: NumPy views of PINNED memory; returns at once -- call wait() before reading out."""
+        nq, nw, nb2 = Ukq.shape
+        self._check(self._lib.phoebe_elph_q_batch_host_async(self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data,
+                                                             ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
+                    "phoebe_elph_q_batch_host_async")
+        return out
+
+    def wait(self):
+        self._check(self._lib.phoebe_elph_wait(self._ctx), "phoebe_elph_wait")
+
+    def q_batch_rates(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None, store_out=False):
+        """q_batch with the linewidth sum of Eq. 29 fused in.  All CUDA tensors; eps_k [nb1],
+        eps_kq [nq][nb2], rate [nb1] f64 is ACCUMULATED INTO.  |g|^2 is stored only if `out` is given or
+        store_out=True.  Returns (rate, out-or-None)."""
+        torch = self._torch
+        nq, nw, nb2 = Ukq.shape
+        nm = self.dims.nmodes
+        for t in (q, Ukq, ev, omega, eps_k, eps_kq, rate):
+            assert t.is_cuda and t.is_contiguous()
+        assert q.shape == (nq, 3) and ev.shape == (nq, nm, nm) and omega.shape == (nq, nm)
+        assert eps_k.shape == (self.nb1,) and eps_kq.shape == (nq, nb2) and rate.shape == (self.nb1,)
+        assert eps_k.dtype == eps_kq.dtype == rate.dtype == torch.float64
+        if out is None and store_out:
+            out = torch.empty((nq, self.nb1, nb2, nm), dtype=torch.float64, device=self.device)
+        prm = RateParams(kT, mu, sigma, pref)
+        self._check(self._lib.phoebe_elph_q_batch_rates(
+            self._ctx, nq, nb2, q.data_ptr(), Ukq.data_ptr(), ev.data_ptr(), omega.data_ptr(), eps_k.data_ptr(),
+            eps_kq.data_ptr(), byref(prm), rate.data_ptr(), None if out is None else out.data_ptr()),
+            "phoebe_elph_q_batch_rates")
+        return rate, out
+
+    def q_batch_rates_host(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):
+        """NumPy arrays; rate [nb1] is accumulated into in place; synchronises before returning."""
+        nq, nw, nb2 = Ukq.shape
+        prm = RateParams(kT, mu, sigma, pref)
+        self._check(self._lib.phoebe_elph_q_batch_rates_host(
+            self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data, ev.ctypes.data, omega.ctypes.data, eps_k.ctypes.data,
+            eps_kq.ctypes.data, byref(prm), rate.ctypes.data, None if out is None else out.ctypes.data),
+            "phoebe_elph_q_batch_rates_host")
+        return rate, out
 
     def copy_g1(self):
         torch = self._torch

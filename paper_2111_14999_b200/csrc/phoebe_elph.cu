@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -50,7 +51,8 @@ struct Layout {
     int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
-           off_g1 = 0, off_Pt = 0, off_C = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_Pt = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+    size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
 int default_nq_sub(const phoebe_elph_dims& d, int nq_max)
@@ -91,12 +93,22 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_C = take((size_t)L.nq_sub * N * 16);
+    // f2: per-CTA linewidth partials [<= nq_max CTAs][nb1], staging of rate / eps_k / eps_kq for the host entry point
+    L.off_part = take((size_t)nq_max * d.nb1_max * 8);
+    L.off_rate = take((size_t)2 * d.nb1_max * 8);
+    L.off_seps = take((size_t)nq_max * d.nb2_max * 8);
     // staging for the host-buffer entry points
-    L.off_sq = take((size_t)nq_max * 3 * 8);
-    L.off_sUkq = take((size_t)nq_max * d.nw * d.nb2_max * 16);
-    L.off_sev = take((size_t)nq_max * d.nmodes * d.nmodes * 16);
-    L.off_som = take((size_t)nq_max * d.nmodes * 8);
-    L.off_sout = take((size_t)nq_max * d.nb1_max * d.nb2_max * d.nmodes * 8);
+    // (two slots each: q_batch_host_async copies batch n+1 in and batch n-1 out while batch n computes)
+    L.sz_sq = align_up((size_t)nq_max * 3 * 8, kAlign);
+    L.sz_sUkq = align_up((size_t)nq_max * d.nw * d.nb2_max * 16, kAlign);
+    L.sz_sev = align_up((size_t)nq_max * d.nmodes * d.nmodes * 16, kAlign);
+    L.sz_som = align_up((size_t)nq_max * d.nmodes * 8, kAlign);
+    L.sz_sout = align_up((size_t)nq_max * d.nb1_max * d.nb2_max * d.nmodes * 8, kAlign);
+    L.off_sq = take(2 * L.sz_sq);
+    L.off_sUkq = take(2 * L.sz_sUkq);
+    L.off_sev = take(2 * L.sz_sev);
+    L.off_som = take(2 * L.sz_som);
+    L.off_sout = take(2 * L.sz_sout);
     L.total = off;
     return L;
 }
@@ -133,7 +145,12 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
-    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0};
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+    // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+    bool async_ready = false;
+    unsigned async_n = 0;
     bool prof = false;
     std::vector<EventPair> evs;
     std::vector<cudaEvent_t> ev_pool;
@@ -302,8 +319,12 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     return PHOEBE_ELPH_OK;
 }
 
+struct RateReq {           // f2: linewidth accumulation fused into the epilogue (nullptr = plain q_batch)
+    const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate;
+};
+
 int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const double2* Ukq, const double2* ev,
-                const double* omega, double* out)
+                const double* omega, double* out, const RateReq* rr = nullptr)
 {
     const phoebe_elph_dims& d = c->dims;
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
@@ -344,17 +365,36 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const int work = gb1 * nb2 * d.nmodes;
         rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
     }
+    const bool fused_rates = rr != nullptr && use_mma;
+    if (fused_rates)       // omega, n, eps_kq, f' per q of the CTA + one row of sums per warp (follows Cs)
+        rot_smem += ((size_t)QG * (2 * 8 * NT + 2 * 8 * ceil_div(nb2, 8)) + 4 * (size_t)nb1) * 8;
+    if (rr && !use_mma && out == nullptr)      // the plain path sums from the stored |g|^2: keep it in the staging area
+        out = reinterpret_cast<double*>(c->ws + c->L.off_sout);
     auto rot_kernel = [&]() -> const void* {
         if (!use_mma) return (const void*)pe::k_rotate_epilogue;
-        switch (NT) {
-            case 1: return (const void*)pe::k_rotate_epilogue_mma<1>;
-            case 2: return (const void*)pe::k_rotate_epilogue_mma<2>;
-            case 3: return (const void*)pe::k_rotate_epilogue_mma<3>;
-            case 4: return (const void*)pe::k_rotate_epilogue_mma<4>;
-            case 5: return (const void*)pe::k_rotate_epilogue_mma<5>;
-            default: return (const void*)pe::k_rotate_epilogue_mma<6>;
+        switch (NT * 2 + (fused_rates ? 1 : 0)) {
+            case 2: return (const void*)pe::k_rotate_epilogue_mma<1, false>;
+            case 3: return (const void*)pe::k_rotate_epilogue_mma<1, true>;
+            case 4: return (const void*)pe::k_rotate_epilogue_mma<2, false>;
+            case 5: return (const void*)pe::k_rotate_epilogue_mma<2, true>;
+            case 6: return (const void*)pe::k_rotate_epilogue_mma<3, false>;
+            case 7: return (const void*)pe::k_rotate_epilogue_mma<3, true>;
+            case 8: return (const void*)pe::k_rotate_epilogue_mma<4, false>;
+            case 9: return (const void*)pe::k_rotate_epilogue_mma<4, true>;
+            case 10: return (const void*)pe::k_rotate_epilogue_mma<5, false>;
+            case 11: return (const void*)pe::k_rotate_epilogue_mma<5, true>;
+            case 12: return (const void*)pe::k_rotate_epilogue_mma<6, false>;
+            default: return (const void*)pe::k_rotate_epilogue_mma<6, true>;
         }
     }();
+    double* partial = reinterpret_cast<double*>(c->ws + c->L.off_part);
+    pe::RateArgs ra{nullptr, nullptr, 0.0, 0.0, 0.0, partial};
+    if (rr) {
+        ra.eps_k = rr->eps_k;
+        ra.inv_kT = 1.0 / rr->prm.kT;
+        ra.mu = rr->prm.mu;
+        ra.inv_sigma2 = 1.0 / (rr->prm.sigma * rr->prm.sigma);
+    }
     if (rot_smem > (48u << 10))
         PE_CUDA(c, cudaFuncSetAttribute(rot_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
 
@@ -392,18 +432,46 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             const double2* Up = Ukq + (size_t)qs * d.nw * nb2;
             const double2* Zp = ev + (size_t)qs * d.nmodes * d.nmodes;
             const double* wp = omega + (size_t)qs * d.nmodes;
-            double* op = out + (size_t)qs * nb1 * nb2 * d.nmodes;
+            double* op = out ? out + (size_t)qs * nb1 * nb2 * d.nmodes : nullptr;
             int nw_ = d.nw, nm_ = d.nmodes, nb1_ = nb1, nb2_ = nb2, gb1_ = gb1, nqs_ = nqs, QG_ = QG;
-            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_};
+            if (rr) ra.eps_kq = rr->eps_kq + (size_t)qs * nb2;
+            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_, &ra};
             void* args_pl[] = {&Cp, &ldc_i, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_};
             PE_CUDA(c, cudaLaunchKernel(rot_kernel, grid, dim3(rot_threads), use_mma ? args_mma : args_pl, rot_smem,
                                         c->stream));
+        }
+        if (rr) {
+            int nparts = ceil_div(nqs, QG);
+            if (!use_mma) {        // plain rotation path: sum from the stored |g|^2, 32 q per warp
+                const int QC = 32;
+                nparts = ceil_div(nqs, QC);
+                LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
+                pe::k_rates_from_out<<<dim3(nparts, nb1), 32, 0, c->stream>>>(
+                    out + (size_t)qs * nb1 * nb2 * d.nmodes, omega + (size_t)qs * d.nmodes, nqs, d.nmodes, nb1, nb2, QC, ra);
+                PE_CUDA(c, cudaGetLastError());
+            }
+            LaunchScope ls(c, PHOEBE_ELPH_K_RATE_REDUCE);
+            const double scale = rr->prm.pref / (sqrt(3.14159265358979323846) * rr->prm.sigma);
+            pe::k_rate_reduce<<<nb1, 256, 0, c->stream>>>(partial, nparts, nb1, scale, rr->rate);
+            PE_CUDA(c, cudaGetLastError());
         }
     }
     return PHOEBE_ELPH_OK;
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// The synchronous host entry points use staging slot 0 on the compute stream: first let the copy-out stream
+// finish with any batch q_batch_host_async still has in flight.
+int drain_async(phoebe_elph_ctx* c)
+{
+    if (c->async_ready && c->async_n > 0) {
+        PE_CUDA(c, cudaStreamSynchronize(c->stream));
+        PE_CUDA(c, cudaStreamSynchronize(c->s_out));
+        c->async_n = 0;
+    }
+    return PHOEBE_ELPH_OK;
+}
 
 }  // namespace
 
@@ -553,7 +621,7 @@ int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const 
     if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host: null pointer");
     if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nb2 out of range");
-    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    if (int rc0 = drain_async(c)) return rc0;
     const phoebe_elph_dims& d = c->dims;
     double* sq = reinterpret_cast<double*>(c->ws + c->L.off_sq);
     double2* sU = reinterpret_cast<double2*>(c->ws + c->L.off_sUkq);
@@ -567,6 +635,130 @@ int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const 
     int rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
     if (rc) return rc;
     PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->stream));
+    PE_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
+                                   const void* ev_host, const double* omega_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_host_async before set_k");
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host_async: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nb2 out of range");
+    if (!c->async_ready) {
+        PE_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+        PE_CUDA(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            PE_CUDA(c, cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming));
+            PE_CUDA(c, cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming));
+            PE_CUDA(c, cudaEventCreateWithFlags(&c->ev_out[i], cudaEventDisableTiming));
+        }
+        c->async_ready = true;
+        c->async_n = 0;
+    }
+    const phoebe_elph_dims& d = c->dims;
+    const unsigned slot = c->async_n & 1u;
+    const bool reuse = c->async_n >= 2;          // the slot has been used before: order behind its last users
+    double* sq = reinterpret_cast<double*>(c->ws + c->L.off_sq + slot * c->L.sz_sq);
+    double2* sU = reinterpret_cast<double2*>(c->ws + c->L.off_sUkq + slot * c->L.sz_sUkq);
+    double2* sZ = reinterpret_cast<double2*>(c->ws + c->L.off_sev + slot * c->L.sz_sev);
+    double* sw = reinterpret_cast<double*>(c->ws + c->L.off_som + slot * c->L.sz_som);
+    double* so = reinterpret_cast<double*>(c->ws + c->L.off_sout + slot * c->L.sz_sout);
+    // copy-in stream: the compute that last read this input slot must be done
+    if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->s_in, c->ev_done[slot], 0));
+    else {      // first use of the slot: order behind whatever the compute stream did with the staging area before
+        PE_CUDA(c, cudaEventRecord(c->ev_done[slot], c->stream));
+        PE_CUDA(c, cudaStreamWaitEvent(c->s_in, c->ev_done[slot], 0));
+    }
+    PE_CUDA(c, cudaMemcpyAsync(sq, q_host, (size_t)nq * 24, cudaMemcpyHostToDevice, c->s_in));
+    PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->s_in));
+    PE_CUDA(c, cudaMemcpyAsync(sZ, ev_host, (size_t)nq * d.nmodes * d.nmodes * 16, cudaMemcpyHostToDevice, c->s_in));
+    PE_CUDA(c, cudaMemcpyAsync(sw, omega_host, (size_t)nq * d.nmodes * 8, cudaMemcpyHostToDevice, c->s_in));
+    PE_CUDA(c, cudaEventRecord(c->ev_in[slot], c->s_in));
+    // compute stream: inputs in, and the copy-out that last read this output slot done
+    PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[slot], 0));
+    if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[slot], 0));
+    int rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
+    if (rc) return rc;
+    PE_CUDA(c, cudaEventRecord(c->ev_done[slot], c->stream));
+    // copy-out stream
+    PE_CUDA(c, cudaStreamWaitEvent(c->s_out, c->ev_done[slot], 0));
+    PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->s_out));
+    PE_CUDA(c, cudaEventRecord(c->ev_out[slot], c->s_out));
+    c->async_n++;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_wait(phoebe_elph_ctx* c)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    PE_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->async_ready) {
+        PE_CUDA(c, cudaStreamSynchronize(c->s_out));
+        // later synchronous calls use staging slot 0 on the compute stream: restart the slot bookkeeping
+        c->async_n = 0;
+    }
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_q_batch_rates(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_dev, const void* Ukq_dev,
+                              const void* ev_dev, const double* omega_dev, const double* eps_k_dev,
+                              const double* eps_kq_dev, const phoebe_elph_rate_params* prm, double* rate_dev,
+                              double* out_dev)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates before set_k");
+    if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !eps_k_dev || !eps_kq_dev || !prm || !rate_dev)
+        return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: nb2 out of range");
+    if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: kT and sigma must be > 0");
+    if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch_rates: complex input not 16-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(q_dev) | reinterpret_cast<uintptr_t>(omega_dev) | reinterpret_cast<uintptr_t>(out_dev) |
+         reinterpret_cast<uintptr_t>(eps_k_dev) | reinterpret_cast<uintptr_t>(eps_kq_dev) | reinterpret_cast<uintptr_t>(rate_dev)) & 7u)
+        return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch_rates: double array not 8-byte aligned");
+    RateReq rr{eps_k_dev, eps_kq_dev, *prm, rate_dev};
+    return run_q_batch(c, nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
+                       omega_dev, out_dev, &rr);
+}
+
+int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host,
+                                   const void* Ukq_host, const void* ev_host, const double* omega_host,
+                                   const double* eps_k_host, const double* eps_kq_host,
+                                   const phoebe_elph_rate_params* prm, double* rate_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates_host before set_k");
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !eps_k_host || !eps_kq_host || !prm || !rate_host)
+        return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_host: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: nb2 out of range");
+    if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: kT and sigma must be > 0");
+    if (int rc0 = drain_async(c)) return rc0;
+    const phoebe_elph_dims& d = c->dims;
+    double* sq = reinterpret_cast<double*>(c->ws + c->L.off_sq);
+    double2* sU = reinterpret_cast<double2*>(c->ws + c->L.off_sUkq);
+    double2* sZ = reinterpret_cast<double2*>(c->ws + c->L.off_sev);
+    double* sw = reinterpret_cast<double*>(c->ws + c->L.off_som);
+    double* so = reinterpret_cast<double*>(c->ws + c->L.off_sout);
+    double* srate = reinterpret_cast<double*>(c->ws + c->L.off_rate);
+    double* se1 = srate + d.nb1_max;
+    double* se2 = reinterpret_cast<double*>(c->ws + c->L.off_seps);
+    PE_CUDA(c, cudaMemcpyAsync(sq, q_host, (size_t)nq * 24, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sZ, ev_host, (size_t)nq * d.nmodes * d.nmodes * 16, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(sw, omega_host, (size_t)nq * d.nmodes * 8, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(srate, rate_host, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(se1, eps_k_host, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(se2, eps_kq_host, (size_t)nq * nb2 * 8, cudaMemcpyHostToDevice, c->stream));
+    RateReq rr{se1, se2, *prm, srate};
+    int rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, out_host ? so : nullptr, &rr);
+    if (rc) return rc;
+    PE_CUDA(c, cudaMemcpyAsync(rate_host, srate, (size_t)c->nb1 * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (out_host)
+        PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->stream));
     PE_CUDA(c, cudaStreamSynchronize(c->stream));
     return PHOEBE_ELPH_OK;
 }
@@ -649,6 +841,10 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "nq_sub_max")) { *value = c->L.nq_sub; return PHOEBE_ELPH_OK; }
+    // byte offsets of the C and Pt scratch areas inside the workspace (debugging aids for the tests)
+    if (!strcmp(key, "off_C")) { *value = (int64_t)c->L.off_C; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "off_Pt")) { *value = (int64_t)c->L.off_Pt; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "ldq")) { *value = c->L.ldq; return PHOEBE_ELPH_OK; }
     return PHOEBE_ELPH_E_DIMS;
 }
 
@@ -657,6 +853,10 @@ int phoebe_elph_destroy(phoebe_elph_ctx* c)
     if (!c) return PHOEBE_ELPH_E_NULL;
     for (const EventPair& p : c->evs) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    if (c->async_ready) {
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_in[i]); cudaEventDestroy(c->ev_done[i]); cudaEventDestroy(c->ev_out[i]); }
+        cudaStreamDestroy(c->s_in); cudaStreamDestroy(c->s_out);
+    }
     delete c;
     return PHOEBE_ELPH_OK;
 }

@@ -136,7 +136,8 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
     //     cr = T1 = sum Ar*Br,  ci = T2 = sum Ai*Bi,  cs = T3 = sum (Ar+Ai)*(Br+Bi)
     //     Re C = T1 - T2,  Im C = T3 - T1 - T2     (formed once, after the k loop)
     constexpr int KS = KC / 4;
-    int s = 0; uint32_t ph = 0;
+    static_assert(STAGES >= 3, "the consumer releases a stage one chunk late: needs >= 3 stages to overlap");
+    int s = 0, s_prev = -1; uint32_t ph = 0;
     for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int tn = (int)(tile % ntn), tm = (int)((tile / ntn) % ntm);
     const long long z = tile / ((long long)ntn * ntm);
@@ -199,8 +200,13 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
                 }
             }
         }
+        // Release the PREVIOUS stage, not this one: ptxas schedules the arrive right behind the ISSUE of the last
+        // LDS of the chunk (ahead of the DMMAs that consume them), and an LDS.128 still in flight then races with the
+        // producer's next bulk copy into the stage (seen on B200 as wrong A fragments in the last quarter-warp when the
+        // producer is starved and refills at once).  One chunk later every LDS of that stage has long been consumed.
         __syncwarp();
-        if (lane == 0) mbar_arrive(empty + s);
+        if (lane == 0 && s_prev >= 0) mbar_arrive(empty + s_prev);
+        s_prev = s;
         if (++s == STAGES) { s = 0; ph ^= 1u; }
     }
     if (M3) {
@@ -248,12 +254,27 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
 // a (q, b1 group) brought in by ONE TMA bulk copy, followed by zeroed slack so that the padded
 // k-steps / columns read finite values (they multiply zero rows of Us / Zs).
 // NT = ceil(nm / 8) <= 6.
+//
+// RATES = true (Eq. 29 L229 with the Gaussian delta of Eq. 61): every
+// |g|^2 value is also multiplied by the occupation/energy-conservation bracket
+//   W = (1 - f' + n) G(eps_k[b1] - omega - eps_kq[q][b2]) + (f' + n) G(eps_k[b1] + omega - eps_kq[q][b2]),
+//   G(x) = exp(-x^2/sigma^2),  f' = 1/(e^{(eps_kq - mu)/kT} + 1),  n = 1/(e^{omega/kT} - 1)
+// and summed over (q, b2, nu) of the CTA in a fixed order: partial[blockIdx.x][b1].  k_rate_reduce adds
+// the partials (fixed order) times pref/(sqrt(pi) sigma) into rate[b1].  `out` may then be nullptr
+// (|g|^2 is not stored).  The extra shared arrays (omega, n, eps_kq, f', per-warp sums) follow Cs.
 // ---------------------------------------------------------------------------
-template <int NT>
+struct RateArgs {
+    const double* eps_k;    // [nb1]
+    const double* eps_kq;   // [nq][nb2] (of this launch)
+    double inv_kT, mu, inv_sigma2;
+    double* partial;        // [gridDim.x][nb1]
+};
+
+template <int NT, bool RATES>
 __global__ void __launch_bounds__(128)
 k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
                       const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
-                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG)
+                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra)
 {
     // One CTA = QG consecutive q-points; it walks the b1 groups (gb1 values of b1 each) with the C panels
     // double-buffered: the TMA bulk copy of group i+1 runs while the warps do the DMMAs of group i.
@@ -269,6 +290,11 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
     double2* Us = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)QG * 8 * NT * sizeof(double));   // [QG][nwp][ldu]
     double2* Zs = Us + (size_t)QG * nwp * ldu;                                           // [QG][8 NT][ldz]
     double2* Cs = Zs + (size_t)QG * 8 * NT * ldz;                                        // [nbuf][QG][panel]
+    double* om_s = reinterpret_cast<double*>(Cs + (size_t)nbuf * QG * panel);            // [QG][8 NT]   (RATES only)
+    double* bose_s = om_s + QG * 8 * NT;                                                 // [QG][8 NT]
+    double* e2_s = bose_s + QG * 8 * NT;                                                 // [QG][8 MT]
+    double* f2_s = e2_s + QG * 8 * MT;                                                   // [QG][8 MT]
+    double* wsum = f2_s + QG * 8 * MT;                                                   // [4 warps][nb1]
     const int q0 = blockIdx.x * QG;
     const int nql = min(QG, nq - q0);
     if (threadIdx.x == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); mbar_fence_init(); }
@@ -306,6 +332,22 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
         const int bq = i / slack, r = i - bq * slack;
         Cs[(size_t)bq * panel + (size_t)gb1 * Y + r] = make_double2(0.0, 0.0);
     }
+    if (RATES) {
+        for (int i = threadIdx.x; i < QG * 8 * NT; i += blockDim.x) {
+            const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
+            const double w = (ql < nql && nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
+            om_s[i] = w;
+            bose_s[i] = (w > 0.0) ? 1.0 / (exp(w * ra.inv_kT) - 1.0) : 0.0;
+        }
+        for (int i = threadIdx.x; i < QG * 8 * MT; i += blockDim.x) {
+            const int ql = i / (8 * MT), b2 = i - ql * 8 * MT;
+            const bool ok = ql < nql && b2 < nb2;
+            const double e2 = ok ? ra.eps_kq[(size_t)(q0 + ql) * nb2 + b2] : 0.0;
+            e2_s[i] = e2;
+            f2_s[i] = ok ? 1.0 / (exp((e2 - ra.mu) * ra.inv_kT) + 1.0) : 0.0;
+        }
+        for (int i = threadIdx.x; i < 4 * nb1; i += blockDim.x) wsum[i] = 0.0;
+    }
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
     const int g = lane >> 2, t = lane & 3;
@@ -341,6 +383,11 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
             double* orow = out + (((size_t)(q0 + ql) * nb1 + b10 + b1) * nb2 + b2) * nm;
             const double2* zq = Zs + (size_t)ql * 8 * NT * ldz;
             const double* iw = inv2w + ql * 8 * NT;
+            double racc = 0.0, x12 = 0.0, f2 = 0.0;
+            if (RATES) {
+                x12 = ra.eps_k[b10 + b1] - e2_s[ql * 8 * MT + b2];
+                f2 = f2_s[ql * 8 * MT + b2];
+            }
 #pragma unroll 1
             for (int n = 0; n < NT; ++n) {       // not unrolled: keeps at most 2 NT fragments of Z in registers
                 double er[2] = {0.0, 0.0}, ei[2] = {0.0, 0.0};
@@ -357,12 +404,75 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
                     }
                 const int nu = 8 * n + 2 * t;
                 if (b2 < nb2) {
-                    if (nu < nm) orow[nu] = (er[0] * er[0] + ei[0] * ei[0]) * iw[nu];
-                    if (nu + 1 < nm) orow[nu + 1] = (er[1] * er[1] + ei[1] * ei[1]) * iw[nu + 1];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        if (nu + h >= nm) continue;
+                        const double v = (er[h] * er[h] + ei[h] * ei[h]) * iw[nu + h];
+                        if (!RATES || out != nullptr) orow[nu + h] = v;
+                        if (RATES) {
+                            const double w = om_s[ql * 8 * NT + nu + h], bn = bose_s[ql * 8 * NT + nu + h];
+                            const double dm = x12 - w, dp = x12 + w;
+                            const double W = (1.0 - f2 + bn) * exp(-(dm * dm) * ra.inv_sigma2) +
+                                             (f2 + bn) * exp(-(dp * dp) * ra.inv_sigma2);
+                            racc = fma(v, W, racc);
+                        }
+                    }
                 }
+            }
+            if (RATES) {            // fixed-order sum over the warp, then into this warp's own row of wsum
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) racc += __shfl_xor_sync(0xffffffffu, racc, o);
+                if (lane == 0) wsum[warp * nb1 + b10 + b1] += racc;
             }
         }
     }
+    if (RATES) {
+        __syncthreads();
+        for (int b = threadIdx.x; b < nb1; b += blockDim.x)
+            ra.partial[(size_t)blockIdx.x * nb1 + b] = ((wsum[b] + wsum[nb1 + b]) + wsum[2 * nb1 + b]) + wsum[3 * nb1 + b];
+    }
+}
+
+// Standalone form of the same sum for the plain rotation path (nm > 48): one warp per (chunk of QC
+// q-points, b1) reads the stored |g|^2 and writes partial[chunk][b1].
+__global__ void __launch_bounds__(32)
+k_rates_from_out(const double* __restrict__ outv /* [nq][nb1][nb2][nm] */, const double* __restrict__ omega, int nq,
+                 int nm, int nb1, int nb2, int QC, RateArgs ra)
+{
+    const int b1 = blockIdx.y, qa = blockIdx.x * QC, qb = min(nq, qa + QC);
+    const int per_q = nb2 * nm, lane = threadIdx.x;
+    const double e1 = ra.eps_k[b1];
+    double acc = 0.0;
+    for (int i = lane; i < (qb - qa) * per_q; i += 32) {
+        const int iq = qa + i / per_q, r = i % per_q, b2 = r / nm, nu = r - b2 * nm;
+        const double w = omega[(size_t)iq * nm + nu];
+        if (!(w > 0.0)) continue;
+        const double e2 = ra.eps_kq[(size_t)iq * nb2 + b2];
+        const double f2 = 1.0 / (exp((e2 - ra.mu) * ra.inv_kT) + 1.0), bn = 1.0 / (exp(w * ra.inv_kT) - 1.0);
+        const double dm = e1 - w - e2, dp = e1 + w - e2;
+        const double W = (1.0 - f2 + bn) * exp(-(dm * dm) * ra.inv_sigma2) + (f2 + bn) * exp(-(dp * dp) * ra.inv_sigma2);
+        acc = fma(outv[(((size_t)iq * nb1 + b1) * nb2 + b2) * nm + nu], W, acc);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) ra.partial[(size_t)blockIdx.x * nb1 + b1] = acc;
+}
+
+// rate[b1] += scale * sum_j partial[j][b1], j in a fixed (strided, then tree) order: deterministic.
+__global__ void __launch_bounds__(256)
+k_rate_reduce(const double* __restrict__ partial, int nparts, int nb1, double scale, double* __restrict__ rate)
+{
+    __shared__ double sh[256];
+    const int b1 = blockIdx.x;
+    double s = 0.0;
+    for (int j = threadIdx.x; j < nparts; j += 256) s += partial[(size_t)j * nb1 + b1];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) rate[b1] += scale * sh[0];
 }
 
 // ---------------------------------------------------------------------------

@@ -287,3 +287,40 @@ def test_band_window_three_k(env):
         worst = max(worst, _relerr(out, ref))
     assert worst <= TOL
     ctx.close()
+
+
+def test_async_pipelined_host_batches(env):
+    """q_batch_host_async: several k-points and batches in flight over the two staging slots, mixed with the
+    synchronous entry point; every batch element by element against the oracle."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=5, nb1=4, nb2=5, nm=6, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nk=3, nq=210, cfg_id=85)
+    gW_np, Re, Rp, ks = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w), wl.k_points(w)
+    ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=210, nk_max=3)
+    Uks = np.stack([wl.U_k(w, ik) for ik in range(3)])
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    ins = [[pin(x) for x in wl.q_inputs(w, ik)] for ik in range(3)]
+    refs = [oracle.elph(gW_np, Re, Rp, None, None, ks[ik], Uks[ik], *wl.q_inputs(w, ik)) for ik in range(3)]
+    for rep in range(2):
+        outs = []
+        ctx.set_k_batch_host(ks, Uks)
+        for ik in range(3):
+            ctx.select_k(ik)
+            for sl in (slice(0, 100), slice(100, 210)):           # 6 batches in flight, slots reused 3 times
+                o = torch.empty((sl.stop - sl.start, 4, 5, 6), dtype=torch.float64).pin_memory()
+                q, U, z, om = [t[sl] for t in ins[ik]]
+                ctx.q_batch_host_async(q.numpy(), U.numpy(), z.numpy(), om.numpy(), o.numpy())
+                outs.append((ik, sl, o))
+        ctx.wait()
+        for ik, sl, o in outs:
+            assert _relerr(o.numpy(), refs[ik][sl]) <= TOL
+        # synchronous call right after (and, on the second round, without an explicit wait in between)
+        ctx.select_k(1)
+        if rep == 1:
+            o = torch.empty((210, 4, 5, 6), dtype=torch.float64).pin_memory()
+            ctx.q_batch_host_async(*[t.numpy() for t in ins[1]], o.numpy())
+        out = np.empty((210, 4, 5, 6))
+        ctx.q_batch_host(*[t.numpy() for t in ins[1]], out)
+        assert _relerr(out, refs[1]) <= TOL
+        if rep == 1:
+            assert _relerr(o.numpy(), refs[1]) <= TOL
+    ctx.close()

@@ -102,12 +102,19 @@ def _full_size_case(env, name, k_check, n_sample):
         worst_out = max(worst_out, float(np.max(np.abs(got - ref))) / max(scale, float(ref.max())))
         # Eq. 87 on the whole batch: q -> q + G leaves out unchanged
         base = out.clone()
+        # the path has a fixed summation order: the same call again is bit-identical (this is what exposed a
+        # shared-memory ring race in the contraction: an early stage release let a bulk copy overwrite fragments
+        # still being loaded, on the first, cold call only)
+        ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
+        assert bool(torch.equal(out, base)), "q_batch is not reproducible"
         (q2_d,) = harness.to_device([q + np.array([2.0, -1.0, 1.0])])
         ctx.q_batch(q2_d, Ukq_d, ev_d, om_d, out)
-        assert float((out - base).abs().max().item()) <= 1e-10 * scale
+        out.sub_(base)
+        shift_err = float(out.abs().max().item())
         del base
+        assert shift_err <= 1e-10 * scale, (shift_err, scale)
     n = ctx.launch_counts()
-    assert n["setk_gemm"] == 1 and n["contract"] == 2 * len(k_check)      # one launch per q batch
+    assert n["setk_gemm"] == 1 and n["contract"] == 3 * len(k_check)      # one launch per q batch
     ctx.close()
     del gW, out
     torch.cuda.empty_cache()

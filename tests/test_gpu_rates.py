@@ -1,0 +1,149 @@
+"""GPU parity of the fused linewidth accumulation (Eq. 29 L229 + Eq. 61):
+phoebe_elph_q_batch_rates against the CPU oracle (oracle.elph -> oracle.rates) on the same seeded inputs.
+
+Bar: max_b1 |rate_gpu - rate_oracle| <= 1e-10 * max_b1 |rate_oracle|  (the north-star tolerance carried through the
+linear sum; derivation in DESIGN.md "Tolerance"), and |g|^2, when also stored, to the bar of test_gpu_parity.py.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def _relerr(got, ref):
+    return float(np.max(np.abs(got - ref)) / np.max(np.abs(ref)))
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import oracle
+    from paper_2111_14999_b200 import binding, build, harness, workloads as wl
+    build.build()
+    binding.load_library()
+    assert torch.cuda.is_available()
+    return dict(torch=torch, oracle=oracle, binding=binding, harness=harness, wl=wl)
+
+
+def _case(wl, w, ik=0):
+    a = dict(gW=wl.gW_full(w), Re=wl.Re_vectors(w), Rp=wl.Rp_vectors(w), k=wl.k_points(w)[ik], Uk=wl.U_k(w, ik),
+             q=wl.q_points(w, ik), Ukq=wl.U_kq(w, ik), ev=wl.ph_eigvecs(w, ik), om=wl.omega(w, ik))
+    a["eps_k"], a["eps_kq"] = wl.band_energies(w, ik)
+    return a
+
+
+def _oracle_rates(oracle, a, P, rate0=None, om=None):
+    om = a["om"] if om is None else om
+    out = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], om)
+    rate = np.zeros(a["Uk"].shape[1]) if rate0 is None else rate0.copy()
+    oracle.rates(out, a["eps_k"], a["eps_kq"], om, P["kT"], P["mu"], P["sigma"], P["pref"], rate=rate)
+    return rate, out
+
+
+CASES = [
+    # nw nb1 nb2 nm  grid_e     grid_p     nq
+    (2, 2, 2, 3, (3, 3, 3), (3, 3, 3), 64),        # the tiny config's shape
+    (3, 2, 1, 2, (5, 1, 1), (7, 1, 1), 1),
+    (5, 4, 3, 6, (3, 3, 2), (2, 5, 3), 257),       # several q per CTA, ragged last CTA
+    (8, 4, 4, 6, (3, 3, 3), (3, 3, 3), 700),       # band-window shape
+    (7, 7, 7, 15, (2, 2, 1), (2, 3, 1), 40),       # NT = 2, nb2 % 8 != 0
+    (9, 9, 9, 30, (2, 1, 1), (3, 1, 1), 20),       # NT = 4 (the "large" cell's mode count)
+    (16, 16, 16, 12, (2, 2, 1), (2, 2, 2), 300),   # the 4-atom cell's band / mode counts (two 8-row b2 tiles)
+    (2, 2, 2, 51, (2, 1, 1), (2, 1, 1), 70),       # nm > 48: plain rotation path + stand-alone rate sum
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "nw%d_nb%d_%d_nm%d_nq%d" % (c[0], c[1], c[2], c[3], c[6]))
+@pytest.mark.parametrize("store", [False, True], ids=["rates_only", "rates_and_out"])
+def test_rates_match_oracle(env, case, store):
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    nw, nb1, nb2, nm, ge, gp, nq = case
+    w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=ge, grid_p=gp, nq=nq, cfg_id=90 + nw)
+    a = _case(wl, w)
+    P = dict(wl.RATE_PARAMS)
+    inc, out_ref = _oracle_rates(oracle, a, P)
+    rate0 = inc[::-1] * np.linspace(0.3, 0.7, nb1)  # accumulated INTO: start from a non-zero array of the same scale
+    ref = rate0 + inc
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=nq)
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    d = harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"], a["eps_k"], a["eps_kq"], rate0])
+    rate, out = ctx.q_batch_rates(*d, store_out=store, **P)
+    rate = rate.cpu().numpy()
+    assert _relerr(rate - rate0, ref - rate0) <= TOL
+    if store:
+        assert _relerr(out.cpu().numpy(), out_ref) <= TOL
+    else:
+        assert out is None
+    n = ctx.launch_counts()
+    assert n["rate_reduce"] == 1
+    ctx.close()
+
+
+def test_rates_sub_batches_accumulate_and_are_reproducible(env):
+    """Several internal q sub-batches and several calls accumulate into the same array (RP5 on the GPU); omega <= 0
+    contributes nothing (R18); two runs give bit-identical sums (fixed summation order)."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=4, nb1=3, nb2=4, nm=3, grid_e=(3, 3, 3), nq=300, cfg_id=95)
+    a = _case(wl, w)
+    om = a["om"].copy(); om[5, 1] = 0.0; om[299, 2] = -0.3
+    P = dict(wl.RATE_PARAMS)
+    ref, _ = _oracle_rates(oracle, a, P, om=om)
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=300)
+    ctx.set_tuning("nq_sub", 128)
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    q_d, U_d, z_d, w_d, e1_d, e2_d = harness.to_device([a["q"], a["Ukq"], a["ev"], om, a["eps_k"], a["eps_kq"]])
+    runs = []
+    for _ in range(2):
+        rate = torch.zeros(3, dtype=torch.float64, device="cuda")
+        ctx.q_batch_rates(q_d, U_d, z_d, w_d, e1_d, e2_d, rate, **P)
+        runs.append(rate.cpu().numpy())
+    assert _relerr(runs[0], ref) <= TOL
+    assert np.array_equal(runs[0], runs[1])
+    # two calls on halves of the q list == one call
+    rate = torch.zeros(3, dtype=torch.float64, device="cuda")
+    for sl in (slice(0, 170), slice(170, 300)):
+        ctx.q_batch_rates(q_d[sl].contiguous(), U_d[sl].contiguous(), z_d[sl].contiguous(), w_d[sl].contiguous(), e1_d,
+                          e2_d[sl].contiguous(), rate, **P)
+    assert _relerr(rate.cpu().numpy(), ref) <= TOL
+    assert ctx.launch_counts()["rate_reduce"] == 3 + 3 + 2 + 2
+    ctx.close()
+
+
+def test_rates_host_entry_point_and_errors(env):
+    wl, oracle, torch, harness, binding = env["wl"], env["oracle"], env["torch"], env["harness"], env["binding"]
+    w = wl.custom(nw=6, nb1=5, nb2=6, nm=9, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nq=150, cfg_id=96)
+    a = _case(wl, w)
+    P = dict(kT=0.01, mu=0.03, sigma=0.02, pref=0.7)
+    ref, out_ref = _oracle_rates(oracle, a, P)
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=150)
+    ctx.set_k_host(a["k"], a["Uk"])
+    rate = np.zeros(5)
+    ctx.q_batch_rates_host(a["q"], a["Ukq"], a["ev"], a["om"], a["eps_k"], a["eps_kq"], rate, **P)
+    assert _relerr(rate, ref) <= TOL
+    rate2, out = np.zeros(5), np.empty((150, 5, 6, 9))
+    ctx.q_batch_rates_host(a["q"], a["Ukq"], a["ev"], a["om"], a["eps_k"], a["eps_kq"], rate2, out=out, **P)
+    assert np.array_equal(rate2, rate)
+    assert _relerr(out, out_ref) <= TOL
+    for bad in (dict(P, kT=0.0), dict(P, sigma=-1.0)):
+        with pytest.raises(binding.PhoebeElphError) as e:
+            ctx.q_batch_rates_host(a["q"], a["Ukq"], a["ev"], a["om"], a["eps_k"], a["eps_kq"], rate, **bad)
+        assert e.value.code == -2
+    ctx.close()
+
+
+def test_rates_si_like_full(env):
+    """BASELINE.json configs[1] with the recipe's band energies: all 4096 q, linewidth of the 8 bands."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.CONFIGS["si-like"]
+    a = _case(wl, w)
+    P = dict(wl.RATE_PARAMS)
+    ref, _ = _oracle_rates(oracle, a, P)
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda())
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    rate = torch.zeros(w.nb1, dtype=torch.float64, device="cuda")
+    ctx.q_batch_rates(*harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"], a["eps_k"], a["eps_kq"]]), rate, **P)
+    assert np.all(ref > 0)
+    assert _relerr(rate.cpu().numpy(), ref) <= TOL
+    ctx.close()
