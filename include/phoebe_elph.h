@@ -197,6 +197,18 @@ int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2
  * nRp*nb1*nw*nmodes*16); for tests of set_k on its own.  Errors: E_NULL, E_NO_K, E_WORKSPACE, E_CUDA. */
 int phoebe_elph_copy_g1(phoebe_elph_ctx* ctx, void* dst_dev, size_t dst_bytes);
 
+/* the paper's "pool" (L576): when g(Re,Rp) does not fit one GPU it is distributed over Re.
+ * Eq. 71 is linear in g_W, so a rank that was set up with ITS Re vectors and ITS slab g_W[nRp][nRe_local][...]
+ * gets from set_k / set_k_batch the partial g1' of its shard; the sum over the ranks is the g1' of Eq. 71.
+ * This call hands out the g1' storage inside the workspace so that the caller can sum it IN PLACE across ranks
+ * (ncclAllReduce / torch.distributed.all_reduce on the context's stream) before q_batch:
+ *   slot >= 0: *ptr_out = DEVICE address of the g1' of k slot `slot` (complex128 [nRp][nb1][nw][nmodes]),
+ *              *bytes_out = nRp*nb1*nw*nmodes*16;
+ *   slot = -1: the storage of all k slots filled by the last set_k / set_k_batch as one range (slots are
+ *              *stride_out bytes apart; the gap after each slot's data is padding and may be summed along).
+ * stride_out may be NULL.  Host-side only.  Errors: E_NULL, E_NO_K, E_DIMS. */
+int phoebe_elph_g1_buffer(phoebe_elph_ctx* ctx, int32_t slot, void** ptr_out, size_t* bytes_out, size_t* stride_out);
+
 /* Launch accounting: counts[PHOEBE_ELPH_K_COUNT] = kernels launched so far, per kind. */
 int phoebe_elph_launch_counts(const phoebe_elph_ctx* ctx, int64_t* counts);
 

@@ -22,7 +22,7 @@ EXPORTS = [
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
-    "phoebe_elph_copy_g1", "phoebe_elph_launch_counts",
+    "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
     "phoebe_elph_version",
@@ -76,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.phoebe_elph_g1_buffer.argtypes = [c_void_p, c_int32, POINTER(c_void_p), POINTER(c_size_t), POINTER(c_size_t)]
     lib.phoebe_elph_launch_counts.argtypes = [c_void_p, POINTER(c_int64)]
     lib.phoebe_elph_profile.argtypes = [c_void_p, c_int32]
     lib.phoebe_elph_profile_read.argtypes = [c_void_p, POINTER(c_double), POINTER(c_int64)]
@@ -291,6 +292,21 @@ class ElphContext:
         g1 = torch.empty((d.nRp, self.nb1, d.nw, d.nmodes), dtype=torch.complex128, device=self.device)
         self._check(self._lib.phoebe_elph_copy_g1(self._ctx, g1.data_ptr(), g1.numel() * 16), "phoebe_elph_copy_g1")
         return g1
+
+    def g1_view(self, slot: int = -1):
+        """float64 view (no copy) of the g1' storage inside the workspace: slot >= 0 -> that k slot's
+        [nRp][nb1][nw][nm][2]; slot = -1 -> every filled slot as one flat range (for an in-place all_reduce of the
+        Re-pool)."""
+        ptr, nbytes, stride = c_void_p(0), c_size_t(0), c_size_t(0)
+        self._check(self._lib.phoebe_elph_g1_buffer(self._ctx, int(slot), byref(ptr), byref(nbytes), byref(stride)),
+                    "phoebe_elph_g1_buffer")
+        off = ptr.value - self._ws.data_ptr()
+        assert 0 <= off and off + nbytes.value <= self._ws.numel()
+        flat = self._ws[off:off + nbytes.value].view(self._torch.float64)
+        if slot >= 0:
+            d = self.dims
+            return flat.view(d.nRp, self.nb1, d.nw, d.nmodes, 2)
+        return flat
 
     def launch_counts(self):
         arr = (c_int64 * len(KERNEL_KINDS))()

@@ -774,6 +774,25 @@ int phoebe_elph_copy_g1(phoebe_elph_ctx* c, void* dst_dev, size_t dst_bytes)
     return PHOEBE_ELPH_OK;
 }
 
+int phoebe_elph_g1_buffer(phoebe_elph_ctx* c, int32_t slot, void** ptr_out, size_t* bytes_out, size_t* stride_out)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!ptr_out || !bytes_out) return fail(c, PHOEBE_ELPH_E_NULL, "g1_buffer: null pointer");
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "g1_buffer before set_k");
+    if (slot < -1 || slot >= c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "g1_buffer: slot out of range");
+    const size_t one = (size_t)c->dims.nRp * c->nb1 * c->dims.nw * c->dims.nmodes * 16;
+    const size_t stride = c->L.g1_stride * 16;
+    if (stride_out) *stride_out = stride;
+    if (slot >= 0) {
+        *ptr_out = c->g1_base + (size_t)slot * c->L.g1_stride;
+        *bytes_out = one;
+    } else {
+        *ptr_out = c->g1_base;
+        *bytes_out = (size_t)(c->nk_have - 1) * stride + one;
+    }
+    return PHOEBE_ELPH_OK;
+}
+
 int phoebe_elph_launch_counts(const phoebe_elph_ctx* c, int64_t* counts)
 {
     if (!c || !counts) return PHOEBE_ELPH_E_NULL;

@@ -324,3 +324,47 @@ def test_async_pipelined_host_batches(env):
         if rep == 1:
             assert _relerr(o.numpy(), refs[1]) <= TOL
     ctx.close()
+
+
+@pytest.mark.parametrize("batch", [False, True], ids=["set_k", "set_k_batch"])
+def test_re_pool_partial_g1_sums_to_eq71(env, batch):
+    """two contexts, each set up with one Re shard (its Re vectors, its slab of g_W),
+    give partial g1'; their in-place sum through g1_view (what the pool's all-reduce does across GPUs) is the g1' of
+    Eq. 71, and q_batch on it matches the oracle on the full problem.  (One device: the two shards run one after the
+    other; the collective itself is covered by the world_size-2 gloo test.)"""
+    from paper_2111_14999_b200 import sharding
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=5, nb1=4, nb2=5, nm=6, grid_e=(3, 3, 2), grid_p=(3, 2, 2), nk=3, nq=90, cfg_id=86)
+    gW_np, Re, Rp, ks = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w), wl.k_points(w)
+    deg_e = np.random.default_rng(8).integers(1, 4, w.nRe).astype(np.float64)
+    nk = 3 if batch else 1
+    Uks = np.stack([wl.U_k(w, ik) for ik in range(nk)])
+    from paper_2111_14999_b200 import binding
+    ctxs = []
+    for r in range(2):
+        lo, hi = sharding.shard_range(w.nRe, r, 2)
+        slab = torch.from_numpy(np.ascontiguousarray(gW_np[:, lo:hi])).cuda()
+        c = binding.ElphContext(slab, Re[lo:hi], Rp, deg_e[lo:hi], None, nb1_max=w.nb1, nb2_max=w.nb2, nq_max=w.nq,
+                                nk_max=nk if batch else 0)
+        if batch:
+            sharding.pool_set_k_batch(c, ks[:nk], harness.to_device([Uks])[0])      # world = 1: no collective
+        else:
+            sharding.pool_set_k(c, ks[0], harness.to_device([Uks[0]])[0])
+        ctxs.append(c)
+    a, b = ctxs[0].g1_view(-1), ctxs[1].g1_view(-1)
+    assert a.shape == b.shape and a.data_ptr() != b.data_ptr()
+    a.add_(b)                                          # what all_reduce(SUM) leaves on every rank of the pool
+    for ik in reversed(range(nk)):
+        ctxs[0].select_k(ik)
+        g1_ref = oracle.setk(gW_np, Re, deg_e, ks[ik], Uks[ik])
+        assert _relerr(ctxs[0].copy_g1().cpu().numpy(), g1_ref) < 1e-12
+        v = ctxs[0].g1_view(ik).cpu().numpy()
+        assert _relerr(v[..., 0] + 1j * v[..., 1], g1_ref) < 1e-12
+        q, Ukq, ev, om = wl.q_inputs(w, ik)
+        out = ctxs[0].q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
+        assert _relerr(out, oracle.qbatch(g1_ref, Rp, None, q, Ukq, ev, om)) <= TOL
+    with pytest.raises(binding.PhoebeElphError) as e:
+        ctxs[0].g1_view(nk)
+    assert e.value.code == -2
+    for c in ctxs:
+        c.close()

@@ -81,3 +81,70 @@ def test_shard_k_properties():
     with pytest.raises(ValueError):
         sharding.shard_k(4, 0, 2, "other")
     assert sharding.max_over_ranks(3.5) == 3.5 and sharding.gather_by_k({1: 2}) == {1: 2}
+
+
+# ---- the Re-pool ------------------------------------------------------------------
+def _pool_worker(rank, world, port, q):
+    import oracle
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = wl.custom(nw=3, nb1=2, nb2=3, nm=3, grid_e=(3, 3, 1), grid_p=(2, 2, 2), nk=1, nq=7, cfg_id=91)
+        gW, Re, Rp = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w)
+        deg_e = np.random.default_rng(3).integers(1, 4, w.nRe).astype(np.float64)
+        k, Uk = wl.k_points(w)[0], wl.U_k(w, 0)
+        lo, hi = sharding.shard_range(w.nRe, rank, world)
+        # this rank's slab of g_W and its Re vectors: the partial g1' of Eq. 71 (stood in for by the oracle on CPU)
+        part = oracle.setk(np.ascontiguousarray(gW[:, lo:hi]), Re[lo:hi], deg_e[lo:hi], k, Uk)
+        g1 = torch.from_numpy(part)
+        sharding.allreduce_g1(g1, dist)                  # the one collective of the path
+        # step 2 shards over q, no collective
+        qq, Ukq, ev, om = wl.q_inputs(w, 0)
+        qlo, qhi = sharding.shard_range(w.nq, rank, world)
+        out = oracle.qbatch(g1.numpy(), Rp, None, qq[qlo:qhi], np.ascontiguousarray(Ukq[qlo:qhi]),
+                            np.ascontiguousarray(ev[qlo:qhi]), om[qlo:qhi])
+        merged = sharding.gather_by_k({rank: (qlo, qhi, out, g1.numpy().copy())}, dist)
+        if rank == 0:
+            q.put(merged)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world2_gloo_re_pool():
+    import oracle
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_pool_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    merged = q.get(timeout=120)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    w = wl.custom(nw=3, nb1=2, nb2=3, nm=3, grid_e=(3, 3, 1), grid_p=(2, 2, 2), nk=1, nq=7, cfg_id=91)
+    gW, Re, Rp = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w)
+    deg_e = np.random.default_rng(3).integers(1, 4, w.nRe).astype(np.float64)
+    g1_ref = oracle.setk(gW, Re, deg_e, wl.k_points(w)[0], wl.U_k(w, 0))
+    qq, Ukq, ev, om = wl.q_inputs(w, 0)
+    ref = oracle.qbatch(g1_ref, Rp, None, qq, Ukq, ev, om)
+    got = np.empty_like(ref)
+    for r in range(world):
+        qlo, qhi, out, g1 = merged[r]
+        assert np.max(np.abs(g1 - g1_ref)) <= 1e-13 * np.max(np.abs(g1_ref))      # sum of the shards == Eq. 71
+        got[qlo:qhi] = out
+    assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(ref)
+
+
+def test_shard_range_properties():
+    for world in (1, 2, 3, 8):
+        for n in (1, 5, 27, 343, 729):
+            parts = [sharding.shard_range(n, r, world) for r in range(world)]
+            assert parts[0][0] == 0 and parts[-1][1] == n
+            assert all(parts[i][1] == parts[i + 1][0] for i in range(world - 1))
+            sizes = [hi - lo for lo, hi in parts]
+            assert max(sizes) - min(sizes) <= 1
+    t = torch.ones(3, dtype=torch.complex128)
+    assert sharding.allreduce_g1(t) is t
