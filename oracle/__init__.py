@@ -145,3 +145,34 @@ def rates(out, eps_k, eps_kq, omega, kT, mu, sigma, pref, rate=None):
     rc = f(nq, nb1, nb2, nm, _p(out), _p(eps_k), _p(eps_kq), _p(omega), kT, mu, sigma, pref, _p(rate))
     assert rc == 0
     return rate
+
+
+# ---- polar long-range term (Eq. 14-15) ---------------------------------------------------------------
+def polar_amplitude(q, ev, recip, G, Zstar, eps_inf, coeff):
+    """P[nq][nm] = i coeff sum_G (Q.Zeff_nu)/(Q.eps_inf.Q): the (q, nu)-only factor of Eq. 15 (readings R20-R24)."""
+    nq, nm, _ = ev.shape
+    q = _c(q, np.float64, (nq, 3)); ev = _c(ev, np.complex128, (nq, nm, nm))
+    recip = _c(recip, np.float64, (3, 3)); G = _c(G, np.float64).reshape(-1, 3)
+    Zstar = _c(Zstar, np.float64, (nm // 3, 3, 3)); eps_inf = _c(eps_inf, np.float64, (3, 3))
+    P = np.empty((nq, nm), dtype=np.complex128)
+    f = _load().oracle_polar_amplitude
+    f.argtypes = [ctypes.c_int] * 3 + [ctypes.c_void_p] * 6 + [ctypes.c_double, ctypes.c_void_p]
+    rc = f(nq, nm, len(G), _p(q), _p(ev), _p(recip), _p(G), _p(Zstar), _p(eps_inf), float(coeff), _p(P))
+    assert rc == 0
+    return P
+
+
+def qbatch_polar(g1, Rp, deg_p, q, Ukq, ev, omega, Uk, P):
+    """qbatch with the long-range amplitude P[q][nu] [U_kq^dagger U_k]_{b2 b1} added before |.|^2 (Eq. 14)."""
+    nRp, nb1, nw, nm = g1.shape
+    nq, _, nb2 = Ukq.shape
+    g1 = _c(g1, np.complex128); Rp = _c(Rp, np.float64, (nRp, 3))
+    deg_p = None if deg_p is None else _c(deg_p, np.float64, (nRp,))
+    q = _c(q, np.float64, (nq, 3)); Ukq = _c(Ukq, np.complex128, (nq, nw, nb2))
+    ev = _c(ev, np.complex128, (nq, nm, nm)); omega = _c(omega, np.float64, (nq, nm))
+    Uk = _c(Uk, np.complex128, (nw, nb1)); P = _c(P, np.complex128, (nq, nm))
+    out = np.empty((nq, nb1, nb2, nm), dtype=np.float64)
+    rc = _load().oracle_qbatch_polar(nRp, nw, nm, nb1, nb2, nq, _p(g1), _p(Rp), _p(deg_p), _p(q), _p(Ukq), _p(ev),
+                                     _p(omega), _p(Uk), _p(P), _p(out))
+    assert rc == 0
+    return out

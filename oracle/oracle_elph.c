@@ -264,3 +264,101 @@ int oracle_rates(int nq, int nb1, int nb2, int nm, const double *out /* [nq][nb1
     }
     return 0;
 }
+
+/* ========================================================================
+ * polar (long-range) correction, Eq. 14-15 (L139-L147):
+ *
+ *   g = g^S + g^L                                                               (Eq. 14)
+ *   g^L_{b'b nu}(k,q) = i (4 pi / V)(e^2 / 4 pi eps0) sum_s (hbar / (2 N_q m_s omega_{q nu}))^{1/2}
+ *        sum_{G != -q} [(q+G).Z*_s.z^s_{q nu}] / [(q+G).eps_inf.(q+G)]
+ *        <psi_{k+q,b'}| e^{i(q+G).r} |psi_{k,b}>                                 (Eq. 15)
+ *
+ * Readings (R20-R24):
+ *   R20 the matrix element is taken in the Wannier-gauge approximation of the paper's Ref. [34]:
+ *       <psi_{k+q,b'}|e^{i(q+G).r}|psi_{k,b}> = [U_{k+q}^dagger U_k]_{b'b}  (Eq. 15 prints psi_{k+q} on both
+ *       sides; the ket belongs to k as in Eq. 7);  O[b1][b2] = sum_w conj(U_kq[w][b2]) U_k[w][b1].
+ *   R21 (hbar/(2 m_s omega))^{1/2}: 1/sqrt(m_s) is folded into ev by the caller (R6), 1/sqrt(2 omega) is the
+ *       library's final 1/(2 omega) on |.|^2 exactly as for the short-range part (R7: 0 where omega <= 0),
+ *       1/sqrt(N_q) and (4 pi/V)(e^2/4 pi eps0) are the caller's real `coeff`.  So what is ADDED to the
+ *       amplitude E of Eq. 13 before |.|^2 is   L[q][b1][b2][nu] = P[q][nu] O[q][b1][b2],
+ *         P[q][nu] = i coeff sum_G [Q.Zeff_nu] / [Q.eps_inf.Q],   Q = (q+G) in Cartesian coordinates,
+ *         Zeff_nu[a] = sum_s sum_b Z*_s[a][b] ev[q][3s+b][nu].
+ *   R22 q, G are in crystal coordinates (L510); Q = (q+G)_0 B[0] + (q+G)_1 B[1] + (q+G)_2 B[2] with the rows
+ *       of `recip` = reciprocal lattice vectors (any 2 pi inside them).
+ *   R23 "G != -q": a term is skipped when, and only when, Q is exactly the zero vector.  The sum runs over the
+ *       caller's finite list of G (Eq. 15 prints no convergence factor; none is applied).
+ *   R24 (q+G).Z*_s.z = sum_{a,b} Q_a Z*_s[a][b] z_b  (row index of Z* with the wavevector).
+ *
+ * Plain loops.  Pins: tests/test_oracle_polar_pins.py (PP1-PP8).
+ * ====================================================================== */
+int oracle_polar_amplitude(int nq, int nm, int nG, const double *q /* [nq][3] */, const cplx *ev /* [nq][nm][nm] */,
+                           const double *recip /* [3][3] */, const double *G /* [nG][3] */,
+                           const double *Zstar /* [nm/3][3][3] */, const double *eps_inf /* [3][3] */, double coeff,
+                           cplx *P /* [nq][nm] */)
+{
+    if (nm % 3) return -2;
+    int nat = nm / 3;
+    for (int iq = 0; iq < nq; ++iq)
+        for (int nu = 0; nu < nm; ++nu) {
+            cplx zeff[3] = {0.0, 0.0, 0.0};
+            for (int s = 0; s < nat; ++s)
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b)
+                        zeff[a] += Zstar[(s * 3 + a) * 3 + b] * ev[((size_t)iq * nm + 3 * s + b) * nm + nu];
+            cplx sum = 0.0;
+            for (int ig = 0; ig < nG; ++ig) {
+                double c[3], Q[3];
+                for (int a = 0; a < 3; ++a) c[a] = q[3 * iq + a] + G[3 * ig + a];
+                for (int a = 0; a < 3; ++a) Q[a] = c[0] * recip[a] + c[1] * recip[3 + a] + c[2] * recip[6 + a];
+                if (Q[0] == 0.0 && Q[1] == 0.0 && Q[2] == 0.0) continue;       /* G = -q */
+                double den = 0.0;
+                for (int a = 0; a < 3; ++a)
+                    for (int b = 0; b < 3; ++b) den += Q[a] * eps_inf[a * 3 + b] * Q[b];
+                cplx num = Q[0] * zeff[0] + Q[1] * zeff[1] + Q[2] * zeff[2];
+                sum += num / den;
+            }
+            P[(size_t)iq * nm + nu] = I * coeff * sum;
+        }
+    return 0;
+}
+
+/* oracle_qbatch with the long-range amplitude added before |.|^2 (Eq. 14):
+ *   E[b1][b2][nu] = (short-range E of oracle_qbatch) + P[q][nu] * sum_w conj(U_kq[w][b2]) U_k[w][b1] */
+int oracle_qbatch_polar(int nRp, int nw, int nm, int nb1, int nb2, int nq,
+                        const cplx *g1, const double *Rp, const double *deg_p,
+                        const double *q, const cplx *Ukq, const cplx *ev, const double *omega,
+                        const cplx *Uk /* [nw][nb1] */, const cplx *P /* [nq][nm] */, double *out)
+{
+    size_t N = (size_t)nb1 * nw * nm;
+    int rc = 0;
+#pragma omp parallel for schedule(static)
+    for (int iq = 0; iq < nq; ++iq) {
+        cplx *C = (cplx *)calloc(N, sizeof(cplx));
+        if (!C) { rc = -1; continue; }
+        for (int p = 0; p < nRp; ++p) {
+            cplx ph = oracle_phase(q + 3 * iq, Rp + 3 * p) / (deg_p ? deg_p[p] : 1.0);
+            const cplx *g = g1 + (size_t)p * N;
+            for (size_t n = 0; n < N; ++n) C[n] += ph * g[n];
+        }
+        const cplx *U = Ukq + (size_t)iq * nw * nb2;
+        const cplx *Z = ev + (size_t)iq * nm * nm;
+        for (int b1 = 0; b1 < nb1; ++b1)
+            for (int b2 = 0; b2 < nb2; ++b2) {
+                cplx ov = 0.0;                                   /* [U_kq^dagger U_k]_{b2 b1} */
+                for (int w = 0; w < nw; ++w) ov += conj(U[(size_t)w * nb2 + b2]) * Uk[(size_t)w * nb1 + b1];
+                for (int nu = 0; nu < nm; ++nu) {
+                    cplx s = 0.0;
+                    for (int ka = 0; ka < nm; ++ka)
+                        for (int w2 = 0; w2 < nw; ++w2)
+                            s += conj(U[(size_t)w2 * nb2 + b2]) * C[((size_t)b1 * nw + w2) * nm + ka] *
+                                 Z[(size_t)ka * nm + nu];
+                    s += P[(size_t)iq * nm + nu] * ov;
+                    double w = omega[(size_t)iq * nm + nu];
+                    double m2 = creal(s) * creal(s) + cimag(s) * cimag(s);
+                    out[(((size_t)iq * nb1 + b1) * nb2 + b2) * nm + nu] = (w > 0.0) ? m2 / (2.0 * w) : 0.0;
+                }
+            }
+        free(C);
+    }
+    return rc;
+}
