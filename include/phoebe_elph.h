@@ -68,7 +68,8 @@ enum {
     PHOEBE_ELPH_K_ROTATE_EPI  = 4,  /* a5-a7: U_kq^dagger, phonon rotation, |.|^2/(2 omega) */
     PHOEBE_ELPH_K_SETK_GEMM   = 5,  /* a1 for a batch of k: one pass over g_W (FP64 GEMM, DMMA) */
     PHOEBE_ELPH_K_RATE_REDUCE = 6,  /* f2: fixed-order sum of the per-CTA linewidth partials    */
-    PHOEBE_ELPH_K_COUNT       = 7
+    PHOEBE_ELPH_K_POLAR       = 7,  /* f4: (q, nu) amplitudes of the polar long-range term        */
+    PHOEBE_ELPH_K_COUNT       = 8
 };
 
 /* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
@@ -196,6 +197,21 @@ int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2
 /* Copy the current g1' (complex128 [nRp][nb1][nw][nmodes]) to dst_dev (DEVICE, >= bytes
  * nRp*nb1*nw*nmodes*16); for tests of set_k on its own.  Errors: E_NULL, E_NO_K, E_WORKSPACE, E_CUDA. */
 int phoebe_elph_copy_g1(phoebe_elph_ctx* ctx, void* dst_dev, size_t dst_bytes);
+
+/* polar (long-range) correction, Eq. 14-15 (L139-L147): g = g^S + g^L.  After this call every
+ * q_batch / q_batch_rates (and their host forms) adds, to the amplitude of Eq. 13 before |.|^2,
+ *   L[q][b1][b2][nu] = P[q][nu] * sum_w conj(U_kq[q][w][b2]) U_k[w][b1]            (overlap [U_kq^dagger U_k])
+ *   P[q][nu] = i coeff sum_{G in list, q+G != 0} (Q . Zeff_nu) / (Q . eps_inf . Q),   Q = (q + G) . recip,
+ *   Zeff_nu[a] = sum_{s,b} Zstar[s][a][b] ev[q][3s+b][nu]
+ * (readings R20-R24 of DESIGN.md: 1/sqrt(m_s) is inside ev, 1/sqrt(2 omega) is the final 1/(2 omega), everything
+ * else of Eq. 15's prefactor is the real `coeff`; no convergence factor is applied -- the caller chooses the G list).
+ *   recip_host HOST [3][3] rows = reciprocal lattice vectors (Cartesian); G_host HOST [nG][3] crystal coordinates,
+ *   0 <= nG <= 4096, nG = 0 switches the term off (the other pointers may then be NULL);
+ *   Zstar_host HOST [nmodes/3][3][3] Born effective charges; eps_inf_host HOST [3][3].  All copied; synchronises
+ *   the stream once.  nmodes must be a multiple of 3.
+ * Errors: E_NULL, E_DIMS, E_CUDA. */
+int phoebe_elph_set_polar(phoebe_elph_ctx* ctx, const double* recip_host, int32_t nG, const double* G_host,
+                          const double* Zstar_host, const double* eps_inf_host, double coeff);
 
 /* the paper's "pool" (L576): when g(Re,Rp) does not fit one GPU it is distributed over Re.
  * Eq. 71 is linear in g_W, so a rank that was set up with ITS Re vectors and ITS slab g_W[nRp][nRe_local][...]

@@ -14,7 +14,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libphoebe_elph.so")
 
-KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm", "rate_reduce"]
+KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm", "rate_reduce", "polar"]
 
 #: every symbol declared in include/phoebe_elph.h
 EXPORTS = [
@@ -22,7 +22,7 @@ EXPORTS = [
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
-    "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_launch_counts",
+    "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
     "phoebe_elph_version",
@@ -76,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.phoebe_elph_set_polar.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_double]
     lib.phoebe_elph_g1_buffer.argtypes = [c_void_p, c_int32, POINTER(c_void_p), POINTER(c_size_t), POINTER(c_size_t)]
     lib.phoebe_elph_launch_counts.argtypes = [c_void_p, POINTER(c_int64)]
     lib.phoebe_elph_profile.argtypes = [c_void_p, c_int32]
@@ -292,6 +293,19 @@ class ElphContext:
         g1 = torch.empty((d.nRp, self.nb1, d.nw, d.nmodes), dtype=torch.complex128, device=self.device)
         self._check(self._lib.phoebe_elph_copy_g1(self._ctx, g1.data_ptr(), g1.numel() * 16), "phoebe_elph_copy_g1")
         return g1
+
+    def set_polar(self, recip=None, G=None, Zstar=None, eps_inf=None, coeff=0.0):
+        """Switch the polar long-range term (Eq. 14-15) on (NumPy arrays: recip [3][3], G [nG][3] crystal coords,
+        Zstar [nm/3][3][3], eps_inf [3][3]) or, with G=None, off."""
+        import numpy as np
+        if G is None:
+            self._check(self._lib.phoebe_elph_set_polar(self._ctx, None, 0, None, None, None, 0.0), "phoebe_elph_set_polar")
+            return
+        recip, G, Zstar, eps_inf = [np.ascontiguousarray(a, dtype=np.float64) for a in (recip, G, Zstar, eps_inf)]
+        assert recip.shape == (3, 3) and eps_inf.shape == (3, 3) and G.ndim == 2 and G.shape[1] == 3
+        assert Zstar.shape == (self.dims.nmodes // 3, 3, 3)
+        self._check(self._lib.phoebe_elph_set_polar(self._ctx, recip.ctypes.data, len(G), G.ctypes.data, Zstar.ctypes.data,
+                                                    eps_inf.ctypes.data, float(coeff)), "phoebe_elph_set_polar")
 
     def g1_view(self, slot: int = -1):
         """float64 view (no copy) of the g1' storage inside the workspace: slot >= 0 -> that k slot's

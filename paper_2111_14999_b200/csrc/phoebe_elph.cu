@@ -23,6 +23,7 @@ constexpr size_t kAlign = 256;
 constexpr int kQPad = 128;                // q columns of Pt are padded to this (largest BM)
 constexpr int kKPad = 16;                 // phase matrices are zero padded to this many rows (largest KC)
 constexpr int kKBatchMax = 32;            // most k-points per set_k_batch (largest BM of the a1 GEMM)
+constexpr int kMaxG = 4096;                // most reciprocal lattice vectors of the polar G sum (f4)
 constexpr size_t kCBytesCap = 9000000000ull;   // C + Pt of one q sub-batch (whole batch whenever it fits)
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -51,7 +52,7 @@ struct Layout {
     int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
-           off_g1 = 0, off_Pt = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_Pt = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
@@ -97,6 +98,10 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_part = take((size_t)nq_max * d.nb1_max * 8);
     L.off_rate = take((size_t)2 * d.nb1_max * 8);
     L.off_seps = take((size_t)nq_max * d.nb2_max * 8);
+    // f4: G list and Born charges of the polar term, its (q, nu) amplitudes
+    L.off_G = take((size_t)kMaxG * 3 * 8);
+    L.off_Zstar = take((size_t)ceil_div(d.nmodes, 3) * 9 * 8);
+    L.off_P = take((size_t)nq_max * d.nmodes * 16);
     // staging for the host-buffer entry points
     // (two slots each: q_batch_host_async copies batch n+1 in and batch n-1 out while batch n computes)
     L.sz_sq = align_up((size_t)nq_max * 3 * 8, kAlign);
@@ -145,12 +150,16 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
-    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
     bool async_ready = false;
     unsigned async_n = 0;
+    // f4: polar long-range term (Eq. 14-15); nG == 0 = off
+    int nG = 0;
+    pe::PolarParams polar{};
+    int k_sel = 0;            // k slot chosen by select_k (its U_k is needed for the overlap of Eq. 15)
     bool prof = false;
     std::vector<EventPair> evs;
     std::vector<cudaEvent_t> ev_pool;
@@ -253,9 +262,18 @@ int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double
     return PHOEBE_ELPH_OK;
 }
 
+// U_k of every k slot is kept in the context (the overlap [U_kq^dagger U_k] of the polar term needs it at q_batch time)
+int keep_Uk(phoebe_elph_ctx* c, const double2* Uk_dev, int nk, int nb1)
+{
+    if (Uk_dev != c->Uk)
+        PE_CUDA(c, cudaMemcpyAsync(c->Uk, Uk_dev, (size_t)nk * c->dims.nw * nb1 * 16, cudaMemcpyDeviceToDevice, c->stream));
+    return PHOEBE_ELPH_OK;
+}
+
 int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb1)
 {
     const phoebe_elph_dims& d = c->dims;
+    if (int rc = keep_Uk(c, Uk_dev, 1, nb1)) return rc;
     const int X = d.nw * d.nw * d.nmodes;
     const int T = setk_threads(X);
     int S = c->s_split > 0 ? c->s_split : setk_auto_split(d.nRe, d.nRp, X);
@@ -273,6 +291,7 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
     if (rc) return rc;
     c->nb1 = nb1;
     c->nk_have = 1;
+    c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
     return PHOEBE_ELPH_OK;
@@ -284,6 +303,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
 {
     const phoebe_elph_dims& d = c->dims;
     const int X = d.nw * d.nw * d.nmodes;
+    if (int rc = keep_Uk(c, Uk_dev, nk, nb1)) return rc;
     PE_CUDA(c, cudaMemcpyAsync(c->kdev, k_host, (size_t)nk * 24, cudaMemcpyHostToDevice, c->stream));
     {
         LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
@@ -314,6 +334,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     }
     c->nb1 = nb1;
     c->nk_have = nk;
+    c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
     return PHOEBE_ELPH_OK;
@@ -367,7 +388,13 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     }
     const bool fused_rates = rr != nullptr && use_mma;
     if (fused_rates)       // omega, n, eps_kq, f' per q of the CTA + one row of sums per warp (follows Cs)
-        rot_smem += ((size_t)QG * (2 * 8 * NT + 2 * 8 * ceil_div(nb2, 8)) + 4 * (size_t)nb1) * 8;
+        rot_smem += ((size_t)QG * (2 * 8 * NT + 2 * 8 * ceil_div(nb2, 8)) + ((4 * (size_t)nb1 + 1) & ~(size_t)1)) * 8;
+    const bool polar = c->nG > 0;
+    if (polar && use_mma)  // P of the CTA's q-points and their overlaps O[b1][b2] (follow the rate arrays)
+        rot_smem += ((size_t)QG * 8 * NT + (size_t)QG * nb1 * 8 * ceil_div(nb2, 8)) * 16;
+    if (rot_smem > (227u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+    double2* Pbuf = reinterpret_cast<double2*>(c->ws + c->L.off_P);
+    pe::PolarArgs pa{nullptr, c->Uk + (size_t)c->k_sel * d.nw * nb1};
     if (rr && !use_mma && out == nullptr)      // the plain path sums from the stored |g|^2: keep it in the staging area
         out = reinterpret_cast<double*>(c->ws + c->L.off_sout);
     auto rot_kernel = [&]() -> const void* {
@@ -425,6 +452,14 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 else PE_CUDA(c, (launch_contract<64, 64, 2, 2, 16, 3, false, 2>(c->stream, g)));
             }
         }
+        if (polar) {
+            LaunchScope ls(c, PHOEBE_ELPH_K_POLAR);
+            pe::k_polar_amp<<<ceil_div(nqs, 4), 128, (size_t)4 * d.nmodes * 8, c->stream>>>(
+                q + 3 * (size_t)qs, ev + (size_t)qs * d.nmodes * d.nmodes, reinterpret_cast<const double*>(c->ws + c->L.off_G),
+                reinterpret_cast<const double*>(c->ws + c->L.off_Zstar), nqs, d.nmodes, c->nG, c->polar, Pbuf);
+            PE_CUDA(c, cudaGetLastError());
+            pa.P = Pbuf;
+        }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
             dim3 grid = use_mma ? dim3(ceil_div(nqs, QG)) : dim3(ceil_div(nb1, gb1), nqs);
@@ -435,8 +470,8 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             double* op = out ? out + (size_t)qs * nb1 * nb2 * d.nmodes : nullptr;
             int nw_ = d.nw, nm_ = d.nmodes, nb1_ = nb1, nb2_ = nb2, gb1_ = gb1, nqs_ = nqs, QG_ = QG;
             if (rr) ra.eps_kq = rr->eps_kq + (size_t)qs * nb2;
-            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_, &ra};
-            void* args_pl[] = {&Cp, &ldc_i, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_};
+            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_, &ra, &pa};
+            void* args_pl[] = {&Cp, &ldc_i, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &pa};
             PE_CUDA(c, cudaLaunchKernel(rot_kernel, grid, dim3(rot_threads), use_mma ? args_mma : args_pl, rot_smem,
                                         c->stream));
         }
@@ -594,6 +629,7 @@ int phoebe_elph_select_k(phoebe_elph_ctx* c, int32_t i)
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "select_k before set_k / set_k_batch");
     if (i < 0 || i >= c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "select_k: index out of range");
     c->g1 = c->g1_base + (size_t)i * c->L.g1_stride;
+    c->k_sel = i;
     return PHOEBE_ELPH_OK;
 }
 
@@ -771,6 +807,23 @@ int phoebe_elph_copy_g1(phoebe_elph_ctx* c, void* dst_dev, size_t dst_bytes)
     const size_t bytes = (size_t)c->dims.nRp * c->nb1 * c->dims.nw * c->dims.nmodes * 16;
     if (dst_bytes < bytes) return fail(c, PHOEBE_ELPH_E_WORKSPACE, "copy_g1: destination too small");
     PE_CUDA(c, cudaMemcpyAsync(dst_dev, c->g1, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_set_polar(phoebe_elph_ctx* c, const double* recip_host, int32_t nG, const double* G_host,
+                          const double* Zstar_host, const double* eps_inf_host, double coeff)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (nG == 0) { c->nG = 0; return PHOEBE_ELPH_OK; }
+    if (!recip_host || !G_host || !Zstar_host || !eps_inf_host) return fail(c, PHOEBE_ELPH_E_NULL, "set_polar: null pointer");
+    if (nG < 0 || nG > kMaxG) return fail(c, PHOEBE_ELPH_E_DIMS, "set_polar: nG out of range (<= 4096)");
+    if (c->dims.nmodes % 3) return fail(c, PHOEBE_ELPH_E_DIMS, "set_polar: nmodes is not 3 x atoms");
+    PE_CUDA(c, cudaMemcpyAsync(c->ws + c->L.off_G, G_host, (size_t)nG * 24, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaMemcpyAsync(c->ws + c->L.off_Zstar, Zstar_host, (size_t)(c->dims.nmodes / 3) * 72, cudaMemcpyHostToDevice, c->stream));
+    PE_CUDA(c, cudaStreamSynchronize(c->stream));      // the host arrays may be pageable
+    for (int i = 0; i < 9; ++i) { c->polar.recip[i] = recip_host[i]; c->polar.eps[i] = eps_inf_host[i]; }
+    c->polar.coeff = coeff;
+    c->nG = nG;
     return PHOEBE_ELPH_OK;
 }
 

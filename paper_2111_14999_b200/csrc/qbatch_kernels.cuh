@@ -38,6 +38,62 @@ k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ 
 }
 
 // ---------------------------------------------------------------------------
+// f4: the (q, nu)-only factor of the polar long-range term (Eq. 15):
+//   P[q][nu] = i coeff sum_G (Q . Zeff_nu) / (Q . eps_inf . Q),  Q = (q + G) . recip,
+//   Zeff_nu[a] = sum_{s,b} Z*_s[a][b] ev[q][3s+b][nu]
+// The G sum does not depend on nu: V[a] = sum_G Q_a / (Q.eps.Q) (real), W[3s+b] = sum_a V_a Z*_s[a][b],
+// P[nu] = i coeff sum_kappa W[kappa] ev[kappa][nu].  One warp per q; lanes stride over G, fixed-order
+// shuffle reduction; the term with Q exactly zero (G = -q) is skipped.
+// ---------------------------------------------------------------------------
+struct PolarParams { double recip[9]; double eps[9]; double coeff; };
+
+__global__ void __launch_bounds__(128)
+k_polar_amp(const double* __restrict__ q /* [nq][3] */, const double2* __restrict__ ev /* [nq][nm][nm] */,
+            const double* __restrict__ G /* [nG][3] */, const double* __restrict__ Zstar /* [nm/3][3][3] */,
+            int nq, int nm, int nG, PolarParams pp, double2* __restrict__ P /* [nq][nm] */)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double* W = reinterpret_cast<double*>(smem_raw) + (size_t)warp * nm;      // [warps][nm]
+    const int iq = blockIdx.x * (blockDim.x >> 5) + warp;
+    if (iq >= nq) return;
+    const double q0 = q[3 * (size_t)iq], q1 = q[3 * (size_t)iq + 1], q2 = q[3 * (size_t)iq + 2];
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+    for (int ig = lane; ig < nG; ig += 32) {
+        const double c0 = q0 + G[3 * ig], c1 = q1 + G[3 * ig + 1], c2 = q2 + G[3 * ig + 2];
+        const double Q0 = c0 * pp.recip[0] + c1 * pp.recip[3] + c2 * pp.recip[6];
+        const double Q1 = c0 * pp.recip[1] + c1 * pp.recip[4] + c2 * pp.recip[7];
+        const double Q2 = c0 * pp.recip[2] + c1 * pp.recip[5] + c2 * pp.recip[8];
+        if (Q0 == 0.0 && Q1 == 0.0 && Q2 == 0.0) continue;
+        const double den = Q0 * (pp.eps[0] * Q0 + pp.eps[1] * Q1 + pp.eps[2] * Q2) +
+                           Q1 * (pp.eps[3] * Q0 + pp.eps[4] * Q1 + pp.eps[5] * Q2) +
+                           Q2 * (pp.eps[6] * Q0 + pp.eps[7] * Q1 + pp.eps[8] * Q2);
+        const double r = 1.0 / den;
+        v0 = fma(Q0, r, v0); v1 = fma(Q1, r, v1); v2 = fma(Q2, r, v2);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+        v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+        v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+    }
+    for (int ka = lane; ka < nm; ka += 32) {
+        const double* Z = Zstar + (size_t)(ka / 3) * 9 + (ka % 3);          // Z*_s[a][b], b = ka % 3
+        W[ka] = v0 * Z[0] + v1 * Z[3] + v2 * Z[6];
+    }
+    __syncwarp();
+    const double2* Zq = ev + (size_t)iq * nm * nm;
+    for (int nu = lane; nu < nm; nu += 32) {
+        double sr = 0.0, si = 0.0;
+        for (int ka = 0; ka < nm; ++ka) {
+            const double2 z = Zq[(size_t)ka * nm + nu];
+            sr = fma(W[ka], z.x, sr); si = fma(W[ka], z.y, si);
+        }
+        P[(size_t)iq * nm + nu] = make_double2(-pp.coeff * si, pp.coeff * sr);     // i * coeff * (sr + i si)
+    }
+}
+
+// ---------------------------------------------------------------------------
 // a4 (and the multi-k form of a1): batched complex128 GEMM on the FP64 tensor cores
 //     C_z[m][n] = sum_{k<K} At[k][m] * B_z[k][n]          z = blockIdx.z
 // At is [Kpad][lda] (k-major, Kpad a multiple of KC, rows K..Kpad-1 and columns >= M zero), shared by all z;
@@ -270,11 +326,19 @@ struct RateArgs {
     double* partial;        // [gridDim.x][nb1]
 };
 
+// f4 (Eq. 14-15): when pa.P != nullptr the long-range amplitude P[q][nu] * O[q][b1][b2],
+// O = sum_w conj(Ukq[q][w][b2]) Uk[w][b1] (the overlap [U_kq^dagger U_k]_{b2 b1}), is added to E before |.|^2.
+// O of the CTA's q-points is formed once in shared memory from Us (already conjugated) and Uk.
+struct PolarArgs {
+    const double2* P;     // [nq][nm] of this launch, or nullptr
+    const double2* Uk;    // [nw][nb1]
+};
+
 template <int NT, bool RATES>
 __global__ void __launch_bounds__(128)
 k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
                       const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
-                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra)
+                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra, PolarArgs pa)
 {
     // One CTA = QG consecutive q-points; it walks the b1 groups (gb1 values of b1 each) with the C panels
     // double-buffered: the TMA bulk copy of group i+1 runs while the warps do the DMMAs of group i.
@@ -295,6 +359,10 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
     double* e2_s = bose_s + QG * 8 * NT;                                                 // [QG][8 MT]
     double* f2_s = e2_s + QG * 8 * MT;                                                   // [QG][8 MT]
     double* wsum = f2_s + QG * 8 * MT;                                                   // [4 warps][nb1]
+    // polar arrays follow the rate arrays when those exist, else Cs (host sizes the block the same way)
+    double2* Ps = reinterpret_cast<double2*>(RATES ? wsum + ((4 * nb1 + 1) & ~1) : om_s);   // [QG][8 NT]
+    double2* Os = Ps + QG * 8 * NT;                                                       // [QG][nb1][8 MT]
+    const bool polar = pa.P != nullptr;
     const int q0 = blockIdx.x * QG;
     const int nql = min(QG, nq - q0);
     if (threadIdx.x == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); mbar_fence_init(); }
@@ -347,6 +415,27 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
             f2_s[i] = ok ? 1.0 / (exp((e2 - ra.mu) * ra.inv_kT) + 1.0) : 0.0;
         }
         for (int i = threadIdx.x; i < 4 * nb1; i += blockDim.x) wsum[i] = 0.0;
+    }
+    if (polar) {
+        for (int i = threadIdx.x; i < QG * 8 * NT; i += blockDim.x) {
+            const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
+            Ps[i] = (ql < nql && nu < nm) ? pa.P[(size_t)(q0 + ql) * nm + nu] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();                    // Us complete
+        for (int i = threadIdx.x; i < nql * nb1 * 8 * MT; i += blockDim.x) {
+            const int ql = i / (nb1 * 8 * MT), r = i - ql * nb1 * 8 * MT;
+            const int b1 = r / (8 * MT), b2 = r - b1 * 8 * MT;
+            double sr = 0.0, si = 0.0;
+            if (b2 < nb2) {
+                const double2* us = Us + (size_t)ql * nwp * ldu + b2;
+                for (int w = 0; w < nw; ++w) {
+                    const double2 u = us[(size_t)w * ldu], k = pa.Uk[(size_t)w * nb1 + b1];
+                    sr = fma(u.x, k.x, sr); sr = fma(-u.y, k.y, sr);
+                    si = fma(u.x, k.y, si); si = fma(u.y, k.x, si);
+                }
+            }
+            Os[i] = make_double2(sr, si);
+        }
     }
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
@@ -403,6 +492,15 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
                         dmma884(ei[0], ei[1], ai, z.x);
                     }
                 const int nu = 8 * n + 2 * t;
+                if (polar) {
+                    const double2 o = Os[((size_t)ql * nb1 + b10 + b1) * 8 * MT + b2];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double2 pz = Ps[ql * 8 * NT + nu + h];
+                        er[h] += pz.x * o.x - pz.y * o.y;
+                        ei[h] += pz.x * o.y + pz.y * o.x;
+                    }
+                }
                 if (b2 < nb2) {
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
@@ -483,7 +581,7 @@ k_rate_reduce(const double* __restrict__ partial, int nparts, int nb1, double sc
 __global__ void __launch_bounds__(256)
 k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restrict__ Ukq,
                   const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
-                  int nw, int nm, int nb1, int nb2, int gb1)
+                  int nw, int nm, int nb1, int nb2, int gb1, PolarArgs pa)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* Uc = reinterpret_cast<double2*>(smem_raw);
@@ -530,6 +628,18 @@ k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restr
             const double2 c = d[ka];
             sr = fma(c.x, z.x, sr); sr = fma(-c.y, z.y, sr);
             si = fma(c.x, z.y, si); si = fma(c.y, z.x, si);
+        }
+        if (pa.P != nullptr) {          // f4: + P[q][nu] * [U_kq^dagger U_k]_{b2 b1}
+            const int b2 = (idx / nm) % nb2, b1 = b10 + idx / (nm * nb2);
+            double orr = 0.0, oi = 0.0;
+            for (int w2 = 0; w2 < nw; ++w2) {
+                const double2 u = Uc[w2 * nb2 + b2], k = pa.Uk[(size_t)w2 * nb1 + b1];
+                orr = fma(u.x, k.x, orr); orr = fma(-u.y, k.y, orr);
+                oi = fma(u.x, k.y, oi); oi = fma(u.y, k.x, oi);
+            }
+            const double2 pz = pa.P[(size_t)iq * nm + nu];
+            sr += pz.x * orr - pz.y * oi;
+            si += pz.x * oi + pz.y * orr;
         }
         const double w = om[nu];
         o[idx] = (w > 0.0) ? (sr * sr + si * si) / (2.0 * w) : 0.0;

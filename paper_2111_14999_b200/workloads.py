@@ -237,3 +237,20 @@ def band_energies(w: Workload, ik: int = 0):
     eps_k = _rng(w, _T_EPS_K, ik).uniform(-0.15, 0.15, w.nb1)
     eps_kq = _rng(w, _T_EPS_KQ, ik).uniform(-0.15, 0.15, (w.nq, w.nb2))
     return eps_k, eps_kq
+
+
+# ---- inputs of the polar long-range term (Eq. 14-15) --------------------------------------
+_T_POLAR = 9
+
+
+def polar_inputs(w: Workload, h: int = 2):
+    """dict(recip [3][3], G [(2h+1)^3][3], Zstar [nm/3][3][3], eps_inf [3][3], coeff): a slightly sheared reciprocal
+    lattice, the integer box {-h..h}^3 of G vectors, random Born charges of order 1 (not symmetric), a symmetric
+    positive-definite high-frequency dielectric tensor, and a coefficient that makes the long-range amplitude
+    comparable to the short-range one of the recipe."""
+    assert w.nm % 3 == 0
+    rng = _rng(w, _T_POLAR)
+    recip = 2.0 * np.pi * (np.eye(3) + 0.1 * rng.normal(size=(3, 3)))
+    A = rng.normal(size=(3, 3))
+    return dict(recip=recip, G=lattice_vectors((2 * h + 1,) * 3), Zstar=rng.normal(size=(w.nm // 3, 3, 3)),
+                eps_inf=A @ A.T + 3.0 * np.eye(3), coeff=2.0)

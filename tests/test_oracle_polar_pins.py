@@ -2,7 +2,7 @@
 (DESIGN.md).  None of them retypes the oracle's loops:
 
   PP1  coeff = 0 or Z* = 0: qbatch_polar == qbatch (Eq. 14 with g^L = 0).
-  PP2  hand-computed closed forms (tests/golden/closed_forms.txt: isotropic eps_inf and Z*, ev = identity, one G).
+  PP2  hand-computed closed forms (tests/golden/polar_closed_forms.txt: isotropic eps_inf and Z*, ev = identity, one G).
   PP3  the overlap factor is [U_kq^dagger U_k]_{b2 b1}: identity for U_kq = U_k (orthonormal columns), a pure phase
        for a re-phased U_kq, and equal to a NumPy matmul for general rectangular U (pins conj and index order).
   PP4  interference with the short-range amplitude: pins the factor i of Eq. 15 and its sign (golden polar_out_c).
@@ -19,7 +19,7 @@ import pytest
 import oracle
 from paper_2111_14999_b200 import workloads as wl
 
-GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "polar_closed_forms.txt")
 
 
 def _golden(name):
