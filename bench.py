@@ -202,6 +202,12 @@ def _with_kbatch(cfg, kb):
     return cfg
 
 
+def _with_multi(cfg, multi):
+    cfg = dict(cfg)
+    cfg["q_batch_multi"] = bool(multi)
+    return cfg
+
+
 # ----------------------------------------------------------------------------- GPU leg
 def run_ours(args):
     import torch
@@ -232,7 +238,11 @@ def run_ours(args):
         dev_inputs.append((k, harness.to_device([Uk], dev)[0], harness.to_device([q, Ukq, ev, om], dev)))
     t_gen = time.perf_counter() - t_gen
     kb = max(1, min(args.k_batch, 32, len(host_inputs)))
-    ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0)
+    # small cells (band windows): the q lists of all k slots of a batch go through ONE phase / contraction / rotation
+    # launch (phoebe_elph_q_batch_multi) -- one k-point's list alone is too small a GEMM for 148 SMs
+    multi = (kb > 1 and args.q_multi != 0 and w.nq % 64 == 0 and len(host_inputs) % kb == 0
+             and (args.q_multi == 1 or kb * w.nq * w.N * 16 <= (4 << 30)))
+    ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0, nq_max=kb * w.nq if multi else None)
     ctx.set_tuning("m3", args.m3)
     if args.tile:
         ctx.set_tuning("tile", args.tile)
@@ -243,7 +253,16 @@ def run_ours(args):
     Uks_np = [np.ascontiguousarray(np.stack([host_inputs[i][1] for i in g])) for g in groups]
     Uks_d = [harness.to_device([u], dev)[0] for u in Uks_np]
 
+    if multi:
+        stacks = [[torch.stack([dev_inputs[i][2][j] for i in g]).contiguous() for j in range(4)] for g in groups]
+        out_multi = torch.empty((kb, w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+
     def step():
+        if multi:
+            for ks, Uk_d, (q_s, Ukq_s, ev_s, om_s) in zip(ks_np, Uks_d, stacks):
+                ctx.set_k_batch(ks, Uk_d)
+                ctx.q_batch_multi(q_s, Ukq_s, ev_s, om_s, out_multi)
+            return
         if kb == 1:
             for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
                 ctx.set_k(k, Uk_d)
@@ -451,7 +470,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": _with_kbatch(_config_dict(w, world), kb),
+            "config": _with_multi(_with_kbatch(_config_dict(w, world), kb), multi),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else "q_batch_host_async + wait"},
@@ -479,6 +498,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=list(wl.CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--q-multi", type=int, default=-1,
+                    help="phoebe_elph_q_batch_multi over the k slots of a batch: -1 = automatic (small cells), 0 = off, 1 = force")
     ap.add_argument("--e2e-sync", action="store_true", help="end-to-end leg with the synchronous q_batch_host (no copy/compute overlap)")
     ap.add_argument("--no-rates", action="store_true", help="skip the extra fused-linewidth (f2) measurement")
     ap.add_argument("--m3", type=int, default=1, help="1 = three-multiply complex product in the GEMMs (default), 0 = four")

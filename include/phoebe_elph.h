@@ -144,6 +144,18 @@ int phoebe_elph_q_batch(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
                         const double* q_dev, const void* Ukq_dev, const void* ev_dev,
                         const double* omega_dev, double* out_dev);
 
+/* q_batch for the first nk k slots of the last set_k_batch in ONE pass (one phase, one contraction and one rotation
+ * launch for all of them): the inputs / outputs of the k slots are stacked, k slowest --
+ *   q_dev [nk][nq][3], Ukq_dev [nk][nq][nw][nb2], ev_dev [nk][nq][nmodes][nmodes], omega_dev [nk][nq][nmodes],
+ *   out_dev [nk][nq][nb1][nb2][nmodes];  rows of slot j are contracted with the g1' of slot j.
+ * Results are identical to nk select_k + q_batch calls.  It exists for band windows with few bands (L526-540), where
+ * one k-point's q list is too small a GEMM to fill 148 SMs.  nq must be a multiple of 64, nk*nq <= dims.nq_max;
+ * not available while the polar term is switched on.
+ * Errors: E_NULL, E_NO_K, E_DIMS, E_ALIGN, E_CUDA. */
+int phoebe_elph_q_batch_multi(phoebe_elph_ctx* ctx, int32_t nk, int32_t nq, int32_t nb2,
+                              const double* q_dev, const void* Ukq_dev, const void* ev_dev,
+                              const double* omega_dev, double* out_dev);
+
 /* Same with HOST buffers: copies the four inputs host->device into staging inside the
  * workspace, runs the batch, copies out device->host, and SYNCHRONISES the stream before
  * returning (so pageable buffers are safe).  This is the end-to-end call. */

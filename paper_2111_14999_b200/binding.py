@@ -20,7 +20,7 @@ KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epil
 EXPORTS = [
     "phoebe_elph_workspace_bytes", "phoebe_elph_setup", "phoebe_elph_set_k", "phoebe_elph_set_k_host",
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
-    "phoebe_elph_q_batch", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
+    "phoebe_elph_q_batch", "phoebe_elph_q_batch_multi", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
     "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
@@ -70,6 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_set_k_batch_host.argtypes = [c_void_p, c_int32, c_void_p, c_void_p, c_int32]
     lib.phoebe_elph_select_k.argtypes = [c_void_p, c_int32]
     lib.phoebe_elph_q_batch.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_q_batch_multi.argtypes = [c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_wait.argtypes = [c_void_p]
@@ -235,6 +236,24 @@ class ElphContext:
             assert out.is_cuda and out.is_contiguous() and out.numel() == nq * self.nb1 * nb2 * nm
         self._check(self._lib.phoebe_elph_q_batch(self._ctx, nq, nb2, q.data_ptr(), Ukq.data_ptr(), ev.data_ptr(),
                                                   omega.data_ptr(), out.data_ptr()), "phoebe_elph_q_batch")
+        return out
+
+    def q_batch_multi(self, q, Ukq, ev, omega, out=None):
+        """q_batch for the first nk k slots of the last set_k_batch in one pass.  CUDA tensors stacked over k:
+        q [nk][nq][3], Ukq [nk][nq][nw][nb2], ev [nk][nq][nm][nm], omega [nk][nq][nm] -> out [nk][nq][nb1][nb2][nm]."""
+        torch = self._torch
+        nk, nq, nw, nb2 = Ukq.shape
+        nm = self.dims.nmodes
+        for t in (q, Ukq, ev, omega):
+            assert t.is_cuda and t.is_contiguous()
+        assert q.shape == (nk, nq, 3) and ev.shape == (nk, nq, nm, nm) and omega.shape == (nk, nq, nm)
+        if out is None:
+            out = torch.empty((nk, nq, self.nb1, nb2, nm), dtype=torch.float64, device=self.device)
+        else:
+            assert out.is_cuda and out.is_contiguous() and out.numel() == nk * nq * self.nb1 * nb2 * nm
+        self._check(self._lib.phoebe_elph_q_batch_multi(self._ctx, nk, nq, nb2, q.data_ptr(), Ukq.data_ptr(),
+                                                        ev.data_ptr(), omega.data_ptr(), out.data_ptr()),
+                    "phoebe_elph_q_batch_multi")
         return out
 
     def q_batch_host(self, q, Ukq, ev, omega, out):

@@ -209,6 +209,7 @@ struct LaunchScope {          // counts the launch and, when profiling, brackets
 struct GemmArgs {
     const double2* At; int lda; const double2* B; int ldb; long long strideB;
     double2* C; long long ldc; long long strideC; int M, N, K, Kpad, batch;
+    int rowsPerB = 0, rowOffset = 0; long long strideBrow = 0;      // multi-k a4: B slab switches every rowsPerB rows
 };
 template <int BM, int BN, int WM, int WN, int KC, int ST, bool M3, int MINB = 1>
 cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persistent = true)
@@ -231,7 +232,8 @@ cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persist
     if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int grid = persistent ? (int)std::min<long long>(ntiles, (long long)kSMs * ctas_per_sm) : (int)ntiles;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(g.At, g.lda, g.B, g.ldb, g.strideB, g.C, g.ldc, g.strideC,
-                                                           g.M, g.N, g.K, g.Kpad, g.batch);
+                                                           g.M, g.N, g.K, g.Kpad, g.batch, g.rowsPerB, g.rowOffset,
+                                                           g.strideBrow);
     return cudaGetLastError();
 }
 
@@ -344,8 +346,9 @@ struct RateReq {           // f2: linewidth accumulation fused into the epilogue
     const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate;
 };
 
+// rows_per_k > 0: the q lists of the k slots 0.. are stacked (nq = slots * rows_per_k rows); row block j uses the g1' of slot j
 int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const double2* Ukq, const double2* ev,
-                const double* omega, double* out, const RateReq* rr = nullptr)
+                const double* omega, double* out, const RateReq* rr = nullptr, int rows_per_k = 0)
 {
     const phoebe_elph_dims& d = c->dims;
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
@@ -438,11 +441,15 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_CONTRACT);
             GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, (long long)N, 0, nqs, N, d.nRp, c->L.Kpad, 1};
+            if (rows_per_k > 0) {
+                g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
+            }
             // tile choice: 64x64 unless that leaves the 148 SMs with a long ragged tail (few tiles);
             // cost model = rounds of tiles per SM x tile area (+5 % for the smaller tile's extra operand traffic)
             const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64;
             const double cost32 = (double)ceil_div(ceil_div(nqs, 32) * ceil_div(N, 32), kSMs) * 32 * 32 * 1.05;
-            const int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
+            int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
+            if (rows_per_k > 0 && tile != 32 && tile != 64) tile = 64;       // the stacked form knows these two tiles
             if (c->m3) {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
                 else if (tile == 6432) PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true, 2>(c->stream, g)));
@@ -647,6 +654,22 @@ int phoebe_elph_q_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const doubl
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
     return run_q_batch(c, nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
                        omega_dev, out_dev);
+}
+
+int phoebe_elph_q_batch_multi(phoebe_elph_ctx* c, int32_t nk, int32_t nq, int32_t nb2, const double* q_dev,
+                              const void* Ukq_dev, const void* ev_dev, const double* omega_dev, double* out_dev)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_multi before set_k_batch");
+    if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !out_dev) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_multi: null pointer");
+    if (nk <= 0 || nk > c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nk exceeds the k slots of the last set_k_batch");
+    if (nq <= 0 || (nq % 64) != 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nq must be a positive multiple of 64");
+    if ((long long)nk * nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nk*nq exceeds nq_max");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nb2 out of range");
+    if (c->nG > 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: not available while the polar term is on");
+    if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch_multi: complex input not 16-byte aligned");
+    return run_q_batch(c, nk * nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
+                       omega_dev, out_dev, nullptr, nq);
 }
 
 int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,

@@ -97,6 +97,7 @@ k_polar_amp(const double* __restrict__ q /* [nq][3] */, const double2* __restric
 // a4 (and the multi-k form of a1): batched complex128 GEMM on the FP64 tensor cores
 //     C_z[m][n] = sum_{k<K} At[k][m] * B_z[k][n]          z = blockIdx.z
 // At is [Kpad][lda] (k-major, Kpad a multiple of KC, rows K..Kpad-1 and columns >= M zero), shared by all z;
+// optionally B switches slab with the row block (rowsPerB, see the producer) -- the multi-k form of a4;
 // B_z = B + z*strideB is [K][ldb] (k-major); C_z = C + z*strideC is [M][ldc].
 //   a4:  At = Pt (phases of the q batch), B = g1' (K = nRp, N = nb1*nw*nm), C = C[q][n]
 //   a1:  At = phases of a k batch, B_z = g_W[p=z] (K = nRe, N = nw*nw*nm), C_z = T[k][p][x]
@@ -129,7 +130,8 @@ struct ContractCfg {
 template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES, bool M3, int MINB = 1>
 __global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32, MINB)
 k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ B, int ldb, long long strideB,
-           double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad, int nbatch)
+           double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad, int nbatch,
+           int rowsPerB, int rowOffset, long long strideBrow)
 {
     using Cfg = ContractCfg<BM, BN, WARPS_M, WARPS_N, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, LDA = Cfg::LDA, LDB = Cfg::LDB;
@@ -163,7 +165,10 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
             const long long z = tile / ((long long)ntn * ntm);
             const int n0 = tn * BN, m0 = tm * BM;
             const double2* a_src = At + m0;
-            const double2* b_src = B + (size_t)z * strideB + n0;
+            // rowsPerB > 0 (q batches of several k-points stacked along M): rows [j*rowsPerB, (j+1)*rowsPerB) of the
+            // whole stack take the B of k slot j (host contract: rowsPerB and rowOffset are multiples of BM)
+            const double2* b_src = B + (size_t)z * strideB + n0 +
+                                   (rowsPerB > 0 ? (size_t)((rowOffset + m0) / rowsPerB) * strideBrow : (size_t)0);
             const int bn = min(BN, N - n0);                     // valid columns of this tile
             for (int c = 0; c < nchunks; ++c) {
                 mbar_wait(empty + s, ph ^ 1u);

@@ -368,3 +368,38 @@ def test_re_pool_partial_g1_sums_to_eq71(env, batch):
     assert e.value.code == -2
     for c in ctxs:
         c.close()
+
+
+@pytest.mark.parametrize("knob", [{}, {"tile": 32}, {"nq_sub": 128}, {"m3": 0}], ids=["auto", "tile32", "sub128", "4m"])
+def test_q_batch_multi_equals_per_k_calls(env, knob):
+    """phoebe_elph_q_batch_multi: the q lists of the k slots stacked along the rows of ONE contraction, row block j
+    against the g1' of slot j -- element by element against the oracle, and bit-identical to select_k + q_batch."""
+    wl, oracle, torch, harness, binding = env["wl"], env["oracle"], env["torch"], env["harness"], env["binding"]
+    nk, nq = 5, 192
+    w = wl.custom(nw=8, nb1=4, nb2=4, nm=6, grid_e=(3, 3, 2), grid_p=(3, 3, 3), nk=nk, nq=nq, cfg_id=87)
+    gW_np, Re, Rp, ks = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w), wl.k_points(w)
+    Uks = np.stack([wl.U_k(w, ik) for ik in range(nk)])
+    ins = [wl.q_inputs(w, ik) for ik in range(nk)]
+    ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=nk * nq, nk_max=nk)
+    for key, val in knob.items():
+        ctx.set_tuning(key, val)
+    ctx.set_k_batch(ks, harness.to_device([Uks])[0])
+    stacked = harness.to_device([np.stack([ins[ik][j] for ik in range(nk)]) for j in range(4)])
+    out = ctx.q_batch_multi(*stacked)
+    assert out.shape == (nk, nq, 4, 4, 6)
+    got = out.cpu().numpy()
+    for ik in range(nk):
+        ref = oracle.elph(gW_np, Re, Rp, None, None, ks[ik], Uks[ik], *ins[ik])
+        assert _relerr(got[ik], ref) <= TOL
+        ctx.select_k(ik)
+        one = ctx.q_batch(*harness.to_device(list(ins[ik]))).cpu().numpy()
+        if "nq_sub" not in knob:
+            assert np.array_equal(one, got[ik])
+    # fewer slots than the batch holds; errors
+    part = ctx.q_batch_multi(*[t[:2].contiguous() for t in stacked]).cpu().numpy()
+    assert np.array_equal(part, got[:2])
+    for bad in ([t[:, :100].contiguous() for t in stacked],):            # nq not a multiple of 64
+        with pytest.raises(binding.PhoebeElphError) as e:
+            ctx.q_batch_multi(*bad)
+        assert e.value.code == -2
+    ctx.close()
