@@ -176,3 +176,19 @@ def qbatch_polar(g1, Rp, deg_p, q, Ukq, ev, omega, Uk, P):
                                      _p(omega), _p(Uk), _p(P), _p(out))
     assert rc == 0
     return out
+
+
+# ---- three-phonon coupling (Eq. 5), the second workload with the Eq. 70 shape ----------------------
+def v3sq(V3, R, R2, q, z, q1, z1, z2):
+    """|bare three-phonon contraction|^2 of Eq. 5 (readings R25-R27): out[nq][n0][n1][nm].
+    V3 [nR2][nR][nm][nm][nm]; z [nm][n0] at q; z1 [nq][nm][n1] at q'; z2 [nq][nm][nm] at q''."""
+    nR2, nR, nm = V3.shape[:3]
+    n0 = z.shape[1]
+    nq, _, n1 = z1.shape
+    V3 = _c(V3, np.complex128, (nR2, nR, nm, nm, nm)); R = _c(R, np.float64, (nR, 3)); R2 = _c(R2, np.float64, (nR2, 3))
+    q = _c(q, np.float64, (3,)); z = _c(z, np.complex128, (nm, n0)); q1 = _c(q1, np.float64, (nq, 3))
+    z1 = _c(z1, np.complex128, (nq, nm, n1)); z2 = _c(z2, np.complex128, (nq, nm, nm))
+    out = np.empty((nq, n0, n1, nm), dtype=np.float64)
+    rc = _load().oracle_v3sq(nR, nR2, nm, n0, n1, nq, _p(V3), _p(R), _p(R2), _p(q), _p(z), _p(q1), _p(z1), _p(z2), _p(out))
+    assert rc == 0
+    return out

@@ -362,3 +362,54 @@ int oracle_qbatch_polar(int nRp, int nw, int nm, int nb1, int nb2, int nq,
     }
     return rc;
 }
+
+/* ========================================================================
+ * SURVEY 8(f) f4 (second half) -- three-phonon coupling, Eq. 5 (L82), the second workload with the
+ * Eq. 70 shape (L137: "Eq. 5 and Eq. 13 are similar from a mathematical point of view"):
+ *
+ *   V3(q nu, q' nu', q'' nu'') = (1/N0^3)(2/hbar)^{3/2} sum_{R R'} sum_{a b c} [mass / frequency factor]
+ *        z*_{q nu}[a] z*_{q' nu'}[b] z*_{q'' nu''}[c] e^{-i(q.R + q'.R')} V3(a R, b R', c 0)
+ *
+ * Readings (R25-R27):
+ *   R25 the mass / frequency factor is printed as sqrt(m m' m'' / (omega omega' omega'')) (masses upstairs,
+ *       garbled); whatever it is, it factorises over the three phonons, so -- like 1/sqrt(m) in R6 -- it is
+ *       folded into the three eigenvector arrays by the caller, as is the constant prefactor.  The oracle (and
+ *       the library) compute the bare triple contraction and return its squared modulus.
+ *   R26 Eq. 5 prints z_{q' nu'}^{s'' beta}: the atom index of the second eigenvector is s' (the one V3 carries
+ *       with beta).
+ *   R27 all three eigenvectors are conjugated and both phases carry a MINUS sign, e^{-2 pi i (q.R + q'.R')} with
+ *       q, q' in crystal coordinates (L510) -- the opposite of Eq. 13's sign.
+ *
+ *   out[nu][nu'][nu''] = | sum_{R,R'} e^{-2 pi i q.R} e^{-2 pi i q'.R'}
+ *                          sum_{a,b,c} conj(z[a][nu]) conj(z1[b][nu']) conj(z2[c][nu'']) V3[R'][R][a][b][c] |^2
+ *
+ * Layout: V3 [nR2][nR][nm][nm][nm] (R' slowest, as g_W's [Rp][Re]); z [nm][n0], z1 [nq][nm][n1], z2 [nq][nm][nm];
+ * q [3]; q1 [nq][3]; out [nq][n0][n1][nm].  Plain 7-deep loop, long double accumulation.
+ * Pins: tests/test_oracle_v3_pins.py (VP1-VP4).
+ * ====================================================================== */
+int oracle_v3sq(int nR, int nR2, int nm, int n0, int n1, int nq, const cplx *V3, const double *R, const double *R2,
+                const double *q, const cplx *z, const double *q1, const cplx *z1, const cplx *z2, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int iq = 0; iq < nq; ++iq)
+        for (int nu = 0; nu < n0; ++nu)
+            for (int nu1 = 0; nu1 < n1; ++nu1)
+                for (int nu2 = 0; nu2 < nm; ++nu2) {
+                    long double sr = 0.0L, si = 0.0L;
+                    for (int r2 = 0; r2 < nR2; ++r2)
+                        for (int r = 0; r < nR; ++r) {
+                            cplx ph = conj(oracle_phase(q, R + 3 * r)) * conj(oracle_phase(q1 + 3 * iq, R2 + 3 * r2));
+                            cplx s = 0.0;
+                            for (int a = 0; a < nm; ++a)
+                                for (int b = 0; b < nm; ++b)
+                                    for (int c = 0; c < nm; ++c)
+                                        s += conj(z[(size_t)a * n0 + nu]) * conj(z1[((size_t)iq * nm + b) * n1 + nu1]) *
+                                             conj(z2[((size_t)iq * nm + c) * nm + nu2]) *
+                                             V3[((((size_t)r2 * nR + r) * nm + a) * nm + b) * nm + c];
+                            s *= ph;
+                            sr += creal(s); si += cimag(s);
+                        }
+                    out[(((size_t)iq * n0 + nu) * n1 + nu1) * nm + nu2] = (double)(sr * sr + si * si);
+                }
+    return 0;
+}
