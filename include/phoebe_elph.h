@@ -225,6 +225,20 @@ int phoebe_elph_copy_g1(phoebe_elph_ctx* ctx, void* dst_dev, size_t dst_bytes);
 int phoebe_elph_set_polar(phoebe_elph_ctx* ctx, const double* recip_host, int32_t nG, const double* G_host,
                           const double* Zstar_host, const double* eps_inf_host, double coeff);
 
+/* the second workload with the Eq. 70 shape: the three-phonon coupling of Eq. 5 (L82; L137, L558:
+ * "either three phonon and electron-phonon scattering ... a tensor operation in the form" of Eq. 70).  Eq. 70 is one
+ * contraction; what differs between its two uses is the sign of the Fourier phases and which rotation matrices enter
+ * conjugated.  Defaults = the el-ph reading of Eq. 13: phase_sign = +1, U_k plain, U_kq conjugated, ev plain.
+ * Eq. 5 (readings R25-R27):  phase_sign = -1 and all three conjugated, with
+ *   g_W := V3[R'][R][a][b][c] (complex128), Re := R, Rp := R', nw = nmodes = 3 x atoms,
+ *   set_k(q, z_q [nm][n0]),  q_batch(q', z_{q'} [nq][nm][n1], z_{q''} [nq][nm][nm], omega := 0.5)  ->
+ *   out[q'][nu][nu'][nu''] = |sum_{R,R'} e^{-2 pi i (q.R + q'.R')} sum_{abc} z*[a][nu] z'*[b][nu'] z''*[c][nu''] V3|^2
+ * (mass / frequency factors of Eq. 5 folded into the eigenvectors by the caller, as in q_batch; with omega = 0.5 the
+ * final 1/(2 omega) is 1).  Invalidates the current set_k.  Not combinable with the polar term.
+ * Errors: E_NULL, E_DIMS. */
+int phoebe_elph_set_conventions(phoebe_elph_ctx* ctx, int32_t phase_sign, int32_t conj_Uk, int32_t conj_Ukq,
+                                int32_t conj_ev);
+
 /* the paper's "pool" (L576): when g(Re,Rp) does not fit one GPU it is distributed over Re.
  * Eq. 71 is linear in g_W, so a rank that was set up with ITS Re vectors and ITS slab g_W[nRp][nRe_local][...]
  * gets from set_k / set_k_batch the partial g1' of its shard; the sum over the ranks is the g1' of Eq. 71.

@@ -22,7 +22,7 @@ EXPORTS = [
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_multi", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
-    "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_launch_counts",
+    "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_set_conventions", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
     "phoebe_elph_version",
@@ -78,6 +78,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.phoebe_elph_set_polar.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_double]
+    lib.phoebe_elph_set_conventions.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int32]
     lib.phoebe_elph_g1_buffer.argtypes = [c_void_p, c_int32, POINTER(c_void_p), POINTER(c_size_t), POINTER(c_size_t)]
     lib.phoebe_elph_launch_counts.argtypes = [c_void_p, POINTER(c_int64)]
     lib.phoebe_elph_profile.argtypes = [c_void_p, c_int32]
@@ -325,6 +326,13 @@ class ElphContext:
         assert Zstar.shape == (self.dims.nmodes // 3, 3, 3)
         self._check(self._lib.phoebe_elph_set_polar(self._ctx, recip.ctypes.data, len(G), G.ctypes.data, Zstar.ctypes.data,
                                                     eps_inf.ctypes.data, float(coeff)), "phoebe_elph_set_polar")
+
+    def set_conventions(self, phase_sign=1, conj_Uk=False, conj_Ukq=True, conj_ev=False):
+        """Sign of the Fourier phases and conjugation of the three rotation matrices of Eq. 70 (defaults: el-ph,
+        Eq. 13; three-phonon coupling of Eq. 5: phase_sign=-1, all three conjugated)."""
+        self._check(self._lib.phoebe_elph_set_conventions(self._ctx, int(phase_sign), int(bool(conj_Uk)),
+                                                          int(bool(conj_Ukq)), int(bool(conj_ev))),
+                    "phoebe_elph_set_conventions")
 
     def g1_view(self, slot: int = -1):
         """float64 view (no copy) of the g1' storage inside the workspace: slot >= 0 -> that k slot's

@@ -159,6 +159,9 @@ struct phoebe_elph_ctx {
     // f4: polar long-range term (Eq. 14-15); nG == 0 = off
     int nG = 0;
     pe::PolarParams polar{};
+    // set_conventions: sign of both Fourier phases and which of the three rotation matrices enter conjugated
+    double phase_sign = 1.0;
+    bool conj_Uk = false, conj_Ukq = true, conj_ev = false;
     int k_sel = 0;            // k slot chosen by select_k (its U_k is needed for the overlap of Eq. 15)
     bool prof = false;
     std::vector<EventPair> evs;
@@ -248,17 +251,17 @@ int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double
         const int ng = ceil_div(nb1, 4);
         dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
         pe::k_setk_rotate<4><<<grid, TR, (size_t)d.nw * 4 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N, ng,
-                                                                             strideT, strideG);
+                                                                             strideT, strideG, c->conj_Uk ? 1 : 0);
     } else if (nb1 <= 8) {
         const int ng = ceil_div(nb1, 8);
         dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
         pe::k_setk_rotate<8><<<grid, TR, (size_t)d.nw * 8 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N, ng,
-                                                                             strideT, strideG);
+                                                                             strideT, strideG, c->conj_Uk ? 1 : 0);
     } else {
         const int ng = ceil_div(nb1, 16);
         dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
         pe::k_setk_rotate<16><<<grid, TR, (size_t)d.nw * 16 * 16, c->stream>>>(T, Uk_dev, S, d.nRp, d.nw, Y, nb1, g1, N,
-                                                                               ng, strideT, strideG);
+                                                                               ng, strideT, strideG, c->conj_Uk ? 1 : 0);
     }
     PE_CUDA(c, cudaGetLastError());
     return PHOEBE_ELPH_OK;
@@ -285,7 +288,7 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
     {
         LaunchScope ls(c, PHOEBE_ELPH_K_SETK_STREAM);
         dim3 grid(ceil_div(X, T), S, d.nRp);
-        pe::k_setk_stream<<<grid, T, (size_t)epc * 16, c->stream>>>(c->gW, c->Re, c->deg_e, k[0], k[1], k[2], d.nRe,
+        pe::k_setk_stream<<<grid, T, (size_t)epc * 16, c->stream>>>(c->gW, c->Re, c->deg_e, c->phase_sign * k[0], c->phase_sign * k[1], c->phase_sign * k[2], d.nRe,
                                                                     d.nRp, X, epc, c->Tpart);
         PE_CUDA(c, cudaGetLastError());
     }
@@ -310,7 +313,8 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     {
         LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
         dim3 grid(1, std::min(c->L.KpadE, 256));
-        pe::k_qphase<<<grid, 32, 0, c->stream>>>(c->kdev, c->Re, c->deg_e, nk, d.nRe, c->L.KpadE, kKBatchMax, c->Ptk);
+        pe::k_qphase<<<grid, 32, 0, c->stream>>>(c->kdev, c->Re, c->deg_e, nk, d.nRe, c->L.KpadE, kKBatchMax, c->Ptk,
+                                                 c->phase_sign);
         PE_CUDA(c, cudaGetLastError());
     }
     {
@@ -397,7 +401,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         rot_smem += ((size_t)QG * 8 * NT + (size_t)QG * nb1 * 8 * ceil_div(nb2, 8)) * 16;
     if (rot_smem > (227u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
     double2* Pbuf = reinterpret_cast<double2*>(c->ws + c->L.off_P);
-    pe::PolarArgs pa{nullptr, c->Uk + (size_t)c->k_sel * d.nw * nb1};
+    pe::PolarArgs pa{nullptr, c->Uk + (size_t)c->k_sel * d.nw * nb1, (c->conj_Ukq ? 0 : 1) | (c->conj_ev ? 2 : 0)};
     if (rr && !use_mma && out == nullptr)      // the plain path sums from the stored |g|^2: keep it in the staging area
         out = reinterpret_cast<double*>(c->ws + c->L.off_sout);
     auto rot_kernel = [&]() -> const void* {
@@ -435,7 +439,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
             dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
             pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
-                                                      c->L.ldq, c->Pt);
+                                                      c->L.ldq, c->Pt, c->phase_sign);
             PE_CUDA(c, cudaGetLastError());
         }
         {
@@ -841,12 +845,26 @@ int phoebe_elph_set_polar(phoebe_elph_ctx* c, const double* recip_host, int32_t 
     if (!recip_host || !G_host || !Zstar_host || !eps_inf_host) return fail(c, PHOEBE_ELPH_E_NULL, "set_polar: null pointer");
     if (nG < 0 || nG > kMaxG) return fail(c, PHOEBE_ELPH_E_DIMS, "set_polar: nG out of range (<= 4096)");
     if (c->dims.nmodes % 3) return fail(c, PHOEBE_ELPH_E_DIMS, "set_polar: nmodes is not 3 x atoms");
+    if (c->phase_sign != 1.0 || c->conj_Uk || !c->conj_Ukq || c->conj_ev)
+        return fail(c, PHOEBE_ELPH_E_DIMS, "set_polar: the polar term belongs to the el-ph conventions");
     PE_CUDA(c, cudaMemcpyAsync(c->ws + c->L.off_G, G_host, (size_t)nG * 24, cudaMemcpyHostToDevice, c->stream));
     PE_CUDA(c, cudaMemcpyAsync(c->ws + c->L.off_Zstar, Zstar_host, (size_t)(c->dims.nmodes / 3) * 72, cudaMemcpyHostToDevice, c->stream));
     PE_CUDA(c, cudaStreamSynchronize(c->stream));      // the host arrays may be pageable
     for (int i = 0; i < 9; ++i) { c->polar.recip[i] = recip_host[i]; c->polar.eps[i] = eps_inf_host[i]; }
     c->polar.coeff = coeff;
     c->nG = nG;
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_set_conventions(phoebe_elph_ctx* c, int32_t phase_sign, int32_t conj_Uk, int32_t conj_Ukq, int32_t conj_ev)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (phase_sign != 1 && phase_sign != -1) return fail(c, PHOEBE_ELPH_E_DIMS, "set_conventions: phase_sign must be +1 or -1");
+    const bool dflt = phase_sign == 1 && !conj_Uk && conj_Ukq && !conj_ev;
+    if (!dflt && c->nG > 0) return fail(c, PHOEBE_ELPH_E_DIMS, "set_conventions: the polar term belongs to the el-ph conventions");
+    c->phase_sign = (double)phase_sign;
+    c->conj_Uk = conj_Uk != 0; c->conj_Ukq = conj_Ukq != 0; c->conj_ev = conj_ev != 0;
+    c->have_k = false;                  // a g1' computed under other conventions must not be reused
     return PHOEBE_ELPH_OK;
 }
 

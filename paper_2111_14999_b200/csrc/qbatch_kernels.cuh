@@ -17,7 +17,8 @@ namespace pe {
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rp, const double* __restrict__ deg_p,
-         int nq, int nRp, int Kpad, int ldq, double2* __restrict__ Pt /* [Kpad][ldq] */)
+         int nq, int nRp, int Kpad, int ldq, double2* __restrict__ Pt /* [Kpad][ldq] */,
+         double sgn /* +1: e^{+2 pi i q.R} (Eq. 13); -1: e^{-2 pi i q.R} (Eq. 5, set_conventions) */)
 {
     const int iq = blockIdx.x * blockDim.x + threadIdx.x;
     if (iq >= ldq) return;
@@ -31,7 +32,7 @@ k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ 
             double sn, cs;
             sincospi(2.0 * x, &sn, &cs);
             const double w = 1.0 / deg_p[p];
-            v = make_double2(cs * w, sn * w);
+            v = make_double2(cs * w, sgn * sn * w);
         }
         Pt[(size_t)p * ldq + iq] = v;
     }
@@ -337,6 +338,7 @@ struct RateArgs {
 struct PolarArgs {
     const double2* P;     // [nq][nm] of this launch, or nullptr
     const double2* Uk;    // [nw][nb1]
+    int conv;             // set_conventions: bit 0 = U_kq enters PLAIN (default: conjugated), bit 1 = ev enters CONJUGATED
 };
 
 template <int NT, bool RATES>
@@ -388,13 +390,15 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
         const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
         const int w2 = r / ldu, b2 = r - w2 * ldu;
         double2 u = make_double2(0.0, 0.0);
-        if (w2 < nw && b2 < nb2) { u = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2]; u.y = -u.y; }
+        if (w2 < nw && b2 < nb2) { u = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2]; if (!(pa.conv & 1)) u.y = -u.y; }
         Us[i] = u;
     }
     for (int i = threadIdx.x; i < nql * 8 * NT * ldz; i += blockDim.x) {
         const int ql = i / (8 * NT * ldz), r = i - ql * 8 * NT * ldz;
         const int ka = r / ldz, nu = r - ka * ldz;
-        Zs[i] = (ka < nm && nu < nm) ? ev[((size_t)(q0 + ql) * nm + ka) * nm + nu] : make_double2(0.0, 0.0);
+        double2 zv = (ka < nm && nu < nm) ? ev[((size_t)(q0 + ql) * nm + ka) * nm + nu] : make_double2(0.0, 0.0);
+        if (pa.conv & 2) zv.y = -zv.y;
+        Zs[i] = zv;
     }
     for (int i = threadIdx.x; i < nql * 8 * NT; i += blockDim.x) {
         const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
@@ -598,9 +602,9 @@ k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restr
     const int nb1l = min(gb1, nb1 - b10);
     const int Y = nw * nm;
     const double2* Uq = Ukq + (size_t)iq * nw * nb2;
-    for (int i = threadIdx.x; i < nw * nb2; i += blockDim.x) { double2 u = Uq[i]; Uc[i] = make_double2(u.x, -u.y); }
+    for (int i = threadIdx.x; i < nw * nb2; i += blockDim.x) { double2 u = Uq[i]; Uc[i] = make_double2(u.x, (pa.conv & 1) ? u.y : -u.y); }
     const double2* Zq = ev + (size_t)iq * nm * nm;
-    for (int i = threadIdx.x; i < nm * nm; i += blockDim.x) Z[i] = Zq[i];
+    for (int i = threadIdx.x; i < nm * nm; i += blockDim.x) { double2 zv = Zq[i]; if (pa.conv & 2) zv.y = -zv.y; Z[i] = zv; }
     const double2* Cq = C + (size_t)iq * ldc + (size_t)b10 * Y;
     for (int i = threadIdx.x; i < nb1l * Y; i += blockDim.x) Cs[i] = Cq[i];
     __syncthreads();

@@ -67,7 +67,7 @@ template <int NBT>
 __global__ void __launch_bounds__(128)
 k_setk_rotate(const double2* __restrict__ Tpart, const double2* __restrict__ Uk /* [nk][nw][nb1] */,
               int S, int nRp, int nw, int Y, int nb1, double2* __restrict__ g1 /* [nk][nRp][nb1][Y] */, int ldg,
-              int ngroups, long long strideT, long long strideG)
+              int ngroups, long long strideT, long long strideG, int conjU /* set_conventions: U_k enters conjugated */)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* U = reinterpret_cast<double2*>(smem_raw);           // [nw][NBT]
@@ -78,7 +78,9 @@ k_setk_rotate(const double2* __restrict__ Tpart, const double2* __restrict__ Uk 
     g1 += (size_t)ik * strideG;
     for (int i = threadIdx.x; i < nw * NBT; i += blockDim.x) {
         int w1 = i / NBT, b = i % NBT;
-        U[i] = (b0 + b < nb1) ? Uk[(size_t)w1 * nb1 + b0 + b] : make_double2(0.0, 0.0);
+        double2 u = (b0 + b < nb1) ? Uk[(size_t)w1 * nb1 + b0 + b] : make_double2(0.0, 0.0);
+        if (conjU) u.y = -u.y;
+        U[i] = u;
     }
     __syncthreads();
     const int p = blockIdx.y;
