@@ -234,9 +234,12 @@ cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persist
     //  loads in flight while this one stores; it passes persistent = false)
     if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int grid = persistent ? (int)std::min<long long>(ntiles, (long long)kSMs * ctas_per_sm) : (int)ntiles;
+    // persistent grid: panels as wide as the grid (each CTA keeps one column tile per panel, B panel L2-resident);
+    // one-tile-per-CTA grid: plain n-fastest order
+    const int panelW = persistent ? grid : 0x7fffffff;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(g.At, g.lda, g.B, g.ldb, g.strideB, g.C, g.ldc, g.strideC,
                                                            g.M, g.N, g.K, g.Kpad, g.batch, g.rowsPerB, g.rowOffset,
-                                                           g.strideBrow);
+                                                           g.strideBrow, panelW);
     return cudaGetLastError();
 }
 
