@@ -69,7 +69,8 @@ enum {
     PHOEBE_ELPH_K_SETK_GEMM   = 5,  /* a1 for a batch of k: one pass over g_W (FP64 GEMM, DMMA) */
     PHOEBE_ELPH_K_RATE_REDUCE = 6,  /* f2: fixed-order sum of the per-CTA linewidth partials    */
     PHOEBE_ELPH_K_POLAR       = 7,  /* f4: (q, nu) amplitudes of the polar long-range term        */
-    PHOEBE_ELPH_K_COUNT       = 8
+    PHOEBE_ELPH_K_PACK        = 8,  /* g1' -> planar blocked operand of the planar contraction    */
+    PHOEBE_ELPH_K_COUNT       = 9
 };
 
 /* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
@@ -269,6 +270,8 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               T3 = (Ar+Ai).(Br+Bi); Re = T1-T2, Im = T3-T1-T2: 6 instead of 8 real flop per complex MAC,
  *               normwise FP64-accurate); 0 = the four-multiply product
  *   "tile"      contraction CTA tile: 0 = automatic (cost model), 32 or 64
+ *   "planar"    1 (default) = a4 through the planar-operand contraction (re / im / re+im planes blocked by 64
+ *               columns, one LDS.128 feeds two DMMA tiles, no operand-sum DADDs); 0 = the interleaved-complex kernel
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)           */
 int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
 int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);

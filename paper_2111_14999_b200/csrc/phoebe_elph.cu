@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "probe_kernels.cuh"
+#include "contract_planar.cuh"
 #include "qbatch_kernels.cuh"
 #include "setk_kernels.cuh"
 
@@ -51,8 +52,9 @@ int setk_auto_split(int nRe, int nRp, int X)
 struct Layout {
     int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
+    size_t g1P_stride = 0;  // doubles between the planar blocked copies of g1' (k_contract_planar) of consecutive k slots
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
-           off_g1 = 0, off_Pt = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_g1P = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
@@ -92,7 +94,11 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_Ptk = take((size_t)L.KpadE * kKBatchMax * 16);
     L.off_Tpart = take((size_t)std::max(L.S_alloc, L.nk_slots) * d.nRp * X * 16);
     L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
+    // planar blocked copies ([rows][tiles of 64][3][64] doubles) of g1' and of the phases for k_contract_planar
+    L.g1P_stride = (size_t)d.nRp * ceil_div((int)N, 64) * 192;
+    L.off_g1P = take((size_t)L.nk_slots * L.g1P_stride * 8);
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
+    L.off_PtP = take((size_t)L.Kpad * L.ldq * 24);
     L.off_C = take((size_t)L.nq_sub * N * 16);
     // f2: per-CTA linewidth partials [<= nq_max CTAs][nb1], staging of rate / eps_k / eps_kq for the host entry point
     L.off_part = take((size_t)nq_max * d.nb1_max * 8);
@@ -150,7 +156,7 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
-    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
@@ -162,6 +168,9 @@ struct phoebe_elph_ctx {
     // set_conventions: sign of both Fourier phases and which of the three rotation matrices enter conjugated
     double phase_sign = 1.0;
     bool conj_Uk = false, conj_Ukq = true, conj_ev = false;
+    double *g1P = nullptr, *PtP = nullptr;   // planar blocked operands of k_contract_planar
+    bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
+    bool g1P_stale = true;    // canonical g1' changed (set_k, or handed out by g1_buffer) since the last pack
     int k_sel = 0;            // k slot chosen by select_k (its U_k is needed for the overlap of Eq. 15)
     bool prof = false;
     std::vector<EventPair> evs;
@@ -299,6 +308,7 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
     if (rc) return rc;
     c->nb1 = nb1;
     c->nk_have = 1;
+    c->g1P_stale = true;
     c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
@@ -317,7 +327,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
         LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
         dim3 grid(1, std::min(c->L.KpadE, 256));
         pe::k_qphase<<<grid, 32, 0, c->stream>>>(c->kdev, c->Re, c->deg_e, nk, d.nRe, c->L.KpadE, kKBatchMax, c->Ptk,
-                                                 c->phase_sign);
+                                                 c->phase_sign, nullptr);
         PE_CUDA(c, cudaGetLastError());
     }
     {
@@ -343,6 +353,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     }
     c->nb1 = nb1;
     c->nk_have = nk;
+    c->g1P_stale = true;
     c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
@@ -438,11 +449,26 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     for (int qs = 0; qs < nq; qs += nq_sub) {
         const int nqs = std::min(nq_sub, nq - qs);
         const int ncols = (int)align_up((size_t)nqs, kQPad);
+        // contraction tile: 64x64 unless that leaves the 148 SMs with a long ragged tail (few tiles);
+        // cost model = rounds of tiles per SM x tile area (+5 % for the smaller tile's extra operand traffic)
+        const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64;
+        const double cost32 = (double)ceil_div(ceil_div(nqs, 32) * ceil_div(N, 32), kSMs) * 32 * 32 * 1.05;
+        int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
+        if (rows_per_k > 0 && tile != 32 && tile != 64) tile = 64;       // the stacked form knows these two tiles
+        const bool use_planar = c->m3 && c->planar && tile == 64;
+        if (use_planar && c->g1P_stale) {      // canonical g1' of every filled k slot -> planar blocked copy
+            LaunchScope ls(c, PHOEBE_ELPH_K_PACK);
+            dim3 grid(ceil_div(N, 64), d.nRp, c->nk_have);
+            pe::k_pack_planar<<<grid, 64, 0, c->stream>>>(c->g1_base, (long long)N, (long long)c->L.g1_stride, N, c->g1P,
+                                                          (long long)c->L.g1P_stride);
+            PE_CUDA(c, cudaGetLastError());
+            c->g1P_stale = false;
+        }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
             dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
             pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
-                                                      c->L.ldq, c->Pt, c->phase_sign);
+                                                      c->L.ldq, c->Pt, c->phase_sign, use_planar ? c->PtP : nullptr);
             PE_CUDA(c, cudaGetLastError());
         }
         {
@@ -451,13 +477,21 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             if (rows_per_k > 0) {
                 g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
             }
-            // tile choice: 64x64 unless that leaves the 148 SMs with a long ragged tail (few tiles);
-            // cost model = rounds of tiles per SM x tile area (+5 % for the smaller tile's extra operand traffic)
-            const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64;
-            const double cost32 = (double)ceil_div(ceil_div(nqs, 32) * ceil_div(N, 32), kSMs) * 32 * 32 * 1.05;
-            int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
-            if (rows_per_k > 0 && tile != 32 && tile != 64) tile = 64;       // the stacked form knows these two tiles
-            if (c->m3) {
+            if (use_planar) {
+                static bool attr_set = false;
+                if (!attr_set) {
+                    PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_planar, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)pe::PlanarCfg::kSmemBytes));
+                    attr_set = true;
+                }
+                const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
+                const int grid = std::min(ntiles, kSMs);
+                const int slot = rows_per_k > 0 ? 0 : c->k_sel;
+                pe::k_contract_planar<<<grid, pe::PlanarCfg::kThreads, pe::PlanarCfg::kSmemBytes, c->stream>>>(
+                    c->PtP, c->L.ldq / 64, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64),
+                    (long long)c->L.g1P_stride, c->C, (long long)N, nqs, N, d.nRp, c->L.Kpad, rows_per_k, qs, grid);
+                PE_CUDA(c, cudaGetLastError());
+            } else if (c->m3) {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
                 else if (tile == 6432) PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true, 2>(c->stream, g)));
                 else PE_CUDA(c, (launch_contract<64, 64, 2, 4, 16, 4, true>(c->stream, g)));
@@ -582,6 +616,8 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     c->kdev = reinterpret_cast<double*>(c->ws + L.off_kdev);
     c->Ptk = reinterpret_cast<double2*>(c->ws + L.off_Ptk);
     c->Pt = reinterpret_cast<double2*>(c->ws + L.off_Pt);
+    c->g1P = reinterpret_cast<double*>(c->ws + L.off_g1P);
+    c->PtP = reinterpret_cast<double*>(c->ws + L.off_PtP);
     c->C = reinterpret_cast<double2*>(c->ws + L.off_C);
 
     std::vector<double> ones((size_t)std::max(dims->nRe, dims->nRp), 1.0);
@@ -879,6 +915,7 @@ int phoebe_elph_g1_buffer(phoebe_elph_ctx* c, int32_t slot, void** ptr_out, size
     if (slot < -1 || slot >= c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "g1_buffer: slot out of range");
     const size_t one = (size_t)c->dims.nRp * c->nb1 * c->dims.nw * c->dims.nmodes * 16;
     const size_t stride = c->L.g1_stride * 16;
+    c->g1P_stale = true;                 // the caller may change g1' in place (Re-pool all-reduce): re-pack before the next a4
     if (stride_out) *stride_out = stride;
     if (slot >= 0) {
         *ptr_out = c->g1_base + (size_t)slot * c->L.g1_stride;
@@ -936,6 +973,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "m3")) { c->m3 = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "planar")) { c->planar = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "s_split")) {
         if (value < 0 || value > c->L.S_alloc) return fail(c, PHOEBE_ELPH_E_DIMS, "s_split out of range");

@@ -18,7 +18,8 @@ namespace pe {
 __global__ void __launch_bounds__(256)
 k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rp, const double* __restrict__ deg_p,
          int nq, int nRp, int Kpad, int ldq, double2* __restrict__ Pt /* [Kpad][ldq] */,
-         double sgn /* +1: e^{+2 pi i q.R} (Eq. 13); -1: e^{-2 pi i q.R} (Eq. 5, set_conventions) */)
+         double sgn /* +1: e^{+2 pi i q.R} (Eq. 13); -1: e^{-2 pi i q.R} (Eq. 5, set_conventions) */,
+         double* __restrict__ PtP /* planar blocked copy [Kpad][ldq/64][3][64] for k_contract_planar, or nullptr */)
 {
     const int iq = blockIdx.x * blockDim.x + threadIdx.x;
     if (iq >= ldq) return;
@@ -34,7 +35,12 @@ k_qphase(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ 
             const double w = 1.0 / deg_p[p];
             v = make_double2(cs * w, sgn * sn * w);
         }
-        Pt[(size_t)p * ldq + iq] = v;
+        if (PtP) {
+            double* d = PtP + ((size_t)p * (ldq >> 6) + (iq >> 6)) * 192 + (iq & 63);
+            d[0] = v.x; d[64] = v.y; d[128] = v.x + v.y;
+        } else {
+            Pt[(size_t)p * ldq + iq] = v;
+        }
     }
 }
 

@@ -101,7 +101,7 @@ def test_ragged_small_cases(env, case, host):
 
 
 @pytest.mark.parametrize("knob", [{"tile": 32, "m3": 0}, {"tile": 64, "m3": 0}, {"tile": 32, "m3": 1},
-                                  {"tile": 64, "m3": 1}, {"rot_plain": 1}],
+                                  {"tile": 64, "m3": 1}, {"tile": 64, "m3": 1, "planar": 0}, {"rot_plain": 1}],
                          ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
 def test_forced_kernel_variants(env, knob):
     """Every kernel variant the dispatcher can pick is parity-checked on the same input."""
@@ -370,7 +370,8 @@ def test_re_pool_partial_g1_sums_to_eq71(env, batch):
         c.close()
 
 
-@pytest.mark.parametrize("knob", [{}, {"tile": 32}, {"nq_sub": 128}, {"m3": 0}], ids=["auto", "tile32", "sub128", "4m"])
+@pytest.mark.parametrize("knob", [{}, {"tile": 32}, {"nq_sub": 128}, {"m3": 0}, {"tile": 64, "planar": 0}, {"tile": 64}],
+                         ids=["auto", "tile32", "sub128", "4m", "tile64_interleaved", "tile64_planar"])
 def test_q_batch_multi_equals_per_k_calls(env, knob):
     """phoebe_elph_q_batch_multi: the q lists of the k slots stacked along the rows of ONE contraction, row block j
     against the g1' of slot j -- element by element against the oracle, and bit-identical to select_k + q_batch."""
