@@ -148,9 +148,12 @@ k_contract_planar(const double* __restrict__ AtP, int ntmA, const double* __rest
             for (int pl = 0; pl < 3; ++pl) {
                 a[0][pl][0] = lda2(0, pl, 0); a[0][pl][1] = lda2(0, pl, 1); b[0][pl] = ldb2(0, pl);
             }
+            // the last chunk runs only the k-steps that hold rows < K (K = 343: 2 of 4), a warp-uniform branch
+            const int ks_n = min(KS, (K + 3 - c * KC) >> 2);
 #pragma unroll
             for (int k4 = 0; k4 < KS; ++k4) {
                 const int cur = k4 & 1, nxt = cur ^ 1;
+                if (k4 >= ks_n) break;
                 if (k4 + 1 < KS) {
 #pragma unroll
                     for (int pl = 0; pl < 3; ++pl) {
