@@ -487,9 +487,13 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs);
                 const int slot = rows_per_k > 0 ? 0 : c->k_sel;
+                // panel width: a divisor of the grid (each CTA keeps its column tile for a whole panel) small enough
+                // that the panel of g1P (width x K x 1536 B) stays L2-resident next to the streaming phase rows and C
+                int panelW = grid;
+                while (panelW % 2 == 0 && (size_t)panelW * d.nRp * pe::PlanarCfg::ROW * 8 > (48u << 20)) panelW /= 2;
                 pe::k_contract_planar<<<grid, pe::PlanarCfg::kThreads, pe::PlanarCfg::kSmemBytes, c->stream>>>(
                     c->PtP, c->L.ldq / 64, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64),
-                    (long long)c->L.g1P_stride, c->C, (long long)N, nqs, N, d.nRp, c->L.Kpad, rows_per_k, qs, grid);
+                    (long long)c->L.g1P_stride, c->C, (long long)N, nqs, N, d.nRp, c->L.Kpad, rows_per_k, qs, panelW);
                 PE_CUDA(c, cudaGetLastError());
             } else if (c->m3) {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
