@@ -431,7 +431,7 @@ def run_ours(args):
         barrier()
         ms_r = maxreduce(e0.elapsed_time(e1))
         eps_pin = [[torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in e] for e in eps_np]
-        rate_h = np.zeros((len(dev_inputs), w.nb1))
+        rate_h = torch.zeros((len(dev_inputs), w.nb1), dtype=torch.float64).pin_memory().numpy()
 
         def step_rates_e2e():
             for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
@@ -442,8 +442,9 @@ def run_ours(args):
                 for j, i in enumerate(g):
                     ctx.select_k(j)
                     _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
-                    ctx.q_batch_rates_host(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(), eps_pin[i][0].numpy(),
-                                           eps_pin[i][1].numpy(), rate_h[i], **P)
+                    ctx.q_batch_rates_host_async(q_p.numpy(), Ukq_p.numpy(), ev_p.numpy(), om_p.numpy(),
+                                                 eps_pin[i][0].numpy(), eps_pin[i][1].numpy(), rate_h[i], **P)
+            ctx.wait()
 
         step_rates_e2e()
         barrier()

@@ -207,6 +207,16 @@ int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2
                                    const double* omega_host, const double* eps_k_host, const double* eps_kq_host,
                                    const phoebe_elph_rate_params* prm, double* rate_host, double* out_host);
 
+/* Pipelined form of q_batch_rates_host, on the same two staging slots and streams as q_batch_host_async (the two may
+ * be mixed; phoebe_elph_wait ends both).  rate_host [nb1] is read when the call is made, accumulated into on the device
+ * and written back by the copy-out stream: give every call in flight its OWN rate array (e.g. one per k-point) and read it
+ * after phoebe_elph_wait.  out_host may be NULL.  Host buffers should be page-locked.
+ * Errors: as q_batch_rates_host. */
+int phoebe_elph_q_batch_rates_host_async(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
+                                         const double* q_host, const void* Ukq_host, const void* ev_host,
+                                         const double* omega_host, const double* eps_k_host, const double* eps_kq_host,
+                                         const phoebe_elph_rate_params* prm, double* rate_host, double* out_host);
+
 /* Copy the current g1' (complex128 [nRp][nb1][nw][nmodes]) to dst_dev (DEVICE, >= bytes
  * nRp*nb1*nw*nmodes*16); for tests of set_k on its own.  Errors: E_NULL, E_NO_K, E_WORKSPACE, E_CUDA. */
 int phoebe_elph_copy_g1(phoebe_elph_ctx* ctx, void* dst_dev, size_t dst_bytes);

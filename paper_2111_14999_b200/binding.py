@@ -21,7 +21,7 @@ EXPORTS = [
     "phoebe_elph_workspace_bytes", "phoebe_elph_setup", "phoebe_elph_set_k", "phoebe_elph_set_k_host",
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_multi", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
-    "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host",
+    "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host", "phoebe_elph_q_batch_rates_host_async",
     "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_set_conventions", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
@@ -76,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_wait.argtypes = [c_void_p]
     lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
+    lib.phoebe_elph_q_batch_rates_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.phoebe_elph_set_polar.argtypes = [c_void_p, c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_double]
     lib.phoebe_elph_set_conventions.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int32]
@@ -305,6 +306,17 @@ class ElphContext:
             self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data, ev.ctypes.data, omega.ctypes.data, eps_k.ctypes.data,
             eps_kq.ctypes.data, byref(prm), rate.ctypes.data, None if out is None else out.ctypes.data),
             "phoebe_elph_q_batch_rates_host")
+        return rate, out
+
+    def q_batch_rates_host_async(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):
+        """Pipelined q_batch_rates_host (NumPy views of PINNED memory; one rate array per call in flight); returns at
+        once -- call wait() before reading rate / out."""
+        nq, nw, nb2 = Ukq.shape
+        prm = RateParams(kT, mu, sigma, pref)
+        self._check(self._lib.phoebe_elph_q_batch_rates_host_async(
+            self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data, ev.ctypes.data, omega.ctypes.data, eps_k.ctypes.data,
+            eps_kq.ctypes.data, byref(prm), rate.ctypes.data, None if out is None else out.ctypes.data),
+            "phoebe_elph_q_batch_rates_host_async")
         return rate, out
 
     def copy_g1(self):

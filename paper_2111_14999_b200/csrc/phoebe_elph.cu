@@ -102,8 +102,8 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_C = take((size_t)L.nq_sub * N * 16);
     // f2: per-CTA linewidth partials [<= nq_max CTAs][nb1], staging of rate / eps_k / eps_kq for the host entry point
     L.off_part = take((size_t)nq_max * d.nb1_max * 8);
-    L.off_rate = take((size_t)2 * d.nb1_max * 8);
-    L.off_seps = take((size_t)nq_max * d.nb2_max * 8);
+    L.off_rate = take((size_t)2 * 2 * d.nb1_max * 8);                 // two slots of (rate, eps_k)
+    L.off_seps = take((size_t)2 * nq_max * d.nb2_max * 8);            // two slots of eps_kq
     // f4: G list and Born charges of the polar term, its (q, nu) amplitudes
     L.off_G = take((size_t)kMaxG * 3 * 8);
     L.off_Zstar = take((size_t)ceil_div(d.nmodes, 3) * 9 * 8);
@@ -745,14 +745,15 @@ int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const 
     return PHOEBE_ELPH_OK;
 }
 
-int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
-                                   const void* ev_host, const double* omega_host, double* out_host)
+}  // extern "C"
+
+namespace {
+struct RateHost { const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate; };
+
+// one pipelined host batch: copy-in stream -> compute stream -> copy-out stream over staging slot (n mod 2)
+int async_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
+                const void* ev_host, const double* omega_host, double* out_host, const RateHost* rh)
 {
-    if (!c) return PHOEBE_ELPH_E_NULL;
-    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_host_async before set_k");
-    if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host_async: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nq out of range");
-    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nb2 out of range");
     if (!c->async_ready) {
         PE_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
         PE_CUDA(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
@@ -782,19 +783,65 @@ int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, 
     PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->s_in));
     PE_CUDA(c, cudaMemcpyAsync(sZ, ev_host, (size_t)nq * d.nmodes * d.nmodes * 16, cudaMemcpyHostToDevice, c->s_in));
     PE_CUDA(c, cudaMemcpyAsync(sw, omega_host, (size_t)nq * d.nmodes * 8, cudaMemcpyHostToDevice, c->s_in));
+    double* srate = reinterpret_cast<double*>(c->ws + c->L.off_rate) + (size_t)slot * 2 * d.nb1_max;
+    double* se1 = srate + d.nb1_max;
+    double* se2 = reinterpret_cast<double*>(c->ws + c->L.off_seps) + (size_t)slot * d.nq_max * d.nb2_max;
+    if (rh) {
+        PE_CUDA(c, cudaMemcpyAsync(srate, rh->rate, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
+        PE_CUDA(c, cudaMemcpyAsync(se1, rh->eps_k, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
+        PE_CUDA(c, cudaMemcpyAsync(se2, rh->eps_kq, (size_t)nq * nb2 * 8, cudaMemcpyHostToDevice, c->s_in));
+    }
     PE_CUDA(c, cudaEventRecord(c->ev_in[slot], c->s_in));
     // compute stream: inputs in, and the copy-out that last read this output slot done
     PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[slot], 0));
     if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[slot], 0));
-    int rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
+    int rc;
+    if (rh) {
+        RateReq rr{se1, se2, rh->prm, srate};
+        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, out_host ? so : nullptr, &rr);
+    } else {
+        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
+    }
     if (rc) return rc;
     PE_CUDA(c, cudaEventRecord(c->ev_done[slot], c->stream));
     // copy-out stream
     PE_CUDA(c, cudaStreamWaitEvent(c->s_out, c->ev_done[slot], 0));
-    PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->s_out));
+    if (rh) PE_CUDA(c, cudaMemcpyAsync(rh->rate, srate, (size_t)c->nb1 * 8, cudaMemcpyDeviceToHost, c->s_out));
+    if (out_host)
+        PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->s_out));
     PE_CUDA(c, cudaEventRecord(c->ev_out[slot], c->s_out));
     c->async_n++;
     return PHOEBE_ELPH_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
+                                   const void* ev_host, const double* omega_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_host_async before set_k");
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host_async: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nb2 out of range");
+    return async_batch(c, nq, nb2, q_host, Ukq_host, ev_host, omega_host, out_host, nullptr);
+}
+
+int phoebe_elph_q_batch_rates_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host,
+                                         const void* Ukq_host, const void* ev_host, const double* omega_host,
+                                         const double* eps_k_host, const double* eps_kq_host,
+                                         const phoebe_elph_rate_params* prm, double* rate_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates_host_async before set_k");
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !eps_k_host || !eps_kq_host || !prm || !rate_host)
+        return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_host_async: null pointer");
+    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: nq out of range");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: nb2 out of range");
+    if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: kT and sigma must be > 0");
+    RateHost rh{eps_k_host, eps_kq_host, *prm, rate_host};
+    return async_batch(c, nq, nb2, q_host, Ukq_host, ev_host, omega_host, out_host, &rh);
 }
 
 int phoebe_elph_wait(phoebe_elph_ctx* c)

@@ -147,3 +147,40 @@ def test_rates_si_like_full(env):
     assert np.all(ref > 0)
     assert _relerr(rate.cpu().numpy(), ref) <= TOL
     ctx.close()
+
+
+def test_rates_async_pipelined_host_batches(env):
+    """q_batch_rates_host_async: several k-points in flight over the two staging slots, one rate array per call, mixed
+    with q_batch_host_async; rates (and |g|^2 where asked for) against the oracle after wait()."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=5, nb1=4, nb2=5, nm=6, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nk=3, nq=210, cfg_id=97)
+    gW_np, Re, Rp, ks = wl.gW_full(w), wl.Re_vectors(w), wl.Rp_vectors(w), wl.k_points(w)
+    ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=210, nk_max=3)
+    Uks = np.stack([wl.U_k(w, ik) for ik in range(3)])
+    P = dict(wl.RATE_PARAMS)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    ins, eps, refs, rref = [], [], [], []
+    for ik in range(3):
+        a = _case(wl, w, ik)
+        ins.append([pin(a[n]) for n in ("q", "Ukq", "ev", "om")])
+        eps.append([pin(a["eps_k"]), pin(a["eps_kq"])])
+        out = oracle.elph(gW_np, Re, Rp, None, None, ks[ik], Uks[ik], a["q"], a["Ukq"], a["ev"], a["om"])
+        refs.append(out)
+        rref.append(oracle.rates(out, a["eps_k"], a["eps_kq"], a["om"], P["kT"], P["mu"], P["sigma"], P["pref"]))
+    rates = torch.zeros((3, 4), dtype=torch.float64).pin_memory()
+    outs = [torch.empty((210, 4, 5, 6), dtype=torch.float64).pin_memory() for _ in range(3)]
+    plain = torch.empty((210, 4, 5, 6), dtype=torch.float64).pin_memory()
+    for rep in range(2):
+        rates.zero_()
+        ctx.set_k_batch_host(ks, Uks)
+        for ik in (0, 1, 2):
+            ctx.select_k(ik)
+            ctx.q_batch_rates_host_async(*[t.numpy() for t in ins[ik]], eps[ik][0].numpy(), eps[ik][1].numpy(),
+                                         rates[ik].numpy(), out=outs[ik].numpy() if ik == 1 else None, **P)
+            if ik == 1:
+                ctx.q_batch_host_async(*[t.numpy() for t in ins[ik]], plain.numpy())
+        ctx.wait()
+        for ik in range(3):
+            assert _relerr(rates[ik].numpy(), rref[ik]) <= TOL
+        assert _relerr(outs[1].numpy(), refs[1]) <= TOL and _relerr(plain.numpy(), refs[1]) <= TOL
+    ctx.close()
