@@ -139,7 +139,8 @@ int phoebe_elph_select_k(phoebe_elph_ctx* ctx, int32_t i);
  *   [nq][nmodes][nmodes] (row kappa = 3*atom+cartesian, column nu = mode; used unconjugated, any
  *   1/sqrt(mass) folded in by the caller); omega_dev DEVICE [nq][nmodes];
  *   out_dev DEVICE double [nq][nb1][nb2][nmodes], written, caller-owned.
- *   1 <= nq <= nq_max, 1 <= nb2 <= nb2_max (uniform within the batch).
+ *   0 <= nq <= nq_max, 1 <= nb2 <= nb2_max (uniform within the batch).  nq = 0 (an empty batch) is a no-op in
+ *   every q_batch* entry point: returns OK, no pointer is read, nothing is written, `rate` is left as it is.
  * Errors: E_NULL, E_DIMS, E_ALIGN, E_NO_K, E_CUDA. */
 int phoebe_elph_q_batch(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
                         const double* q_dev, const void* Ukq_dev, const void* ev_dev,

@@ -15,6 +15,7 @@
 #include "probe_kernels.cuh"
 #include "contract_planar.cuh"
 #include "qbatch_kernels.cuh"
+#include "rotate_v2.cuh"
 #include "setk_kernels.cuh"
 
 namespace {
@@ -156,6 +157,7 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
+    bool rot_v1 = false;      // tuning "rot_v1": a5-a7 through k_rotate_epilogue_mma (first tensor-core form) instead of _v2
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -169,6 +171,7 @@ struct phoebe_elph_ctx {
     double phase_sign = 1.0;
     bool conj_Uk = false, conj_Ukq = true, conj_ev = false;
     double *g1P = nullptr, *PtP = nullptr;   // planar blocked operands of k_contract_planar
+    bool planar_attr = false; // k_contract_planar's shared-memory opt-in done on this context's device
     bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
     bool g1P_stale = true;    // canonical g1' changed (set_k, or handed out by g1_buffer) since the last pack
     int k_sel = 0;            // k slot chosen by select_k (its U_k is needed for the overlap of Eq. 15)
@@ -360,6 +363,31 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     return PHOEBE_ELPH_OK;
 }
 
+// k_rotate_epilogue_v2<KS, MTW, RATES>: KS = ceil(nm/4) in 1..12, MTW = m-tiles of b2 per warp item
+template <int KS>
+const void* rot2_pick(int mtw, bool rates)
+{
+    if (mtw == 2) return rates ? (const void*)pe::k_rotate_epilogue_v2<KS, 2, true> : (const void*)pe::k_rotate_epilogue_v2<KS, 2, false>;
+    return rates ? (const void*)pe::k_rotate_epilogue_v2<KS, 1, true> : (const void*)pe::k_rotate_epilogue_v2<KS, 1, false>;
+}
+const void* rot2_kernel(int KS, int mtw, bool rates)
+{
+    switch (KS) {
+        case 1: return rot2_pick<1>(mtw, rates);
+        case 2: return rot2_pick<2>(mtw, rates);
+        case 3: return rot2_pick<3>(mtw, rates);
+        case 4: return rot2_pick<4>(mtw, rates);
+        case 5: return rot2_pick<5>(mtw, rates);
+        case 6: return rot2_pick<6>(mtw, rates);
+        case 7: return rot2_pick<7>(mtw, rates);
+        case 8: return rot2_pick<8>(mtw, rates);
+        case 9: return rot2_pick<9>(mtw, rates);
+        case 10: return rot2_pick<10>(mtw, rates);
+        case 11: return rot2_pick<11>(mtw, rates);
+        default: return rot2_pick<12>(mtw, rates);
+    }
+}
+
 struct RateReq {           // f2: linewidth accumulation fused into the epilogue (nullptr = plain q_batch)
     const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate;
 };
@@ -376,8 +404,33 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     const bool use_mma = NT <= 6 && !c->rot_plain;
     int gb1, rot_threads;
     size_t rot_smem;
-    int QG = 1;
-    if (use_mma) {
+    int QG = 1, rot_mtw = 1;
+    const bool use_v2 = use_mma && !c->rot_v1;
+    const bool fused_rates = rr != nullptr && use_mma;
+    const bool polar = c->nG > 0;
+    if (use_v2) {
+        // k_rotate_epilogue_v2: same CTA shape as v1 (QG q-points, b1 groups of gb1 double-buffered), its own layout
+        const int KS = ceil_div(d.nmodes, 4), G = (KS == 1 || KS == 3) ? 2 : 1;
+        const size_t whole_q = pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, nb1, false, false).total - 16;
+        if (whole_q <= (64u << 10)) {
+            gb1 = nb1;
+            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (64u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
+        } else {
+            gb1 = 0;
+            for (int cand = nb1 - 1; cand >= 1; --cand)           // largest group that leaves room for 2 CTAs per SM
+                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, cand, false, false).total <= (100u << 10)) { gb1 = cand; break; }
+            if (gb1 == 0) {
+                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, 1, fused_rates, polar).total > (227u << 10))
+                    return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+                gb1 = 1;
+            }
+            if (G == 2 && gb1 > 1) gb1 &= ~1;
+        }
+        // two m-tiles of b2 per warp item (a B fragment of a5 then feeds both) unless that leaves warps without an item
+        rot_mtw = (nb2 > 8 && QG * ceil_div(gb1, G) * ceil_div(ceil_div(nb2, 8), 2) >= 4) ? 2 : 1;
+        rot_smem = pe::rot2_layout(QG, d.nw, d.nmodes, nb1, nb2, gb1, fused_rates, polar).total;
+        rot_threads = 128;
+    } else if (use_mma) {
         const int nwp = (d.nw + 3) & ~3, MT = ceil_div(nb2, 8);
         const size_t slack = (size_t)(4 * d.nmodes + 8) * 16;
         const size_t fixed_q = (size_t)8 * NT * 8 + ((size_t)nwp * (MT * 8 + 2) + (size_t)8 * NT * (NT * 8 + 1)) * 16;
@@ -407,11 +460,9 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const int work = gb1 * nb2 * d.nmodes;
         rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
     }
-    const bool fused_rates = rr != nullptr && use_mma;
-    if (fused_rates)       // omega, n, eps_kq, f' per q of the CTA + one row of sums per warp (follows Cs)
+    if (fused_rates && !use_v2)       // omega, n, eps_kq, f' per q of the CTA + one row of sums per warp (follows Cs)
         rot_smem += ((size_t)QG * (2 * 8 * NT + 2 * 8 * ceil_div(nb2, 8)) + ((4 * (size_t)nb1 + 1) & ~(size_t)1)) * 8;
-    const bool polar = c->nG > 0;
-    if (polar && use_mma)  // P of the CTA's q-points and their overlaps O[b1][b2] (follow the rate arrays)
+    if (polar && use_mma && !use_v2)  // P of the CTA's q-points and their overlaps O[b1][b2] (follow the rate arrays)
         rot_smem += ((size_t)QG * 8 * NT + (size_t)QG * nb1 * 8 * ceil_div(nb2, 8)) * 16;
     if (rot_smem > (227u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
     double2* Pbuf = reinterpret_cast<double2*>(c->ws + c->L.off_P);
@@ -420,6 +471,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         out = reinterpret_cast<double*>(c->ws + c->L.off_sout);
     auto rot_kernel = [&]() -> const void* {
         if (!use_mma) return (const void*)pe::k_rotate_epilogue;
+        if (use_v2) return rot2_kernel(ceil_div(d.nmodes, 4), rot_mtw, fused_rates);
         switch (NT * 2 + (fused_rates ? 1 : 0)) {
             case 2: return (const void*)pe::k_rotate_epilogue_mma<1, false>;
             case 3: return (const void*)pe::k_rotate_epilogue_mma<1, true>;
@@ -478,11 +530,10 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
             }
             if (use_planar) {
-                static bool attr_set = false;
-                if (!attr_set) {
+                if (!c->planar_attr) {
                     PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_planar, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)pe::PlanarCfg::kSmemBytes));
-                    attr_set = true;
+                    c->planar_attr = true;
                 }
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs);
@@ -692,13 +743,13 @@ int phoebe_elph_q_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const doubl
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !out_dev) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch: nb2 out of range");
     if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch: complex input not 16-byte aligned");
     if ((reinterpret_cast<uintptr_t>(q_dev) | reinterpret_cast<uintptr_t>(omega_dev) | reinterpret_cast<uintptr_t>(out_dev)) & 7u)
         return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch: double array not 8-byte aligned");
-    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
     return run_q_batch(c, nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
                        omega_dev, out_dev);
 }
@@ -710,7 +761,8 @@ int phoebe_elph_q_batch_multi(phoebe_elph_ctx* c, int32_t nk, int32_t nq, int32_
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_multi before set_k_batch");
     if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !out_dev) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_multi: null pointer");
     if (nk <= 0 || nk > c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nk exceeds the k slots of the last set_k_batch");
-    if (nq <= 0 || (nq % 64) != 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nq must be a positive multiple of 64");
+    if (nq < 0 || (nq % 64) != 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nq must be a multiple of 64");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // empty q lists: no-op
     if ((long long)nk * nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nk*nq exceeds nq_max");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: nb2 out of range");
     if (c->nG > 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_multi: not available while the polar term is on");
@@ -724,8 +776,9 @@ int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const 
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host: nb2 out of range");
     if (int rc0 = drain_async(c)) return rc0;
     const phoebe_elph_dims& d = c->dims;
@@ -822,8 +875,9 @@ int phoebe_elph_q_batch_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, 
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_host_async before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_host_async: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_host_async: nb2 out of range");
     return async_batch(c, nq, nb2, q_host, Ukq_host, ev_host, omega_host, out_host, nullptr);
 }
@@ -835,9 +889,10 @@ int phoebe_elph_q_batch_rates_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates_host_async before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_host || !Ukq_host || !ev_host || !omega_host || !eps_k_host || !eps_kq_host || !prm || !rate_host)
         return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_host_async: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: nb2 out of range");
     if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: kT and sigma must be > 0");
     RateHost rh{eps_k_host, eps_kq_host, *prm, rate_host};
@@ -863,9 +918,10 @@ int phoebe_elph_q_batch_rates(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !eps_k_dev || !eps_kq_dev || !prm || !rate_dev)
         return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: nb2 out of range");
     if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates: kT and sigma must be > 0");
     if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch_rates: complex input not 16-byte aligned");
@@ -884,9 +940,10 @@ int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, 
 {
     if (!c) return PHOEBE_ELPH_E_NULL;
     if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates_host before set_k");
+    if (nq == 0) return PHOEBE_ELPH_OK;          // an empty batch is a no-op (nothing is read or written)
     if (!q_host || !Ukq_host || !ev_host || !omega_host || !eps_k_host || !eps_kq_host || !prm || !rate_host)
         return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_host: null pointer");
-    if (nq <= 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: nq out of range");
+    if (nq < 0 || nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: nq out of range");
     if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: nb2 out of range");
     if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host: kT and sigma must be > 0");
     if (int rc0 = drain_async(c)) return rc0;
@@ -1026,6 +1083,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "m3")) { c->m3 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "planar")) { c->planar = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "rot_v1")) { c->rot_v1 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "s_split")) {
         if (value < 0 || value > c->L.S_alloc) return fail(c, PHOEBE_ELPH_E_DIMS, "s_split out of range");
         c->s_split = (int)value;

@@ -101,7 +101,7 @@ def test_ragged_small_cases(env, case, host):
 
 
 @pytest.mark.parametrize("knob", [{"tile": 32, "m3": 0}, {"tile": 64, "m3": 0}, {"tile": 32, "m3": 1},
-                                  {"tile": 64, "m3": 1}, {"tile": 64, "m3": 1, "planar": 0}, {"rot_plain": 1}],
+                                  {"tile": 64, "m3": 1}, {"tile": 64, "m3": 1, "planar": 0}, {"rot_plain": 1}, {"rot_v1": 1}],
                          ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
 def test_forced_kernel_variants(env, knob):
     """Every kernel variant the dispatcher can pick is parity-checked on the same input."""
@@ -253,6 +253,34 @@ def test_periodicity_on_gpu(env):
     ctx.set_k(a["k"] + np.array([-1.0, 2.0, 1.0]), Uk_d)
     shifted_k = ctx.q_batch(q_d, Ukq_d, ev_d, om_d).cpu().numpy()
     assert _relerr(shifted_k, base) < 1e-11
+    ctx.close()
+
+
+def test_empty_batch_is_a_noop(env):
+    """nq = 0 in every q_batch* entry point: OK, nothing launched, nothing written, `rate` untouched; the next
+    non-empty batch is unaffected."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=3, nb1=2, nb2=3, nm=3, grid_e=(3, 2, 1), grid_p=(2, 2, 2), nq=70, cfg_id=86)
+    a = _inputs(wl, w)
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=70)
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    before = dict(ctx.launch_counts())
+    z = lambda *s, dt=torch.float64: torch.zeros(s, dtype=dt, device="cuda")
+    c128 = torch.complex128
+    out = ctx.q_batch(z(0, 3), z(0, 3, 3, dt=c128), z(0, 3, 3, dt=c128), z(0, 3))
+    assert out.shape == (0, 2, 3, 3)
+    rate = torch.full((2,), 7.0, dtype=torch.float64, device="cuda")
+    ctx.q_batch_rates(z(0, 3), z(0, 3, 3, dt=c128), z(0, 3, 3, dt=c128), z(0, 3), z(2), z(0, 3), rate,
+                      kT=0.02, mu=0.0, sigma=0.01, pref=1.0)
+    e = lambda *s, dt=np.float64: np.zeros(s, dtype=dt)
+    ctx.q_batch_host(e(0, 3), e(0, 3, 3, dt=np.complex128), e(0, 3, 3, dt=np.complex128), e(0, 3), e(0, 2, 3, 3))
+    ctx.q_batch_host_async(e(0, 3), e(0, 3, 3, dt=np.complex128), e(0, 3, 3, dt=np.complex128), e(0, 3), e(0, 2, 3, 3))
+    ctx.wait()
+    assert dict(ctx.launch_counts()) == before
+    assert rate.cpu().tolist() == [7.0, 7.0]
+    got = ctx.q_batch(*harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])).cpu().numpy()
+    ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+    assert _relerr(got, ref) <= TOL
     ctx.close()
 
 
