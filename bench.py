@@ -248,6 +248,9 @@ def run_ours(args):
     ctx.set_tuning("m3", args.m3)
     if args.tile:
         ctx.set_tuning("tile", args.tile)
+    for kv in args.tune:                      # kernel-variant experiments: --tune rot_qg=4 (see include/phoebe_elph.h, set_tuning)
+        key, val = kv.split("=")
+        ctx.set_tuning(key, int(val))
     out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
     # k-points grouped into batches of kb: one pass over g_W per batch (set_k_batch)
     groups = [list(range(i, min(i + kb, len(host_inputs)))) for i in range(0, len(host_inputs), kb)]
@@ -507,6 +510,8 @@ def main():
     ap.add_argument("--no-rates", action="store_true", help="skip the extra fused-linewidth (f2) measurement")
     ap.add_argument("--m3", type=int, default=1, help="1 = three-multiply complex product in the GEMMs (default), 0 = four")
     ap.add_argument("--tile", type=int, default=0, help="force the contraction CTA tile (0 = automatic)")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="phoebe_elph_set_tuning knob for kernel-variant experiments (repeatable)")
     ap.add_argument("--k-batch", type=int, default=16,
                     help="k-points per pass over g_W (phoebe_elph_set_k_batch); 1 = one set_k per k")
     args = ap.parse_args()

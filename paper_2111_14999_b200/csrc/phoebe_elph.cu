@@ -157,6 +157,7 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
+    int rot_qg = 0, rot_gb1 = 0, rot_mtw = 0;   // tuning "rot_qg" / "rot_gb1" / "rot_mtw": override the v2 rotation geometry (0 = automatic)
     bool rot_v1 = false;      // tuning "rot_v1": a5-a7 through k_rotate_epilogue_mma (first tensor-core form) instead of _v2
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
@@ -413,12 +414,15 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const int KS = ceil_div(d.nmodes, 4), G = (KS == 1 || KS == 3) ? 2 : 1;
         const size_t whole_q = pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, nb1, false, false).total - 16;
         if (whole_q <= (64u << 10)) {
+            // several q per CTA only up to ~24 KB of shared memory: the kernel is latency-bound for small cells (prologue
+            // loads, one TMA wait per CTA) and 8 resident CTAs per SM hide more of it than a longer CTA does
+            // (measured, band-window: QG 1/2/4/8/16 -> 3.55/2.72/2.50/3.39/5.41 ms; si-like QG 1/2/4/8 -> 27/25/29/39 us)
             gb1 = nb1;
-            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (64u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
+            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (24u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
         } else {
             gb1 = 0;
             for (int cand = nb1 - 1; cand >= 1; --cand)           // largest group that leaves room for 2 CTAs per SM
-                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, cand, false, false).total <= (100u << 10)) { gb1 = cand; break; }
+                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, cand, fused_rates, polar).total <= (112u << 10)) { gb1 = cand; break; }
             if (gb1 == 0) {
                 if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, 1, fused_rates, polar).total > (227u << 10))
                     return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
@@ -426,8 +430,11 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             }
             if (G == 2 && gb1 > 1) gb1 &= ~1;
         }
+        if (c->rot_gb1 > 0) { gb1 = std::min(c->rot_gb1, nb1); if (gb1 < nb1) QG = 1; }
+        if (c->rot_qg > 0 && gb1 == nb1) QG = std::min(c->rot_qg, 16);
         // two m-tiles of b2 per warp item (a B fragment of a5 then feeds both) unless that leaves warps without an item
         rot_mtw = (nb2 > 8 && QG * ceil_div(gb1, G) * ceil_div(ceil_div(nb2, 8), 2) >= 4) ? 2 : 1;
+        if (c->rot_mtw > 0) rot_mtw = (c->rot_mtw >= 2 && nb2 > 8) ? 2 : 1;
         rot_smem = pe::rot2_layout(QG, d.nw, d.nmodes, nb1, nb2, gb1, fused_rates, polar).total;
         rot_threads = 128;
     } else if (use_mma) {
@@ -1084,6 +1091,11 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "planar")) { c->planar = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_v1")) { c->rot_v1 = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "rot_qg") || !strcmp(key, "rot_gb1") || !strcmp(key, "rot_mtw")) {
+        if (value < 0 || value > 1024) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation geometry override out of range");
+        (key[4] == 'q' ? c->rot_qg : key[4] == 'g' ? c->rot_gb1 : c->rot_mtw) = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "s_split")) {
         if (value < 0 || value > c->L.S_alloc) return fail(c, PHOEBE_ELPH_E_DIMS, "s_split out of range");
         c->s_split = (int)value;
