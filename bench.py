@@ -335,8 +335,13 @@ def run_ours(args):
         # multi-k a1: g_W read once per launch, nk_b x the flops; bound = whichever floor is higher
         "setk_gemm": ("alu", gemm_flop) if gemm_alu else ("hbm", counts["setk_stream_bytes"]),
         "contract": ("alu", counts["contract_flop"] * n_k / max(1, kernels.get("contract", {}).get("launches_per_step", 1))),
-        "rotate_epilogue": ("alu", counts["rotate_flop"] * n_k / max(1, kernels.get("rotate_epilogue", {}).get("launches_per_step", 1))),
     }
+    # a5-a7: HBM-bound for small cells, FP64-bound for 4-atom / large: report against the higher floor.
+    # Its flops are the ALGORITHMIC four-multiply count of SURVEY 8(d) (the kernel executes fewer: three-multiply product)
+    rot_launches = max(1, kernels.get("rotate_epilogue", {}).get("launches_per_step", 1))
+    rot_flop, rot_bytes = counts["rotate_flop"] * n_k / rot_launches, counts["rotate_bytes"] * n_k / rot_launches
+    rot_alu = rot_flop / (FP64_PEAK_TFLOPS * 1e12) > rot_bytes / (hbm_peak * 1e9)
+    per_launch["rotate_epilogue"] = ("alu", rot_flop) if rot_alu else ("hbm", rot_bytes)
     for kind, (bound, work) in per_launch.items():
         if kind in kernels:
             dur = kernels[kind]["avg_ms"] * 1e-3

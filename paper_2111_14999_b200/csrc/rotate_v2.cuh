@@ -59,8 +59,12 @@ __host__ __device__ inline Rot2Layout rot2_layout(int QG, int nw, int nm, int nb
     return L;
 }
 
+// Second launch-bound argument (resident CTAs the register allocation must leave room for): 2 for the mid-size
+// accumulator sets -- the large cell's two-m-tile variant gains from it (31.5 -> 29.7 ms); 0 (= unspecified) elsewhere:
+// any tighter bound changes ptxas' schedule of the small-cell variants for the worse (band-window 2.50 -> 2.71 ms even at
+// the same occupancy) and the 4-atom variant sits at 166 registers = 3 CTAs on its own.
 template <int KS, int MTW, bool RATES>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, (KS >= 5 && KS <= 8) ? 2 : 0)
 k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
                      const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra, PolarArgs pa)
@@ -102,7 +106,9 @@ k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2
                      C + (size_t)(q0 + ql) * ldc + (size_t)b10 * Y, bytes, fb);
     };
     if (threadIdx.x == 0) issue(0);
-    // while the first panels are in flight: conj(Ukq) -> Us, ev -> Zs / Zsum, 1/(2 omega), zero padding / slack
+    // while the first panels are in flight: conj(Ukq) -> Us, ev -> Zs / Zsum, 1/(2 omega), zero padding / slack.
+    // These two loops come FIRST: their dependent global-load rounds are the longest latency chain of the CTA
+    // (4-atom: 4.15 ms with this order, 4.67 ms with the small fills ahead of them -- measured).
     for (int i = threadIdx.x; i < nql * nwp * ldu; i += blockDim.x) {
         const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
         const int w2 = r / ldu, b2 = r - w2 * ldu;
