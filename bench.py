@@ -517,7 +517,7 @@ def main():
     ap.add_argument("--tile", type=int, default=0, help="force the contraction CTA tile (0 = automatic)")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="phoebe_elph_set_tuning knob for kernel-variant experiments (repeatable)")
-    ap.add_argument("--k-batch", type=int, default=16,
+    ap.add_argument("--k-batch", type=int, default=32,
                     help="k-points per pass over g_W (phoebe_elph_set_k_batch); 1 = one set_k per k")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -283,7 +283,11 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *   "tile"      contraction CTA tile: 0 = automatic (cost model), 32 or 64
  *   "planar"    1 (default) = a4 through the planar-operand contraction (re / im / re+im planes blocked by 64
  *               columns, one LDS.128 feeds two DMMA tiles, no operand-sum DADDs); 0 = the interleaved-complex kernel
- *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)           */
+ *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
+ *   "rot_v1"    1 = a5-a7 through the first tensor-core form (padded 8-wide kappa tiles, four-multiply product)
+ *               instead of the default second form (packed (b1,kappa) columns, three-multiply product)
+ *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the second form's geometry: q-points per CTA, b1 per TMA group,
+ *               8-row tiles of b2 per warp item (0 = automatic; measurement aids)                  */
 int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
 int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);
 
