@@ -419,7 +419,17 @@ def run_ours(args):
         eps_d = [harness.to_device([e1, e2], dev) for e1, e2 in eps_np]
         rate_d = torch.zeros((len(dev_inputs), w.nb1), dtype=torch.float64, device=dev)
 
+        if multi:       # stacked form: eps / rate arrays of a k batch side by side
+            eps_k_s = [torch.stack([eps_d[i][0] for i in g]).contiguous() for g in groups]
+            eps_kq_s = [torch.stack([eps_d[i][1] for i in g]).contiguous() for g in groups]
+            rate_s = [torch.zeros((len(g), w.nb1), dtype=torch.float64, device=dev) for g in groups]
+
         def step_rates():
+            if multi:
+                for ig, (ks, Uk_d, (q_s, Ukq_s, ev_s, om_s)) in enumerate(zip(ks_np, Uks_d, stacks)):
+                    ctx.set_k_batch(ks, Uk_d)
+                    ctx.q_batch_rates_multi(q_s, Ukq_s, ev_s, om_s, eps_k_s[ig], eps_kq_s[ig], rate_s[ig], **P)
+                return
             for g, ks, Uk_d in zip(groups, ks_np, Uks_d):
                 if kb == 1:
                     ctx.set_k(ks[0], Uk_d[0])
@@ -463,8 +473,8 @@ def run_ours(args):
         e1.record()
         barrier()
         ms_re = maxreduce(max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3))
-        rates = {"what": "same pass with phoebe_elph_q_batch_rates: Eq. 29 linewidth sum fused into the |g|^2 epilogue, "
-                         "|g|^2 not stored; the result per k-point is nb1 doubles",
+        rates = {"what": "same pass with phoebe_elph_q_batch_rates%s: Eq. 29 linewidth sum fused into the |g|^2 epilogue, "
+                         "|g|^2 not stored; the result per k-point is nb1 doubles" % ("_multi (k batch stacked)" if multi else ""),
                  "value": pairs_per_step_all * args.steps / (ms_r * 1e-3), "unit": UNIT,
                  "e2e": {"value": pairs_per_step_all * e2e_steps / (ms_re * 1e-3), "unit": UNIT,
                          "h2d_bytes_per_step": int(h2d + sum(a.numel() * 8 for e in eps_pin for a in e)),

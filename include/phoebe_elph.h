@@ -201,6 +201,20 @@ int phoebe_elph_q_batch_rates(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,
                               const double* eps_k_dev, const double* eps_kq_dev, const phoebe_elph_rate_params* prm,
                               double* rate_dev, double* out_dev);
 
+/* q_batch_rates for the first nk k slots of the last set_k_batch in ONE pass (the stacked form of q_batch_multi: one
+ * phase, one contraction, one rotation + linewidth launch): the use the paper describes -- scattering rates of the bands
+ * in a window around the chemical potential (L526-540, Eq. 29) for many k-points, where one k-point's q list is too small
+ * a GEMM for 148 SMs.  Arrays stacked, k slowest: q_dev [nk][nq][3], Ukq_dev [nk][nq][nw][nb2], ev_dev [nk][nq][nmodes][nmodes],
+ * omega_dev [nk][nq][nmodes], eps_k_dev [nk][nb1], eps_kq_dev [nk][nq][nb2], rate_dev [nk][nb1] (ACCUMULATED INTO),
+ * out_dev [nk][nq][nb1][nb2][nmodes] or NULL.  Results equal nk select_k + q_batch_rates calls up to the rounding order of
+ * the sum (fixed, reproducible).  nq a multiple of 64, nk*nq <= dims.nq_max and small enough for one contraction launch
+ * (E_DIMS otherwise), nmodes <= 48, polar term off.
+ * Errors: E_NULL, E_NO_K, E_DIMS, E_ALIGN, E_CUDA. */
+int phoebe_elph_q_batch_rates_multi(phoebe_elph_ctx* ctx, int32_t nk, int32_t nq, int32_t nb2,
+                                    const double* q_dev, const void* Ukq_dev, const void* ev_dev, const double* omega_dev,
+                                    const double* eps_k_dev, const double* eps_kq_dev, const phoebe_elph_rate_params* prm,
+                                    double* rate_dev, double* out_dev);
+
 /* Same with HOST buffers (rate_host [nb1] is read, accumulated into and written back; out_host may be
  * NULL, and then only nb1 doubles come back); SYNCHRONISES the stream before returning. */
 int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,

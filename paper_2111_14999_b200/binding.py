@@ -22,6 +22,7 @@ EXPORTS = [
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_multi", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host", "phoebe_elph_q_batch_rates_host_async",
+    "phoebe_elph_q_batch_rates_multi",
     "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_set_conventions", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
@@ -75,6 +76,7 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_q_batch_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_wait.argtypes = [c_void_p]
     lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
+    lib.phoebe_elph_q_batch_rates_multi.argtypes = [c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_copy_g1.argtypes = [c_void_p, c_void_p, c_size_t]
@@ -296,6 +298,27 @@ class ElphContext:
             self._ctx, nq, nb2, q.data_ptr(), Ukq.data_ptr(), ev.data_ptr(), omega.data_ptr(), eps_k.data_ptr(),
             eps_kq.data_ptr(), byref(prm), rate.data_ptr(), None if out is None else out.data_ptr()),
             "phoebe_elph_q_batch_rates")
+        return rate, out
+
+    def q_batch_rates_multi(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None, store_out=False):
+        """q_batch_rates for the first nk k slots of the last set_k_batch in one pass.  CUDA tensors stacked over k:
+        q [nk][nq][3], Ukq [nk][nq][nw][nb2], ev [nk][nq][nm][nm], omega [nk][nq][nm], eps_k [nk][nb1], eps_kq [nk][nq][nb2],
+        rate [nk][nb1] (ACCUMULATED INTO).  Returns (rate, out-or-None)."""
+        torch = self._torch
+        nk, nq, nw, nb2 = Ukq.shape
+        nm = self.dims.nmodes
+        for t in (q, Ukq, ev, omega, eps_k, eps_kq, rate):
+            assert t.is_cuda and t.is_contiguous()
+        assert q.shape == (nk, nq, 3) and ev.shape == (nk, nq, nm, nm) and omega.shape == (nk, nq, nm)
+        assert eps_k.shape == (nk, self.nb1) and eps_kq.shape == (nk, nq, nb2) and rate.shape == (nk, self.nb1)
+        assert eps_k.dtype == eps_kq.dtype == rate.dtype == torch.float64
+        if out is None and store_out:
+            out = torch.empty((nk, nq, self.nb1, nb2, nm), dtype=torch.float64, device=self.device)
+        prm = RateParams(kT, mu, sigma, pref)
+        self._check(self._lib.phoebe_elph_q_batch_rates_multi(
+            self._ctx, nk, nq, nb2, q.data_ptr(), Ukq.data_ptr(), ev.data_ptr(), omega.data_ptr(), eps_k.data_ptr(),
+            eps_kq.data_ptr(), byref(prm), rate.data_ptr(), None if out is None else out.data_ptr()),
+            "phoebe_elph_q_batch_rates_multi")
         return rate, out
 
     def q_batch_rates_host(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):

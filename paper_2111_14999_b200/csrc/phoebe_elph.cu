@@ -432,6 +432,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
         if (c->rot_gb1 > 0) { gb1 = std::min(c->rot_gb1, nb1); if (gb1 < nb1) QG = 1; }
         if (c->rot_qg > 0 && gb1 == nb1) QG = std::min(c->rot_qg, 16);
+        if (rr && rows_per_k > 0) while (rows_per_k % QG) --QG;     // stacked linewidths: a CTA's q-points share one k slot
         // two m-tiles of b2 per warp item (a B fragment of a5 then feeds both) unless that leaves warps without an item
         rot_mtw = (nb2 > 8 && QG * ceil_div(gb1, G) * ceil_div(ceil_div(nb2, 8), 2) >= 4) ? 2 : 1;
         if (c->rot_mtw > 0) rot_mtw = (c->rot_mtw >= 2 && nb2 > 8) ? 2 : 1;
@@ -449,6 +450,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             // at least ~4 CTAs per SM in the grid
             gb1 = nb1;
             QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (64u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
+            if (rr && rows_per_k > 0) while (rows_per_k % QG) --QG;
             rot_smem = 16 + whole_q * QG;
         } else {
             if (fixed_q + 2 * (per_b1 + slack) > (200u << 10))
@@ -495,7 +497,12 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
     }();
     double* partial = reinterpret_cast<double*>(c->ws + c->L.off_part);
-    pe::RateArgs ra{nullptr, nullptr, 0.0, 0.0, 0.0, partial};
+    pe::RateArgs ra{nullptr, nullptr, 0.0, 0.0, 0.0, partial, 0};
+    if (rr && rows_per_k > 0) {
+        if (!use_mma) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: not available for nmodes > 48");
+        if (nq > nq_sub) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: the stacked batch must fit one contraction launch (fewer k slots)");
+        ra.rows_per_k = rows_per_k;
+    }
     if (rr) {
         ra.eps_k = rr->eps_k;
         ra.inv_kT = 1.0 / rr->prm.kT;
@@ -597,7 +604,10 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             }
             LaunchScope ls(c, PHOEBE_ELPH_K_RATE_REDUCE);
             const double scale = rr->prm.pref / (sqrt(3.14159265358979323846) * rr->prm.sigma);
-            pe::k_rate_reduce<<<nb1, 256, 0, c->stream>>>(partial, nparts, nb1, scale, rr->rate);
+            if (rows_per_k > 0)        // one (partial rows, rate[nb1]) block per k slot
+                pe::k_rate_reduce<<<dim3(nb1, nq / rows_per_k), 256, 0, c->stream>>>(partial, rows_per_k / QG, nb1, scale, rr->rate);
+            else
+                pe::k_rate_reduce<<<nb1, 256, 0, c->stream>>>(partial, nparts, nb1, scale, rr->rate);
             PE_CUDA(c, cudaGetLastError());
         }
     }
@@ -938,6 +948,28 @@ int phoebe_elph_q_batch_rates(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const
     RateReq rr{eps_k_dev, eps_kq_dev, *prm, rate_dev};
     return run_q_batch(c, nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
                        omega_dev, out_dev, &rr);
+}
+
+int phoebe_elph_q_batch_rates_multi(phoebe_elph_ctx* c, int32_t nk, int32_t nq, int32_t nb2, const double* q_dev,
+                                    const void* Ukq_dev, const void* ev_dev, const double* omega_dev, const double* eps_k_dev,
+                                    const double* eps_kq_dev, const phoebe_elph_rate_params* prm, double* rate_dev,
+                                    double* out_dev)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "q_batch_rates_multi before set_k_batch");
+    if (!q_dev || !Ukq_dev || !ev_dev || !omega_dev || !eps_k_dev || !eps_kq_dev || !prm || !rate_dev)
+        return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_multi: null pointer");
+    if (nk <= 0 || nk > c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: nk exceeds the k slots of the last set_k_batch");
+    if (nq < 0 || (nq % 64) != 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: nq must be a multiple of 64");
+    if (nq == 0) return PHOEBE_ELPH_OK;
+    if ((long long)nk * nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: nk*nq exceeds nq_max");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: nb2 out of range");
+    if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: kT and sigma must be > 0");
+    if (c->nG > 0) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi: not available while the polar term is on");
+    if (!aligned16(Ukq_dev) || !aligned16(ev_dev)) return fail(c, PHOEBE_ELPH_E_ALIGN, "q_batch_rates_multi: complex input not 16-byte aligned");
+    RateReq rr{eps_k_dev, eps_kq_dev, *prm, rate_dev};
+    return run_q_batch(c, nk * nq, nb2, q_dev, static_cast<const double2*>(Ukq_dev), static_cast<const double2*>(ev_dev),
+                       omega_dev, out_dev, &rr, nq);
 }
 
 int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host,

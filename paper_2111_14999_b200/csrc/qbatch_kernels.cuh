@@ -348,10 +348,11 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
 // (|g|^2 is not stored).  The extra shared arrays (omega, n, eps_kq, f', per-warp sums) follow Cs.
 // ---------------------------------------------------------------------------
 struct RateArgs {
-    const double* eps_k;    // [nb1]
+    const double* eps_k;    // [nb1]; stacked form: [k slots][nb1], the slot of a CTA = (first q row of the CTA) / rows_per_k
     const double* eps_kq;   // [nq][nb2] (of this launch)
     double inv_kT, mu, inv_sigma2;
     double* partial;        // [gridDim.x][nb1]
+    int rows_per_k;         // > 0: the q lists of several k slots are stacked (host contract: a CTA never straddles two slots)
 };
 
 // f4 (Eq. 14-15): when pa.P != nullptr the long-range amplitude P[q][nu] * O[q][b1][b2],
@@ -505,7 +506,7 @@ k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double
             const double* iw = inv2w + ql * 8 * NT;
             double racc = 0.0, x12 = 0.0, f2 = 0.0;
             if (RATES) {
-                x12 = ra.eps_k[b10 + b1] - e2_s[ql * 8 * MT + b2];
+                x12 = ra.eps_k[(ra.rows_per_k > 0 ? (q0 / ra.rows_per_k) * nb1 : 0) + b10 + b1] - e2_s[ql * 8 * MT + b2];
                 f2 = f2_s[ql * 8 * MT + b2];
             }
 #pragma unroll 1
@@ -591,8 +592,11 @@ k_rates_from_out(const double* __restrict__ outv /* [nq][nb1][nb2][nm] */, const
 __global__ void __launch_bounds__(256)
 k_rate_reduce(const double* __restrict__ partial, int nparts, int nb1, double scale, double* __restrict__ rate)
 {
+    // blockIdx.y = k slot of the stacked form (its own nparts rows of partial and its own rate[nb1]); 0 otherwise
     __shared__ double sh[256];
     const int b1 = blockIdx.x;
+    partial += (size_t)blockIdx.y * nparts * nb1;
+    rate += (size_t)blockIdx.y * nb1;
     double s = 0.0;
     for (int j = threadIdx.x; j < nparts; j += 256) s += partial[(size_t)j * nb1 + b1];
     sh[threadIdx.x] = s;

@@ -311,7 +311,7 @@ k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2
                         double* orow = out + (((size_t)(q0 + ql) * nb1 + b1) * nb2 + b2) * nm;
                         double x12 = 0.0, f2 = 0.0;
                         if (RATES) {
-                            x12 = ra.eps_k[b1] - e2_s[ql * 8 * MT + b2];
+                            x12 = ra.eps_k[(ra.rows_per_k > 0 ? (q0 / ra.rows_per_k) * nb1 : 0) + b1] - e2_s[ql * 8 * MT + b2];
                             f2 = f2_s[ql * 8 * MT + b2];
                         }
 #pragma unroll

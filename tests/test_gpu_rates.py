@@ -184,3 +184,43 @@ def test_rates_async_pipelined_host_batches(env):
             assert _relerr(rates[ik].numpy(), rref[ik]) <= TOL
         assert _relerr(outs[1].numpy(), refs[1]) <= TOL and _relerr(plain.numpy(), refs[1]) <= TOL
     ctx.close()
+
+
+@pytest.mark.parametrize("shape", [(8, 4, 4, 6, 192, {}), (12, 5, 12, 12, 128, {}), (5, 3, 4, 21, 64, {"rot_v1": 1}),
+                                   (8, 4, 4, 6, 192, {"rot_qg": 3})],
+                         ids=["band_window_shape", "two_m_tiles", "first_form", "qg_not_dividing"])
+def test_rates_multi_equals_oracle_per_k(env, shape):
+    """phoebe_elph_q_batch_rates_multi: the q lists of all k slots of a set_k_batch stacked into one pass; every k slot's
+    linewidths (and |g|^2 when stored) against the oracle, and against per-k q_batch_rates calls."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    nw, nb1, nb2, nm, nq, knobs = shape
+    nk = 3
+    w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=(2, 2, 1), grid_p=(2, 1, 2), nk=nk, nq=nq, cfg_id=97)
+    P = dict(wl.RATE_PARAMS)
+    cases = [_case(wl, w, ik) for ik in range(nk)]
+    gW_np = cases[0]["gW"]
+    ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=nk * nq, nk_max=nk)
+    for key, val in knobs.items():
+        ctx.set_tuning(key, val)
+    ks = wl.k_points(w)
+    Uks = np.stack([c["Uk"] for c in cases])
+    ctx.set_k_batch(ks, harness.to_device([Uks])[0])
+    st = lambda key: np.ascontiguousarray(np.stack([c[key] for c in cases]))
+    d = harness.to_device([st("q"), st("Ukq"), st("ev"), st("om"), st("eps_k"), st("eps_kq")])
+    rate0 = np.linspace(0.1, 0.2, nk * nb1).reshape(nk, nb1) * 1e-3
+    (rate_d,) = harness.to_device([rate0])
+    rate, out = ctx.q_batch_rates_multi(*d, rate_d, store_out=True, **P)
+    rate, out = rate.cpu().numpy(), out.cpu().numpy()
+    # rates only (|g|^2 never stored) gives the same sums bit for bit
+    (rate2_d,) = harness.to_device([rate0])
+    ctx.q_batch_rates_multi(*d, rate2_d, **P)
+    assert np.array_equal(rate2_d.cpu().numpy(), rate)
+    for ik, c in enumerate(cases):
+        ref, out_ref = _oracle_rates(oracle, c, P)
+        assert _relerr(rate[ik] - rate0[ik], ref) <= TOL
+        assert _relerr(out[ik], out_ref) <= TOL
+        ctx.select_k(ik)
+        dk = harness.to_device([c["q"], c["Ukq"], c["ev"], c["om"], c["eps_k"], c["eps_kq"], np.zeros(nb1)])
+        rk, _ = ctx.q_batch_rates(*dk, **P)
+        assert _relerr(rk.cpu().numpy(), ref) <= TOL
+    ctx.close()
