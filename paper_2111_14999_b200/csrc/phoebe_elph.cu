@@ -9,11 +9,14 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <array>
+#include <map>
 #include <string>
 #include <vector>
 
 #include "probe_kernels.cuh"
 #include "contract_planar.cuh"
+#include "contract_pair.cuh"
 #include "qbatch_kernels.cuh"
 #include "rotate_v2.cuh"
 #include "setk_kernels.cuh"
@@ -55,7 +58,7 @@ struct Layout {
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t g1P_stride = 0;  // doubles between the planar blocked copies of g1' (k_contract_planar) of consecutive k slots
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
-           off_g1 = 0, off_g1P = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
@@ -98,6 +101,8 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     // planar blocked copies ([rows][tiles of 64][3][64] doubles) of g1' and of the phases for k_contract_planar
     L.g1P_stride = (size_t)d.nRp * ceil_div((int)N, 64) * 192;
     L.off_g1P = take((size_t)L.nk_slots * L.g1P_stride * 8);
+    // +R / -R pair map of the Rp list for k_contract_pair: 3 int + 4 double per real row, at most 2 nRp rows
+    L.off_pair = take((size_t)2 * d.nRp * (3 * 4 + 4 * 8));
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_PtP = take((size_t)L.Kpad * L.ldq * 24);
     L.off_C = take((size_t)L.nq_sub * N * 16);
@@ -174,6 +179,13 @@ struct phoebe_elph_ctx {
     double *g1P = nullptr, *PtP = nullptr;   // planar blocked operands of k_contract_planar
     bool planar_attr = false; // k_contract_planar's shared-memory opt-in done on this context's device
     bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
+    // k_contract_pair: the Rp list folded into Kr real rows (pair_Kr == 0: not usable); g1P then holds the pair form
+    int pair_Kr = 0, pair_KrPad = 0;
+    int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
+    bool pair_attr = false;
+    int g1P_form = 0;         // what g1P holds: 0 nothing, 1 planar (re, im, re+im), 2 pair rows (re, im)
+    int *pair_pa = nullptr, *pair_pb = nullptr, *pair_kind = nullptr;
+    double *pair_R = nullptr, *pair_w = nullptr;
     bool g1P_stale = true;    // canonical g1' changed (set_k, or handed out by g1_buffer) since the last pack
     int k_sel = 0;            // k slot chosen by select_k (its U_k is needed for the overlap of Eq. 15)
     bool prof = false;
@@ -522,19 +534,36 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
         if (rows_per_k > 0 && tile != 32 && tile != 64) tile = 64;       // the stacked form knows these two tiles
         const bool use_planar = c->m3 && c->planar && tile == 64;
-        if (use_planar && c->g1P_stale) {      // canonical g1' of every filled k slot -> planar blocked copy
+        // +R / -R pairs folded (contract_pair.cuh): real phases x complex pair rows, 4 real flop per MAC instead of 6
+        const bool use_pair = use_planar && c->pair_Kr > 0 &&
+                              (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * d.nRp));
+        if (use_planar && (c->g1P_stale || c->g1P_form != (use_pair ? 2 : 1))) {
+            // canonical g1' of every filled k slot -> blocked operand copy (planar planes, or pair rows)
             LaunchScope ls(c, PHOEBE_ELPH_K_PACK);
-            dim3 grid(ceil_div(N, 64), d.nRp, c->nk_have);
-            pe::k_pack_planar<<<grid, 64, 0, c->stream>>>(c->g1_base, (long long)N, (long long)c->L.g1_stride, N, c->g1P,
-                                                          (long long)c->L.g1P_stride);
+            if (use_pair) {
+                dim3 grid(ceil_div(N, 64), c->pair_Kr, c->nk_have);
+                pe::k_pack_pair<<<grid, 64, 0, c->stream>>>(c->g1_base, (long long)N, (long long)c->L.g1_stride, N, c->pair_pa,
+                                                            c->pair_pb, c->pair_kind, c->g1P, (long long)c->L.g1P_stride);
+            } else {
+                dim3 grid(ceil_div(N, 64), d.nRp, c->nk_have);
+                pe::k_pack_planar<<<grid, 64, 0, c->stream>>>(c->g1_base, (long long)N, (long long)c->L.g1_stride, N, c->g1P,
+                                                              (long long)c->L.g1P_stride);
+            }
             PE_CUDA(c, cudaGetLastError());
             c->g1P_stale = false;
+            c->g1P_form = use_pair ? 2 : 1;
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
-            dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
-            pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
-                                                      c->L.ldq, c->Pt, c->phase_sign, use_planar ? c->PtP : nullptr);
+            if (use_pair) {
+                dim3 grid(ceil_div(ncols, 256), std::min(c->pair_KrPad, 64));
+                pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_kind, nqs,
+                                                               c->pair_Kr, c->pair_KrPad, c->L.ldq, c->phase_sign, c->PtP);
+            } else {
+                dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
+                pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
+                                                          c->L.ldq, c->Pt, c->phase_sign, use_planar ? c->PtP : nullptr);
+            }
             PE_CUDA(c, cudaGetLastError());
         }
         {
@@ -543,7 +572,22 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             if (rows_per_k > 0) {
                 g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
             }
-            if (use_planar) {
+            if (use_pair) {
+                if (!c->pair_attr) {
+                    PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_pair, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)pe::PairCfg::kSmemBytes));
+                    c->pair_attr = true;
+                }
+                const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
+                const int grid = std::min(ntiles, kSMs);
+                const int slot = rows_per_k > 0 ? 0 : c->k_sel;
+                int panelW = grid;      // as for the planar form: the panel of pair rows (width x Kr x 1024 B) stays in L2
+                while (panelW % 2 == 0 && (size_t)panelW * c->pair_Kr * pe::PairCfg::ROWB * 8 > (48u << 20)) panelW /= 2;
+                pe::k_contract_pair<<<grid, pe::PairCfg::kThreads, pe::PairCfg::kSmemBytes, c->stream>>>(
+                    c->PtP, c->L.ldq, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64), (long long)c->L.g1P_stride,
+                    c->C, (long long)N, nqs, N, c->pair_Kr, c->pair_KrPad, rows_per_k, qs, panelW);
+                PE_CUDA(c, cudaGetLastError());
+            } else if (use_planar) {
                 if (!c->planar_attr) {
                     PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_planar, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)pe::PlanarCfg::kSmemBytes));
@@ -701,6 +745,56 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     up(c->Rp, Rp_host, (size_t)dims->nRp * 24);
     up(c->deg_e, deg_e_host ? deg_e_host : ones.data(), (size_t)dims->nRe * 8);
     up(c->deg_p, deg_p_host ? deg_p_host : ones.data(), (size_t)dims->nRp * 8);
+    // ---- +R / -R pair map of the Rp list (contract_pair.cuh): groups of two real rows (cos | sin) for a pair or a
+    // vector without partner, then one row (cos) per self-inverse vector (R = 0) ----
+    std::vector<int> h_pa, h_pb, h_kind;
+    std::vector<double> h_R, h_w;
+    {
+        const int nRp = dims->nRp;
+        auto key = [&](int p, double sg) {
+            return std::array<double, 3>{sg * Rp_host[3 * p] + 0.0, sg * Rp_host[3 * p + 1] + 0.0, sg * Rp_host[3 * p + 2] + 0.0};
+        };
+        auto wt = [&](int p) { return deg_p_host ? deg_p_host[p] : 1.0; };
+        std::map<std::array<double, 3>, int> first;
+        for (int p = nRp - 1; p >= 0; --p) first[key(p, 1.0)] = p;
+        std::vector<char> used((size_t)nRp, 0);
+        std::vector<int> selfs;
+        auto row = [&](int a, int b, int kind) {
+            h_pa.push_back(a); h_pb.push_back(b); h_kind.push_back(kind);
+            h_R.push_back(Rp_host[3 * a]); h_R.push_back(Rp_host[3 * a + 1]); h_R.push_back(Rp_host[3 * a + 2]);
+            h_w.push_back(1.0 / wt(a));
+        };
+        for (int p = 0; p < nRp; ++p) {
+            if (used[p]) continue;
+            used[p] = 1;
+            if (key(p, 1.0) == key(p, -1.0)) { selfs.push_back(p); continue; }
+            int partner = -1;
+            auto it = first.find(key(p, -1.0));
+            if (it != first.end() && !used[it->second] && wt(it->second) == wt(p)) { partner = it->second; used[partner] = 1; }
+            row(p, partner, 0);
+            row(p, partner, 1);
+        }
+        for (int p : selfs) row(p, -1, 0);
+        c->pair_Kr = (int)h_pa.size();
+        c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, kKPad);
+        // the pair form reuses the planar buffers: rows must fit them (g1P: Kr*128 <= nRp*192 doubles per tile column,
+        // PtP: KrPad*8 <= Kpad*24 bytes per q)
+        if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
+        if (c->pair_Kr > 0) {
+            char* base = c->ws + L.off_pair;
+            const size_t cap = (size_t)2 * nRp;
+            c->pair_pa = reinterpret_cast<int*>(base);
+            c->pair_pb = c->pair_pa + cap;
+            c->pair_kind = c->pair_pb + cap;
+            c->pair_R = reinterpret_cast<double*>(base + align_up(3 * cap * 4, 8));
+            c->pair_w = c->pair_R + 3 * cap;
+            up(c->pair_pa, h_pa.data(), h_pa.size() * 4);
+            up(c->pair_pb, h_pb.data(), h_pb.size() * 4);
+            up(c->pair_kind, h_kind.data(), h_kind.size() * 4);
+            up(c->pair_R, h_R.data(), h_R.size() * 8);
+            up(c->pair_w, h_w.data(), h_w.size() * 8);
+        }
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { delete c; return PHOEBE_ELPH_E_CUDA; }
     *ctx_out = c;
@@ -1121,6 +1215,11 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "m3")) { c->m3 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "planar")) { c->planar = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "pair")) {
+        if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "pair must be 0, 1 or 2");
+        c->pair = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_v1")) { c->rot_v1 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_qg") || !strcmp(key, "rot_gb1") || !strcmp(key, "rot_mtw")) {
@@ -1141,6 +1240,13 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
     if (!c || !key || !value) return PHOEBE_ELPH_E_NULL;
     if (!strcmp(key, "nq_sub")) { *value = c->nq_sub; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "m3")) { *value = c->m3 ? 1 : 0; return PHOEBE_ELPH_OK; }
+    // real rows of the +R / -R pair form when the default (64 x 64) contraction would use it with the current knobs, else 0
+    if (!strcmp(key, "pair_rows")) {
+        const bool on = c->m3 && c->planar && (c->tile == 0 || c->tile == 64) && c->pair_Kr > 0 &&
+                        (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * c->dims.nRp));
+        *value = on ? c->pair_Kr : 0;
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "s_split")) {
         *value = c->s_split > 0 ? c->s_split
                                 : setk_auto_split(c->dims.nRe, c->dims.nRp, c->dims.nw * c->dims.nw * c->dims.nmodes);
