@@ -317,7 +317,8 @@ def run_ours(args):
     prof = ctx.profile_read()
     ctx.profile(False)
     m3 = bool(ctx.get_tuning("m3"))
-    counts = harness.algorithmic_counts(w, m3=m3)
+    pair_rows = ctx.get_tuning("pair_rows")     # > 0: a4 runs the +R / -R pair form (4 real flop per MAC)
+    counts = harness.algorithmic_counts(w, m3=m3, pair_rows=pair_rows)
     peaks, peak_src = _measured_peaks()
     hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
     kernels = {}
@@ -358,8 +359,10 @@ def run_ours(args):
                 "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % peak_src) if dk.get("bound") == "hbm"
                 else "derived: 64 FP64 FMA/clk/SM x 148 SMs x 1.965 GHz x 2 = 37.24 TFLOP/s",
                 "share_of_step": dk["ms_total"] / sum(v["ms_total"] for v in kernels.values()),
-                "flop_per_complex_mac": counts["flop_per_complex_mac"],
-                "note": "achieved counts EXECUTED flops (6 per complex MAC with the three-multiply product, 8 without)"}
+                "flop_per_complex_mac": counts["contract_flop_per_mac"] if dominant == "contract" else counts["flop_per_complex_mac"],
+                "note": "achieved counts EXECUTED flops: 4 per complex MAC in a4's +R/-R pair form (real phases x complex "
+                        "pair rows), 6 with the three-multiply product, 8 with the plain one; the algorithmic count of "
+                        "SURVEY 8(d) is 8"}
     fp64_probe = None
     if rank == 0:
         try:

@@ -19,10 +19,20 @@
 #pragma once
 #include "ptx_helpers.cuh"
 
+// Rows per ring stage: 32 (ring = 4 x 32 x 1600 B = 200 KB, one CTA per SM).  Measured on the 4-atom cell: KC = 16 runs
+// the stacked launch in 34.55 ms (91.3 % of the FP64 peak), KC = 32 in 33.26 ms (94.8 %): with 16 instead of 24 DMMA per
+// k-step the per-chunk barrier traffic weighs more than in the planar kernel; two CTAs per SM at KC = 16: no change.
+#ifndef PHOEBE_PAIR_KC
+#define PHOEBE_PAIR_KC 32
+#endif
+#ifndef PHOEBE_PAIR_STAGES
+#define PHOEBE_PAIR_STAGES 4
+#endif
+
 namespace pe {
 
 struct PairCfg {
-    static constexpr int BM = 64, BN = 64, WARPS_M = 2, WARPS_N = 4, KC = 16, STAGES = 4;
+    static constexpr int BM = 64, BN = 64, WARPS_M = 2, WARPS_N = 4, KC = PHOEBE_PAIR_KC, STAGES = PHOEBE_PAIR_STAGES;
     static constexpr int kConsumerWarps = WARPS_M * WARPS_N;
     static constexpr int kThreads = (kConsumerWarps + 1) * 32;
     static constexpr int TM = 4, TN = 2;

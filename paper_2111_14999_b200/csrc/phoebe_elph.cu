@@ -183,6 +183,8 @@ struct phoebe_elph_ctx {
     int pair_Kr = 0, pair_KrPad = 0;
     int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
     bool pair_attr = false;
+    int pair_ctas = 1;        // tuning "pair_ctas": persistent CTAs of k_contract_pair per SM (its ring is 100 KB: two fit)
+    int last_pair = -1;       // did the last contraction launch use the pair form (-1: no launch yet)
     int g1P_form = 0;         // what g1P holds: 0 nothing, 1 planar (re, im, re+im), 2 pair rows (re, im)
     int *pair_pa = nullptr, *pair_pb = nullptr, *pair_kind = nullptr;
     double *pair_R = nullptr, *pair_w = nullptr;
@@ -529,7 +531,11 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const int ncols = (int)align_up((size_t)nqs, kQPad);
         // contraction tile: 64x64 unless that leaves the 148 SMs with a long ragged tail (few tiles);
         // cost model = rounds of tiles per SM x tile area (+5 % for the smaller tile's extra operand traffic)
-        const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64;
+        // (the 64 x 64 tile is the one with the +R / -R pair form: 4 instead of 6 real flop per MAC)
+        const bool pair_ok = c->m3 && c->planar && c->pair_Kr > 0 &&
+                             (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * d.nRp));
+        const double cost64 = (double)ceil_div(ceil_div(nqs, 64) * ceil_div(N, 64), kSMs) * 64 * 64 *
+                              (pair_ok ? 4.0 * c->pair_Kr / (6.0 * d.nRp) : 1.0);
         const double cost32 = (double)ceil_div(ceil_div(nqs, 32) * ceil_div(N, 32), kSMs) * 32 * 32 * 1.05;
         int tile = c->tile > 0 ? c->tile : (cost32 < cost64 ? 32 : 64);
         if (rows_per_k > 0 && tile != 32 && tile != 64) tile = 64;       // the stacked form knows these two tiles
@@ -537,6 +543,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         // +R / -R pairs folded (contract_pair.cuh): real phases x complex pair rows, 4 real flop per MAC instead of 6
         const bool use_pair = use_planar && c->pair_Kr > 0 &&
                               (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * d.nRp));
+        c->last_pair = use_pair ? 1 : 0;
         if (use_planar && (c->g1P_stale || c->g1P_form != (use_pair ? 2 : 1))) {
             // canonical g1' of every filled k slot -> blocked operand copy (planar planes, or pair rows)
             LaunchScope ls(c, PHOEBE_ELPH_K_PACK);
@@ -579,7 +586,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                     c->pair_attr = true;
                 }
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
-                const int grid = std::min(ntiles, kSMs);
+                const int grid = std::min(ntiles, kSMs * c->pair_ctas);
                 const int slot = rows_per_k > 0 ? 0 : c->k_sel;
                 int panelW = grid;      // as for the planar form: the panel of pair rows (width x Kr x 1024 B) stays in L2
                 while (panelW % 2 == 0 && (size_t)panelW * c->pair_Kr * pe::PairCfg::ROWB * 8 > (48u << 20)) panelW /= 2;
@@ -776,7 +783,7 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
         }
         for (int p : selfs) row(p, -1, 0);
         c->pair_Kr = (int)h_pa.size();
-        c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, kKPad);
+        c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, (size_t)std::max(kKPad, pe::PairCfg::KC));
         // the pair form reuses the planar buffers: rows must fit them (g1P: Kr*128 <= nRp*192 doubles per tile column,
         // PtP: KrPad*8 <= Kpad*24 bytes per q)
         if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
@@ -1215,9 +1222,15 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "m3")) { c->m3 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "planar")) { c->planar = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "pair_ctas")) {
+        if (value < 1 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "pair_ctas must be 1 or 2");
+        c->pair_ctas = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "pair")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "pair must be 0, 1 or 2");
         c->pair = (int)value;
+        c->last_pair = -1;
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
@@ -1240,11 +1253,12 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
     if (!c || !key || !value) return PHOEBE_ELPH_E_NULL;
     if (!strcmp(key, "nq_sub")) { *value = c->nq_sub; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "m3")) { *value = c->m3 ? 1 : 0; return PHOEBE_ELPH_OK; }
-    // real rows of the +R / -R pair form when the default (64 x 64) contraction would use it with the current knobs, else 0
+    // real rows of the +R / -R pair form if the LAST contraction launch used it, else 0 (before any launch: whether the
+    // 64 x 64 tile would use it with the current knobs)
     if (!strcmp(key, "pair_rows")) {
         const bool on = c->m3 && c->planar && (c->tile == 0 || c->tile == 64) && c->pair_Kr > 0 &&
                         (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * c->dims.nRp));
-        *value = on ? c->pair_Kr : 0;
+        *value = (c->last_pair < 0 ? on : c->last_pair == 1) ? c->pair_Kr : 0;
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "s_split")) {

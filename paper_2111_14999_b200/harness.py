@@ -71,7 +71,7 @@ def to_device(arrs, device="cuda:0"):
     return [torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in arrs]
 
 
-def algorithmic_counts(w: wl.Workload, nq: int | None = None, m3: bool = False):
+def algorithmic_counts(w: wl.Workload, nq: int | None = None, m3: bool = False, pair_rows: int = 0):
     """Flop / byte counts of SURVEY 8(d), per k-point and per q-batch of nq.  The two GEMMs count the flops they
     EXECUTE: 8 real flop per complex MAC with the four-multiply product, 6 with the three-multiply product (m3;
     its few extra additions -- 2 per operand element loaded, 3 per output -- are not counted)."""
@@ -86,7 +86,9 @@ def algorithmic_counts(w: wl.Workload, nq: int | None = None, m3: bool = False):
         "setk_stream_flop": 8 * w.nRp * w.nRe * X,
         "setk_gemm_flop": fpc * w.nRp * w.nRe * X,
         # a4: 8 flop per complex MAC
-        "contract_flop": fpc * nq * w.nRp * N,
+        # pair_rows > 0: the +R / -R pair form (contract_pair.cuh) -- real phases x complex rows, 4 flop per (q, row, n)
+        "contract_flop": 4 * nq * pair_rows * N if pair_rows else fpc * nq * w.nRp * N,
+        "contract_flop_per_mac": 4 if pair_rows else fpc,
         "contract_flop_4m": 8 * nq * w.nRp * N,
         "flop_per_complex_mac": fpc,
         # a5-a7 per batch
