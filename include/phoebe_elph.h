@@ -297,6 +297,11 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *   "tile"      contraction CTA tile: 0 = automatic (cost model), 32 or 64
  *   "planar"    1 (default) = a4 through the planar-operand contraction (re / im / re+im planes blocked by 64
  *               columns, one LDS.128 feeds two DMMA tiles, no operand-sum DADDs); 0 = the interleaved-complex kernel
+ *   "pair"      1 (default) = a4 in the +R / -R pair form (real cos / sin phase rows x complex rows g1'[p] + g1'[pbar],
+ *               i (g1'[p] - g1'[pbar]): 4 real flop per complex MAC, exact) whenever the Rp list has enough inversion
+ *               pairs (4 Kr < 6 nRp, Kr = real rows: 2 per pair or partner-less vector, 1 for R = 0); 0 = never; 2 = whenever
+ *               the rows fit the operand buffers (Kr <= 1.5 nRp).  get_tuning("pair_rows") = Kr if the last contraction
+ *               launch used the form, else 0.   "pair_ctas" 1 | 2 = persistent CTAs per SM of that kernel
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
  *   "rot_v1"    1 = a5-a7 through the first tensor-core form (padded 8-wide kappa tiles, four-multiply product)
  *               instead of the default second form (packed (b1,kappa) columns, three-multiply product)
