@@ -64,9 +64,11 @@ k_pack_pair(const double2* __restrict__ src, long long ld, long long strideS, in
 }
 
 // A rows: AtR[r][q] = w[r] * (trig[r] ? sgn * sin : cos)(2 pi q . Rrow[r]); zero for r >= Kr or q >= nq.
+// Rows come in (cos, sin) pairs of the same lattice vector for r < 2*K2 and as single cos rows behind them (host
+// contract, phoebe_elph_setup): one sincospi serves both rows of a pair.  blockIdx.y strides over row PAIRS.
 __global__ void __launch_bounds__(256)
 k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rrow /* [Kr][3] */,
-              const double* __restrict__ wrow, const int* __restrict__ trig, int nq, int Kr, int KrPad, int ldq,
+              const double* __restrict__ wrow, int K2, int nq, int Kr, int KrPad, int ldq,
               double sgn, double* __restrict__ AtR /* [KrPad][ldq] */)
 {
     const int iq = blockIdx.x * blockDim.x + threadIdx.x;
@@ -74,15 +76,19 @@ k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restri
     double q0 = 0.0, q1 = 0.0, q2 = 0.0;
     const bool valid = iq < nq;
     if (valid) { q0 = q[3 * (size_t)iq]; q1 = q[3 * (size_t)iq + 1]; q2 = q[3 * (size_t)iq + 2]; }
-    for (int r = blockIdx.y; r < KrPad; r += gridDim.y) {
-        double v = 0.0;
+    const int nslots = K2 + (KrPad - 2 * K2);            // K2 two-row slots, then one slot per remaining (single or padding) row
+    for (int sl = blockIdx.y; sl < nslots; sl += gridDim.y) {
+        const bool two = sl < K2;
+        const int r = two ? 2 * sl : sl + K2;
+        double vc = 0.0, vs = 0.0;
         if (valid && r < Kr) {
             const double x = q0 * Rrow[3 * r] + q1 * Rrow[3 * r + 1] + q2 * Rrow[3 * r + 2];
             double sn, cs;
             sincospi(2.0 * x, &sn, &cs);
-            v = wrow[r] * (trig[r] ? sgn * sn : cs);
+            vc = wrow[r] * cs; vs = wrow[r] * sgn * sn;
         }
-        AtR[(size_t)r * ldq + iq] = v;
+        AtR[(size_t)r * ldq + iq] = vc;
+        if (two) AtR[(size_t)(r + 1) * ldq + iq] = vs;
     }
 }
 

@@ -180,7 +180,7 @@ struct phoebe_elph_ctx {
     bool planar_attr = false; // k_contract_planar's shared-memory opt-in done on this context's device
     bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
     // k_contract_pair: the Rp list folded into Kr real rows (pair_Kr == 0: not usable); g1P then holds the pair form
-    int pair_Kr = 0, pair_KrPad = 0;
+    int pair_Kr = 0, pair_KrPad = 0, pair_K2 = 0;   // K2 = (cos, sin) row pairs; single cos rows (R = 0) follow them
     int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
     bool pair_attr = false;
     int pair_ctas = 1;        // tuning "pair_ctas": persistent CTAs of k_contract_pair per SM (its ring is 100 KB: two fit)
@@ -563,8 +563,8 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
             if (use_pair) {
-                dim3 grid(ceil_div(ncols, 256), std::min(c->pair_KrPad, 64));
-                pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_kind, nqs,
+                dim3 grid(ceil_div(ncols, 256), std::min(c->pair_KrPad - c->pair_K2, 64));
+                pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, nqs,
                                                                c->pair_Kr, c->pair_KrPad, c->L.ldq, c->phase_sign, c->PtP);
             } else {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
@@ -781,6 +781,7 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
             row(p, partner, 0);
             row(p, partner, 1);
         }
+        c->pair_K2 = (int)h_pa.size() / 2;
         for (int p : selfs) row(p, -1, 0);
         c->pair_Kr = (int)h_pa.size();
         c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, (size_t)std::max(kKPad, pe::PairCfg::KC));
