@@ -94,6 +94,9 @@ int phoebe_elph_workspace_bytes(const phoebe_elph_dims* dims, size_t hbm_budget_
  *   workspace_dev DEVICE, BORROWED for the life of ctx, >= phoebe_elph_workspace_bytes(), 256-B aligned.
  *   cuda_stream a cudaStream_t (NULL = default stream).
  * Synchronises the stream once (the small copies use pageable host memory).
+ *   At setup the library also pairs every Rp vector with its inverse -R (exact match, equal degeneracy): step a4 then
+ *   runs as real (cos | sin) phase rows times complex rows g1'[R] + g1'[-R], i (g1'[R] - g1'[-R]) -- see tuning "pair".
+ *   Any list is accepted; vectors without partner cost two rows instead of one.  Re / Rp must be finite (E_DIMS).
  * Errors: E_NULL, E_DIMS, E_ALIGN, E_WORKSPACE, E_CUDA. */
 int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev,
                       const double* Re_host, const double* Rp_host,

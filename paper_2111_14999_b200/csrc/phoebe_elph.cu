@@ -712,6 +712,8 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     if (!gW_dev || !Re_host || !Rp_host || !dims || !workspace_dev) return PHOEBE_ELPH_E_NULL;
     if (!dims_ok(dims, true)) return PHOEBE_ELPH_E_DIMS;
     if (!aligned16(gW_dev) || (reinterpret_cast<uintptr_t>(workspace_dev) & (kAlign - 1))) return PHOEBE_ELPH_E_ALIGN;
+    for (int i = 0; i < 3 * dims->nRe; ++i) if (!std::isfinite(Re_host[i])) return PHOEBE_ELPH_E_DIMS;
+    for (int i = 0; i < 3 * dims->nRp; ++i) if (!std::isfinite(Rp_host[i])) return PHOEBE_ELPH_E_DIMS;
     for (int i = 0; deg_e_host && i < dims->nRe; ++i) if (!(deg_e_host[i] > 0.0)) return PHOEBE_ELPH_E_DIMS;
     for (int i = 0; deg_p_host && i < dims->nRp; ++i) if (!(deg_p_host[i] > 0.0)) return PHOEBE_ELPH_E_DIMS;
     Layout L = make_layout(*dims, dims->nq_max);
