@@ -25,6 +25,10 @@
 #include "ptx_helpers.cuh"
 #include "qbatch_kernels.cuh"
 
+#ifndef PHOEBE_ROT_EB
+#define PHOEBE_ROT_EB 3
+#endif
+
 namespace pe {
 
 struct Rot2Layout {
@@ -109,24 +113,50 @@ k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2
     // while the first panels are in flight: conj(Ukq) -> Us, ev -> Zs / Zsum, 1/(2 omega), zero padding / slack.
     // These two loops come FIRST: their dependent global-load rounds are the longest latency chain of the CTA
     // (4-atom: 4.15 ms with this order, 4.67 ms with the small fills ahead of them -- measured).
-    for (int i = threadIdx.x; i < nql * nwp * ldu; i += blockDim.x) {
-        const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
-        const int w2 = r / ldu, b2 = r - w2 * ldu;
-        double2 u = make_double2(0.0, 0.0);
-        if (w2 < nw && b2 < nb2) { u = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2]; if (!(pa.conv & 1)) u.y = -u.y; }
-        Us[i] = u;
+    // Each thread first ISSUES the global loads of up to EB of its elements (of both arrays), then stores them: one
+    // exposed load latency per round instead of one per element.
+    double om_first = 0.0;                   // omega of this thread's first inv2w element rides along with the first round
+    if ((int)threadIdx.x < nql * 8 * NT) {
+        const int ql = threadIdx.x / (8 * NT), nu = threadIdx.x - ql * 8 * NT;
+        if (nu < nm) om_first = omega[(size_t)(q0 + ql) * nm + nu];
     }
-    for (int i = threadIdx.x; i < nql * 4 * KS * (8 * NT); i += blockDim.x) {
-        const int ql = i / (4 * KS * 8 * NT), r = i - ql * 4 * KS * 8 * NT;
-        const int ka = r / (8 * NT), nu = r - ka * 8 * NT;
-        double2 zv = (ka < nm && nu < nm) ? ev[((size_t)(q0 + ql) * nm + ka) * nm + nu] : make_double2(0.0, 0.0);
-        if (pa.conv & 2) zv.y = -zv.y;
-        Zs[((size_t)ql * 4 * KS + ka) * ldz + nu] = zv;
-        Zsum[((size_t)ql * 4 * KS + ka) * ldzs + nu] = zv.x + zv.y;
+    {
+        constexpr int EB = PHOEBE_ROT_EB;
+        const int totU = nql * nwp * ldu, totZ = nql * 4 * KS * (8 * NT);
+        for (int base = 0; base < max(totU, totZ); base += EB * blockDim.x) {
+            double2 u[EB], zv[EB];
+#pragma unroll
+            for (int e = 0; e < EB; ++e) {
+                const int i = base + e * blockDim.x + threadIdx.x;
+                u[e] = make_double2(0.0, 0.0); zv[e] = make_double2(0.0, 0.0);
+                if (i < totU) {
+                    const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
+                    const int w2 = r / ldu, b2 = r - w2 * ldu;
+                    if (w2 < nw && b2 < nb2) u[e] = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2];
+                }
+                if (i < totZ) {
+                    const int ql = i / (4 * KS * 8 * NT), r = i - ql * 4 * KS * 8 * NT;
+                    const int ka = r / (8 * NT), nu = r - ka * 8 * NT;
+                    if (ka < nm && nu < nm) zv[e] = ev[((size_t)(q0 + ql) * nm + ka) * nm + nu];
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < EB; ++e) {
+                const int i = base + e * blockDim.x + threadIdx.x;
+                if (i < totU) { if (!(pa.conv & 1)) u[e].y = -u[e].y; Us[i] = u[e]; }
+                if (i < totZ) {
+                    const int ql = i / (4 * KS * 8 * NT), r = i - ql * 4 * KS * 8 * NT;
+                    const int ka = r / (8 * NT), nu = r - ka * 8 * NT;
+                    if (pa.conv & 2) zv[e].y = -zv[e].y;
+                    Zs[((size_t)ql * 4 * KS + ka) * ldz + nu] = zv[e];
+                    Zsum[((size_t)ql * 4 * KS + ka) * ldzs + nu] = zv[e].x + zv[e].y;
+                }
+            }
+        }
     }
     for (int i = threadIdx.x; i < nql * 8 * NT; i += blockDim.x) {
         const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
-        const double w = (nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
+        const double w = (i == (int)threadIdx.x) ? om_first : ((nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0);
         inv2w[i] = (w > 0.0) ? 0.5 / w : 0.0;
     }
     for (int i = threadIdx.x; i < nbuf * QG * slack; i += blockDim.x) {
