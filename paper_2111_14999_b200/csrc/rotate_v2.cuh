@@ -66,9 +66,10 @@ __host__ __device__ inline Rot2Layout rot2_layout(int QG, int nw, int nm, int nb
 // Second launch-bound argument (resident CTAs the register allocation must leave room for): 2 for the mid-size
 // accumulator sets -- the large cell's two-m-tile variant gains from it (31.5 -> 29.7 ms); 0 (= unspecified) elsewhere:
 // any tighter bound changes ptxas' schedule of the small-cell variants for the worse (band-window 2.50 -> 2.71 ms even at
-// the same occupancy) and the 4-atom variant sits at 166 registers = 3 CTAs on its own.
+// the same occupancy); 3 for the 4-atom variant, which sits on that register edge (168): at 2 CTAs its launch takes 6.3 ms
+// instead of 3.8 ms.
 template <int KS, int MTW, bool RATES>
-__global__ void __launch_bounds__(128, (KS >= 5 && KS <= 8) ? 2 : 0)
+__global__ void __launch_bounds__(128, (KS >= 5 && KS <= 8) ? 2 : ((KS == 3 || KS == 4) && MTW == 2 && !RATES) ? 3 : 0)
 k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
                      const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra, PolarArgs pa)
@@ -315,6 +316,10 @@ k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2
                     }
                 }
                 const int nu = 8 * n + 2 * t;
+                // per n-tile, outside the (b1, m-tile) loops: 1/(2 omega) of this lane's two columns (the padded array is
+                // 8 NT long) and which of them exist -- the compiler does not hoist shared-memory loads over the stores
+                const double iw0 = iw[nu], iw1 = iw[nu + 1];
+                const bool okh[2] = {nu < nm, nu + 1 < nm};
 #pragma unroll
                 for (int bl = 0; bl < G; ++bl) {
                     if (b1a + bl >= nb1l) continue;
@@ -346,8 +351,8 @@ k_rotate_epilogue_v2(const double2* __restrict__ C, long long ldc, const double2
                         }
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
-                            if (nu + h >= nm) continue;
-                            const double v = (er[h] * er[h] + ei[h] * ei[h]) * iw[nu + h];
+                            if (!okh[h]) continue;
+                            const double v = (er[h] * er[h] + ei[h] * ei[h]) * (h ? iw1 : iw0);
                             if (!RATES || out != nullptr) orow[nu + h] = v;
                             if (RATES) {
                                 const double w = om_s[ql * 8 * NT + nu + h], bn_ = bose_s[ql * 8 * NT + nu + h];
