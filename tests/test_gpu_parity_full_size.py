@@ -1,5 +1,6 @@
 """GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
-(set_k_batch over the workload's k-points, three-multiply GEMMs, whole q batch per launch):
+(set_k_batch over the workload's k-points, pair-form contraction, whole q batch per launch; the 4-atom workload also
+through the stacked launch of all its k slots, phoebe_elph_q_batch_multi):
 
   * 4-atom  (configs[2]): g_W 26.1 GB resident, 16 k in one pass, 8192 q per k
   * large   (configs[4]): g_W 57.8 GB resident,  4 k in one pass, 16384 q per k
@@ -70,7 +71,7 @@ def _upload_and_oracle_setk(env, w, k_ids):
     return gW, g1_ref
 
 
-def _full_size_case(env, name, k_check, n_sample):
+def _full_size_case(env, name, k_check, n_sample, stacked=False):
     torch, oracle, wl, harness = env["torch"], env["oracle"], env["wl"], env["harness"]
     w = wl.CONFIGS[name]
     free, _ = torch.cuda.mem_get_info()
@@ -79,8 +80,11 @@ def _full_size_case(env, name, k_check, n_sample):
     gW, g1_ref = _upload_and_oracle_setk(env, w, k_check)
     Rp, ks = wl.Rp_vectors(w), wl.k_points(w)
     kb = min(16, w.nk)
-    ctx = harness.make_context(w, gW, nk_max=kb)
-    assert ctx.nq_batch == w.nq                      # the whole q list is one batch (L576 sizing)
+    # stacked: bench.py runs the q lists of all kb k slots through ONE phase / contraction / rotation launch
+    # (phoebe_elph_q_batch_multi) when the stacked C fits 8 GB -- the 4-atom workload
+    ctx = harness.make_context(w, gW, nk_max=kb, nq_max=kb * w.nq if stacked else None)
+    assert ctx.nq_batch == (kb * w.nq if stacked else w.nq)      # the whole q list is one batch (L576 sizing)
+    refs, bases = {}, {}
     Uks = np.stack([wl.U_k(w, ik) for ik in range(kb)])
     ctx.set_k_batch(ks[:kb], harness.to_device([Uks])[0])
     out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device="cuda")
@@ -111,10 +115,25 @@ def _full_size_case(env, name, k_check, n_sample):
         ctx.q_batch(q2_d, Ukq_d, ev_d, om_d, out)
         out.sub_(base)
         shift_err = float(out.abs().max().item())
+        if stacked:
+            refs[ik], bases[ik] = (ref, scale), base
         del base
         assert shift_err <= 1e-10 * scale, (shift_err, scale)
+    if stacked:
+        # the launch configuration of bench.py: all kb q lists stacked, one launch of each kernel
+        ins = [wl.q_inputs(w, ik) for ik in range(kb)]
+        st = [torch.from_numpy(np.ascontiguousarray(np.stack([ins[ik][j] for ik in range(kb)]))).cuda() for j in range(4)]
+        del ins
+        outm = ctx.q_batch_multi(*st)
+        assert outm.shape == (kb, w.nq, w.nb1, w.nb2, w.nm)
+        for ik in k_check:
+            ref, scale = refs[ik]
+            got = outm[ik][torch.from_numpy(idx).cuda()].cpu().numpy()
+            worst_out = max(worst_out, float(np.max(np.abs(got - ref))) / max(scale, float(ref.max())))
+            assert bool(torch.equal(outm[ik], bases[ik])), "stacked form differs from the per-k call"
+        del outm, st, bases
     n = ctx.launch_counts()
-    assert n["setk_gemm"] == 1 and n["contract"] == 3 * len(k_check)      # one launch per q batch
+    assert n["setk_gemm"] == 1 and n["contract"] == 3 * len(k_check) + (1 if stacked else 0)   # one launch per q batch
     ctx.close()
     del gW, out
     torch.cuda.empty_cache()
@@ -123,8 +142,9 @@ def _full_size_case(env, name, k_check, n_sample):
 
 
 def test_4atom_full_size_sampled(env):
-    """BASELINE.json configs[2]: 16 k in one pass over the 26.1 GB g_W; k-points 0 and 15, 96 sampled q of 8192."""
-    _full_size_case(env, "4-atom", k_check=(0, 15), n_sample=96)
+    """BASELINE.json configs[2]: 16 k in one pass over the 26.1 GB g_W; k-points 0 and 15, 96 sampled q of 8192 -- per k
+    and through the stacked launch of all 16 x 8192 q that bench.py times."""
+    _full_size_case(env, "4-atom", k_check=(0, 15), n_sample=96, stacked=True)
 
 
 def test_large_full_size_sampled(env):
