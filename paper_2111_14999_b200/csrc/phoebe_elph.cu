@@ -355,7 +355,9 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
         cudaError_t e;
         if (c->m3) {
             if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, true>(c->stream, g, false);
-            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 4, true>(c->stream, g, false);
+            // 6 ring stages: the deepest ring that still leaves two CTAs per SM (2 x 114 KB); measured on the 4-atom cell
+            // 4 / 5 / 6 / 8 stages -> 5.06 / 5.03 / 4.93 / 6.79 ms
+            else if (nk <= 16) e = launch_contract<16, 128, 1, 4, 8, 6, true>(c->stream, g, false);
             else e = launch_contract<32, 128, 1, 8, 8, 4, true>(c->stream, g, false);
         } else {
             if (nk <= 8) e = launch_contract<8, 128, 1, 4, 8, 4, false>(c->stream, g, false);
