@@ -187,7 +187,7 @@ def test_rates_async_pipelined_host_batches(env):
 
 
 @pytest.mark.parametrize("shape", [(8, 4, 4, 6, 192, {}), (12, 5, 12, 12, 128, {}), (5, 3, 4, 21, 64, {"rot_v1": 1}),
-                                   (8, 4, 4, 6, 192, {"rot_qg": 3})],
+                                   (8, 4, 4, 6, 192, {"rot_qg": 5})],
                          ids=["band_window_shape", "two_m_tiles", "first_form", "qg_not_dividing"])
 def test_rates_multi_equals_oracle_per_k(env, shape):
     """phoebe_elph_q_batch_rates_multi: the q lists of all k slots of a set_k_batch stacked into one pass; every k slot's
