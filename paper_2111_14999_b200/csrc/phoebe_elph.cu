@@ -246,7 +246,11 @@ cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persist
 {
     using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
     auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST, M3, MINB>;
-    static int ctas_per_sm = 0;          // per instantiation; set once
+    // per instantiation AND per device: the shared-memory opt-in is a per-device function attribute
+    static int ctas_by_dev[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
+    int& ctas_per_sm = ctas_by_dev[dev];
     if (ctas_per_sm == 0) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
         if (e != cudaSuccess) return e;
