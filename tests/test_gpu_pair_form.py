@@ -99,3 +99,67 @@ def test_pair_form_opposite_phase_sign_and_stacked(env):
         assert _relerr(res[(sign, 1)], res[(sign, 0)]) <= 1e-12
     assert _relerr(res[(1, 1)], res[(-1, 1)]) > 1e-3          # the conventions really differ
     ctx.close()
+
+
+def _run_custom_lists(env, gW, Re, Rp, deg_p, k, Uk, q, Ukq, ev, om, pair):
+    """The C ABI over explicit lattice-vector lists (not a grid of workloads.py) -> (out, real rows of the pair form)."""
+    torch, binding, harness = env["torch"], env["binding"], env["harness"]
+    ctx = binding.ElphContext(torch.from_numpy(gW).cuda(), Re, Rp, None, deg_p, nb1_max=Uk.shape[1],
+                              nb2_max=Ukq.shape[2], nq_max=len(q))
+    ctx.set_tuning("tile", 64)
+    ctx.set_tuning("pair", pair)
+    rows = ctx.get_tuning("pair_rows")
+    ctx.set_k(k, harness.to_device([Uk])[0])
+    out = ctx.q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
+    ctx.close()
+    return out, rows
+
+
+def _custom_inputs(wl, nRe, nRp, seed, nw=4, nb1=3, nb2=4, nm=6, nq=200):
+    rng = np.random.default_rng(seed)
+    w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=(nRe, 1, 1), grid_p=(nRp, 1, 1), nq=nq, cfg_id=142)
+    gW = (rng.standard_normal((nRp, nRe, nw, nw, nm)) + 1j * rng.standard_normal((nRp, nRe, nw, nw, nm)))
+    return w, rng, gW, wl.k_points(w)[0], wl.U_k(w), wl.q_points(w), wl.U_kq(w), wl.ph_eigvecs(w), wl.omega(w)
+
+
+@pytest.mark.parametrize("kind", ["generic", "symmetric"])
+@pytest.mark.parametrize("pair", [0, 1, 2])
+def test_non_integer_lattice_vectors(env, kind, pair):
+    """Reading R12: Re / Rp are doubles and need not be integers (only Eq. 87's periodicity needs that).  generic: no
+    vector has an inversion partner (the pair map degenerates to two rows per vector); symmetric: non-integer vectors
+    that do come in exact +R / -R pairs, plus the origin."""
+    wl, oracle = env["wl"], env["oracle"]
+    nRe, nRp = 5, 11
+    w, rng, gW, k, Uk, q, Ukq, ev, om = _custom_inputs(wl, nRe, nRp, 7)
+    Re = rng.uniform(-2.5, 2.5, (nRe, 3))
+    if kind == "generic":
+        Rp = rng.uniform(-3.0, 3.0, (nRp, 3))
+    else:
+        half = rng.uniform(-3.0, 3.0, (nRp // 2, 3))
+        Rp = np.concatenate([half, np.zeros((1, 3)), -half[::-1]])
+        Rp = Rp[rng.permutation(nRp)]
+    ref = oracle.elph(gW, Re, Rp, None, None, k, Uk, q, Ukq, ev, om)
+    out, rows = _run_custom_lists(env, gW, Re, Rp, None, k, Uk, q, Ukq, ev, om, pair)
+    if kind == "symmetric" and pair:
+        assert rows == nRp
+    assert _relerr(out, ref) <= TOL
+
+
+@pytest.mark.parametrize("pair", [0, 1, 2])
+def test_duplicated_lattice_vectors(env, pair):
+    """An Rp list that names the same vector more than once (each entry with its own slab of g_W and its own
+    degeneracy): the sum of Eq. 13 runs over list ENTRIES, so duplicates simply add.  Pair-map edge cases: a vector
+    with two copies and one partner, a duplicated origin, a duplicated partner."""
+    wl, oracle = env["wl"], env["oracle"]
+    Rp = np.array([[1, 0, 0], [-1, 0, 0], [1, 0, 0], [0, 0, 0], [0, 0, 0], [0, 2, -1], [0, -2, 1], [0, -2, 1],
+                   [2, 1, 0], [1, 0, 0]], dtype=np.float64)
+    nRp, nRe = len(Rp), 3
+    w, rng, gW, k, Uk, q, Ukq, ev, om = _custom_inputs(wl, nRe, nRp, 11)
+    Re = wl.Re_vectors(w)
+    deg_p = np.array([1, 1, 1, 2, 2, 1, 1, 3, 1, 2], dtype=np.float64)
+    ref = oracle.elph(gW, Re, Rp, None, deg_p, k, Uk, q, Ukq, ev, om)
+    out, rows = _run_custom_lists(env, gW, Re, Rp, deg_p, k, Uk, q, Ukq, ev, om, pair)
+    assert _relerr(out, ref) <= TOL
+    # q -> q + G (Eq. 87) still holds for this integer list
+    out2, _ = _run_custom_lists(env, gW, Re, Rp, deg_p, k, Uk, q + np.array([1.0, -2.0, 3.0]), Ukq, ev, om, pair)
+    assert _relerr(out2, ref) <= TOL
