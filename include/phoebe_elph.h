@@ -292,7 +292,8 @@ int phoebe_elph_profile(phoebe_elph_ctx* ctx, int32_t enable);
 int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches);
 
 /* Tuning knobs (integers); unknown key -> E_DIMS.  Keys:
- *   "nq_sub"    q-points per contraction / rotation launch (default: the whole batch when C fits)
+ *   "nq_sub"    q-points per contraction / rotation launch (default: the whole batch when C fits); rounded down to a
+ *               multiple of 128 (at least 128), so that no contraction row tile straddles two sub-batches or k slots
  *   "s_split"   number of Re chunks in the set_k stream (0 = automatic)
  *   "m3"        1 (default) = three-multiply complex product in the two GEMMs (T1 = Ar.Br, T2 = Ai.Bi,
  *               T3 = (Ar+Ai).(Br+Bi); Re = T1-T2, Im = T3-T1-T2: 6 instead of 8 real flop per complex MAC,
@@ -306,10 +307,9 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               the rows fit the operand buffers (Kr <= 1.5 nRp).  get_tuning("pair_rows") = Kr if the last contraction
  *               launch used the form, else 0.   "pair_ctas" 1 | 2 = persistent CTAs per SM of that kernel
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
- *   "rot_v1"    1 = a5-a7 through the first tensor-core form (padded 8-wide kappa tiles, four-multiply product)
- *               instead of the default second form (packed (b1,kappa) columns, three-multiply product)
- *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the second form's geometry: q-points per CTA, b1 per TMA group,
- *               8-row tiles of b2 per warp item (0 = automatic; measurement aids)                  */
+ *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the geometry of the tensor-core rotation kernel (rotate_v3.cuh):
+ *               q-points per ring stage, b1 per C stage (forces the two-ring form), 8-row tiles of b2 per warp item
+ *               (0 = automatic; measurement aids)                  */
 int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
 int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);
 

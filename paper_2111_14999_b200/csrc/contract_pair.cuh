@@ -97,7 +97,7 @@ k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restri
 __global__ void __launch_bounds__(PairCfg::kThreads, 1)
 k_contract_pair(const double* __restrict__ AtR, int lda, const double* __restrict__ BP2, int ntnB, long long strideBslot,
                 double2* __restrict__ C, long long ldc, int M, int N, int K, int Kpad, int rowsPerB, int rowOffset,
-                int panelW)
+                int panelW, CMap cm)
 {
     using Cfg = PairCfg;
     constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = Cfg::STAGES, LDA = Cfg::LDA, LDB = Cfg::LDB;
@@ -215,16 +215,19 @@ k_contract_pair(const double* __restrict__ AtR, int lda, const double* __restric
         }
 
         // ---------------- store C: a lane owns 4 consecutive columns of each of its 4 rows ----------------
+        const int nleft = N - (n0 + wn * 16 + 4 * t);
+        long long coff[4];                                  // where the rotation kernel wants them (CMap)
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) coff[cc] = cc < nleft ? cmap_off(n0 + wn * 16 + 4 * t + cc, cm) : 0;
 #pragma unroll
         for (int i = 0; i < TM; ++i) {
             const int m = m0 + wm * 32 + 16 * (i >> 1) + 2 * g + (i & 1);
             if (m >= M) continue;
-            double2* dst = C + (size_t)m * ldc + n0 + wn * 16 + 4 * t;
-            const int nleft = N - (n0 + wn * 16 + 4 * t);
+            double2* dst = C + (size_t)m * ldc;
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
                 const int j = cc & 1, h = cc >> 1;
-                if (cc < nleft) dst[cc] = make_double2(cr[i][j][h], ci[i][j][h]);
+                if (cc < nleft) dst[coff[cc]] = make_double2(cr[i][j][h], ci[i][j][h]);
             }
         }
     }

@@ -57,7 +57,7 @@ k_pack_planar(const double2* __restrict__ src, long long ld, long long strideS, 
 __global__ void __launch_bounds__(PlanarCfg::kThreads, 1)
 k_contract_planar(const double* __restrict__ AtP, int ntmA, const double* __restrict__ BP, int ntnB,
                   long long strideBslot, double2* __restrict__ C, long long ldc, int M, int N, int K, int Kpad,
-                  int rowsPerB, int rowOffset, int panelW)
+                  int rowsPerB, int rowOffset, int panelW, CMap cm)
 {
     using Cfg = PlanarCfg;
     constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = Cfg::STAGES, LDP = Cfg::LDP, ROW = Cfg::ROW;
@@ -185,17 +185,20 @@ k_contract_planar(const double* __restrict__ AtP, int ntmA, const double* __rest
         }
 
         // ---------------- store C: a lane owns 4 consecutive columns of each of its 4 rows ----------------
+        const int nleft = N - (n0 + wn * 16 + 4 * t);
+        long long coff[4];                                  // where the rotation kernel wants them (CMap)
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) coff[cc] = cc < nleft ? cmap_off(n0 + wn * 16 + 4 * t + cc, cm) : 0;
 #pragma unroll
         for (int i = 0; i < TM; ++i) {
             const int m = m0 + wm * 32 + 16 * (i >> 1) + 2 * g + (i & 1);
             if (m >= M) continue;
-            double2* dst = C + (size_t)m * ldc + n0 + wn * 16 + 4 * t;
-            const int nleft = N - (n0 + wn * 16 + 4 * t);
+            double2* dst = C + (size_t)m * ldc;
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
                 const int j = cc & 1, h = cc >> 1;
                 const double t1 = cr[i][j][h], t2 = ci[i][j][h];
-                if (cc < nleft) dst[cc] = make_double2(t1 - t2, cs[i][j][h] - t1 - t2);
+                if (cc < nleft) dst[coff[cc]] = make_double2(t1 - t2, cs[i][j][h] - t1 - t2);
             }
         }
     }

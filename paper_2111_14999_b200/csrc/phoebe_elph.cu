@@ -11,6 +11,7 @@
 #include <cstring>
 #include <array>
 #include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -18,7 +19,7 @@
 #include "contract_planar.cuh"
 #include "contract_pair.cuh"
 #include "qbatch_kernels.cuh"
-#include "rotate_v2.cuh"
+#include "rotate_v3.cuh"
 #include "setk_kernels.cuh"
 
 namespace {
@@ -62,10 +63,15 @@ struct Layout {
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
+// complex elements of C per q-point in the layout rotate_v3.cuh reads (row pitch P >= nm, b1 block pitch PB <= nw*P + 7)
+size_t c_elems_per_q(const phoebe_elph_dims& d, int nb1)
+{
+    return (size_t)nb1 * ((size_t)d.nw * pe::rot3_row_pitch(d.nmodes) + 7);
+}
+
 int default_nq_sub(const phoebe_elph_dims& d, int nq_max)
 {
-    const size_t N = (size_t)d.nb1_max * d.nw * d.nmodes;
-    const size_t per_q = 16 * (N + (size_t)d.nRp + 4);
+    const size_t per_q = 16 * (c_elems_per_q(d, d.nb1_max) + (size_t)d.nRp + 4);
     long n = (long)(kCBytesCap / per_q);
     n = n / kQPad * kQPad;
     n = std::max<long>(n, kQPad);
@@ -105,9 +111,9 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_pair = take((size_t)2 * d.nRp * (3 * 4 + 4 * 8));
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_PtP = take((size_t)L.Kpad * L.ldq * 24);
-    L.off_C = take((size_t)L.nq_sub * N * 16);
-    // f2: per-CTA linewidth partials [<= nq_max CTAs][nb1], staging of rate / eps_k / eps_kq for the host entry point
-    L.off_part = take((size_t)nq_max * d.nb1_max * 8);
+    L.off_C = take((size_t)L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16);
+    // f2: linewidth partials [nq][groups of b2 tiles][nb1], staging of rate / eps_k / eps_kq for the host entry point
+    L.off_part = take((size_t)nq_max * ceil_div(d.nb2_max, 8) * d.nb1_max * 8);
     L.off_rate = take((size_t)2 * 2 * d.nb1_max * 8);                 // two slots of (rate, eps_k)
     L.off_seps = take((size_t)2 * nq_max * d.nb2_max * 8);            // two slots of eps_kq
     // f4: G list and Born charges of the polar term, its (q, nu) amplitudes
@@ -136,7 +142,8 @@ bool dims_ok(const phoebe_elph_dims* d, bool need_nq)
     if (d->nb1_max <= 0 || d->nb1_max > d->nw || d->nb2_max <= 0 || d->nb2_max > d->nw) return false;
     if (d->nq_max < 0 || (need_nq && d->nq_max == 0)) return false;
     if (d->nk_max < 0 || d->nk_max > kKBatchMax) return false;
-    if (d->nRp > 65535) return false;                       // grid.z / grid.y limits of the kernels
+    if (d->nRp > 32768 || d->nRe > 65535) return false;     // grid.y / grid.z limits of the kernels (pair rows <= 1.5 nRp)
+    if (d->nmodes > 48 && d->nq_max > 0 && (size_t)d->nq_max > ((size_t)1 << 30)) return false;
     if ((long)d->nw * d->nw * d->nmodes > (1L << 24)) return false;
     return true;
 }
@@ -163,7 +170,6 @@ struct phoebe_elph_ctx {
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
     int rot_qg = 0, rot_gb1 = 0, rot_mtw = 0;   // tuning "rot_qg" / "rot_gb1" / "rot_mtw": override the v2 rotation geometry (0 = automatic)
-    bool rot_v1 = false;      // tuning "rot_v1": a5-a7 through k_rotate_epilogue_mma (first tensor-core form) instead of _v2
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -177,12 +183,10 @@ struct phoebe_elph_ctx {
     double phase_sign = 1.0;
     bool conj_Uk = false, conj_Ukq = true, conj_ev = false;
     double *g1P = nullptr, *PtP = nullptr;   // planar blocked operands of k_contract_planar
-    bool planar_attr = false; // k_contract_planar's shared-memory opt-in done on this context's device
     bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
     // k_contract_pair: the Rp list folded into Kr real rows (pair_Kr == 0: not usable); g1P then holds the pair form
     int pair_Kr = 0, pair_KrPad = 0, pair_K2 = 0;   // K2 = (cos, sin) row pairs; single cos rows (R = 0) follow them
     int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
-    bool pair_attr = false;
     int pair_ctas = 1;        // tuning "pair_ctas": persistent CTAs of k_contract_pair per SM (its ring is 100 KB: two fit)
     int last_pair = -1;       // did the last contraction launch use the pair form (-1: no launch yet)
     int g1P_form = 0;         // what g1P holds: 0 nothing, 1 planar (re, im, re+im), 2 pair rows (re, im)
@@ -218,7 +222,7 @@ cudaEvent_t get_event(phoebe_elph_ctx* c)
 {
     if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
     cudaEvent_t e = nullptr;
-    cudaEventCreate(&e);
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
     return e;
 }
 struct LaunchScope {          // counts the launch and, when profiling, brackets it with events
@@ -228,36 +232,67 @@ struct LaunchScope {          // counts the launch and, when profiling, brackets
         c->launches[kind]++;
         if (c->prof) {
             cudaEvent_t a = get_event(c); b = get_event(c);
-            cudaEventRecord(a, c->stream);
-            c->evs.push_back({kind, a, b});
+            if (a && b) {
+                cudaEventRecord(a, c->stream);
+                c->evs.push_back({kind, a, b});
+            } else {                       // out of events: this launch goes untimed
+                if (a) c->ev_pool.push_back(a);
+                if (b) c->ev_pool.push_back(b);
+                b = nullptr;
+            }
         }
     }
     ~LaunchScope() { if (b) cudaEventRecord(b, c->stream); }
 };
+
+// Per-device function attributes (the shared-memory opt-in is per device, not per context): set once per
+// (device, kernel, size), behind a mutex -- contexts on several threads share the table.
+cudaError_t ensure_smem_optin(const void* kern, size_t bytes)
+{
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, size_t> done;
+    if (bytes <= (48u << 10)) return cudaSuccess;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t& have = done[{dev, kern}];
+    if (have >= bytes) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) have = bytes;
+    return e;
+}
 
 // ---- batched complex GEMM launcher (a4 and multi-k a1) ------------------------------
 struct GemmArgs {
     const double2* At; int lda; const double2* B; int ldb; long long strideB;
     double2* C; long long ldc; long long strideC; int M, N, K, Kpad, batch;
     int rowsPerB = 0, rowOffset = 0; long long strideBrow = 0;      // multi-k a4: B slab switches every rowsPerB rows
+    pe::CMap cm{0, 0, 0, 0};                                        // a4: column -> offset map of the C layout (ptx_helpers.cuh)
 };
 template <int BM, int BN, int WM, int WN, int KC, int ST, bool M3, int MINB = 1>
 cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persistent = true)
 {
     using Cfg = pe::ContractCfg<BM, BN, WM, WN, KC, ST>;
     auto kern = pe::k_contract<BM, BN, WM, WN, KC, ST, M3, MINB>;
-    // per instantiation AND per device: the shared-memory opt-in is a per-device function attribute
+    // per instantiation AND per device (the shared-memory opt-in is a per-device function attribute); contexts on
+    // several threads share the table
+    static std::mutex mu;
     static int ctas_by_dev[64] = {0};
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) dev = 0;
-    int& ctas_per_sm = ctas_by_dev[dev];
-    if (ctas_per_sm == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
-        if (e != cudaSuccess) return e;
-        int nb = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, Cfg::kThreads, Cfg::kSmemBytes);
-        if (e != cudaSuccess) return e;
-        ctas_per_sm = std::max(1, nb);
+    int ctas_per_sm;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (ctas_by_dev[dev] == 0) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes);
+            if (e != cudaSuccess) return e;
+            int nb = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, Cfg::kThreads, Cfg::kSmemBytes);
+            if (e != cudaSuccess) return e;
+            ctas_by_dev[dev] = std::max(1, nb);
+        }
+        ctas_per_sm = ctas_by_dev[dev];
     }
     // persistent grid: one CTA per resident slot, each walks the tile list with stride gridDim.x
     const long long ntiles = (long long)ceil_div(g.N, BN) * ceil_div(g.M, BM) * g.batch;
@@ -270,7 +305,7 @@ cudaError_t launch_contract(cudaStream_t stream, const GemmArgs& g, bool persist
     const int panelW = persistent ? grid : 0x7fffffff;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, stream>>>(g.At, g.lda, g.B, g.ldb, g.strideB, g.C, g.ldc, g.strideC,
                                                            g.M, g.N, g.K, g.Kpad, g.batch, g.rowsPerB, g.rowOffset,
-                                                           g.strideBrow, panelW);
+                                                           g.strideBrow, panelW, g.cm);
     return cudaGetLastError();
 }
 
@@ -319,6 +354,8 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
     S = std::min(S, c->L.S_alloc);
     const int epc = ceil_div(d.nRe, S);
     S = ceil_div(d.nRe, epc);
+    if ((size_t)epc * 16 > (size_t)(227u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "set_k: nRe too large for one Re chunk (raise s_split)");
+    PE_CUDA(c, ensure_smem_optin((const void*)pe::k_setk_stream, (size_t)epc * 16));
     {
         LaunchScope ls(c, PHOEBE_ELPH_K_SETK_STREAM);
         dim3 grid(ceil_div(X, T), S, d.nRp);
@@ -384,29 +421,93 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     return PHOEBE_ELPH_OK;
 }
 
-// k_rotate_epilogue_v2<KS, MTW, RATES>: KS = ceil(nm/4) in 1..12, MTW = m-tiles of b2 per warp item
-template <int KS>
-const void* rot2_pick(int mtw, bool rates)
+// ---- k_rotate_v3<KS, GB, MTW, RATES> (rotate_v3.cuh): KS = ceil(nm/4) in 1..12, GB = b1 per warp item, MTW = tiles of b2 ----
+// GB per KS: the smallest that fills whole a5 column tiles (2 for odd KS <= 3, else 1) or, when nb1 allows, the largest
+// whose accumulators fit (a U_kq / ev fragment then feeds GB x as many tensor instructions).
+int rot3_min_gb(int KS) { return (KS == 1 || KS == 3) ? 2 : 1; }
+int rot3_max_gb(int KS, int MTW)
 {
-    if (mtw == 2) return rates ? (const void*)pe::k_rotate_epilogue_v2<KS, 2, true> : (const void*)pe::k_rotate_epilogue_v2<KS, 2, false>;
-    return rates ? (const void*)pe::k_rotate_epilogue_v2<KS, 1, true> : (const void*)pe::k_rotate_epilogue_v2<KS, 1, false>;
+    if (MTW == 1) return KS == 1 ? 8 : KS == 2 ? 4 : (KS == 3 || KS == 4) ? 2 : 1;
+    return KS == 1 ? 4 : (KS == 2 || KS == 3) ? 2 : 1;
 }
-const void* rot2_kernel(int KS, int mtw, bool rates)
+template <int KS, int GB, int MTW>
+const void* rot3_pick(bool rates)
+{
+    return rates ? (const void*)pe::k_rotate_v3<KS, GB, MTW, true> : (const void*)pe::k_rotate_v3<KS, GB, MTW, false>;
+}
+template <int KS>
+const void* rot3_kernel_ks(int GB, int MTW, bool rates)
+{
+    constexpr int g0 = (KS == 1 || KS == 3) ? 2 : 1;
+    constexpr int g1 = KS == 1 ? 8 : KS == 2 ? 4 : (KS == 3 || KS == 4) ? 2 : 1;      // rot3_max_gb(KS, 1)
+    constexpr int g2 = KS == 1 ? 4 : (KS == 2 || KS == 3) ? 2 : 1;                    // rot3_max_gb(KS, 2)
+    if (MTW == 1) return GB == g1 ? rot3_pick<KS, g1, 1>(rates) : rot3_pick<KS, g0, 1>(rates);
+    return GB == g2 ? rot3_pick<KS, g2, 2>(rates) : rot3_pick<KS, g0, 2>(rates);
+}
+const void* rot3_kernel(int KS, int GB, int MTW, bool rates)
 {
     switch (KS) {
-        case 1: return rot2_pick<1>(mtw, rates);
-        case 2: return rot2_pick<2>(mtw, rates);
-        case 3: return rot2_pick<3>(mtw, rates);
-        case 4: return rot2_pick<4>(mtw, rates);
-        case 5: return rot2_pick<5>(mtw, rates);
-        case 6: return rot2_pick<6>(mtw, rates);
-        case 7: return rot2_pick<7>(mtw, rates);
-        case 8: return rot2_pick<8>(mtw, rates);
-        case 9: return rot2_pick<9>(mtw, rates);
-        case 10: return rot2_pick<10>(mtw, rates);
-        case 11: return rot2_pick<11>(mtw, rates);
-        default: return rot2_pick<12>(mtw, rates);
+        case 1: return rot3_kernel_ks<1>(GB, MTW, rates);
+        case 2: return rot3_kernel_ks<2>(GB, MTW, rates);
+        case 3: return rot3_kernel_ks<3>(GB, MTW, rates);
+        case 4: return rot3_kernel_ks<4>(GB, MTW, rates);
+        case 5: return rot3_kernel_ks<5>(GB, MTW, rates);
+        case 6: return rot3_kernel_ks<6>(GB, MTW, rates);
+        case 7: return rot3_kernel_ks<7>(GB, MTW, rates);
+        case 8: return rot3_kernel_ks<8>(GB, MTW, rates);
+        case 9: return rot3_kernel_ks<9>(GB, MTW, rates);
+        case 10: return rot3_kernel_ks<10>(GB, MTW, rates);
+        case 11: return rot3_kernel_ks<11>(GB, MTW, rates);
+        default: return rot3_kernel_ks<12>(GB, MTW, rates);
     }
+}
+
+// geometry of one rotation launch
+struct Rot3Geom { int KS, GB, MTW, P, PB, QS, gb1, nmg; size_t smem; };
+constexpr size_t kRot3SmemBudget = 200u << 10;
+
+bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_over, int gb1_over, int mtw_over,
+                   Rot3Geom* G)
+{
+    const int KS = ceil_div(nm, 4), NT = ceil_div(nm, 8), MT = ceil_div(nb2, 8);
+    G->KS = KS;
+    G->MTW = (mtw_over > 0) ? ((mtw_over >= 2 && MT >= 2) ? 2 : 1) : (MT >= 2 ? 2 : 1);
+    G->GB = nb1 >= rot3_max_gb(KS, G->MTW) ? rot3_max_gb(KS, G->MTW) : rot3_min_gb(KS);
+    G->nmg = ceil_div(MT, G->MTW);
+    G->P = pe::rot3_row_pitch(nm);
+    // a5 column tiles that hold pairs of two different b1 (GB >= 2, odd KS): b1 block pitch = 4 mod 8 keeps their B
+    // fragment loads conflict-free
+    const int raw = nw * G->P;
+    G->PB = raw + ((G->GB >= 2 && (KS & 1)) ? ((4 - raw % 8) + 8) % 8 : 0);
+    auto total = [&](int QS, int gb1) { return (size_t)pe::rot3_layout(nw, nm, nb2, G->PB, QS, gb1, rates).total; };
+    const int qs_cap = std::max(1, 128 / (8 * std::max(NT, MT)));      // the producer lanes' register slots
+    if (total(1, nb1) <= kRot3SmemBudget && gb1_over <= 0) {
+        // whole q-points per stage: enough of them that every consumer warp has an item, while the q list still
+        // gives every SM several stages
+        const int per_q = ceil_div(nb1, G->GB) * G->nmg;
+        int QS = ceil_div(pe::kRot3Consumers, per_q);
+        if (qs_over > 0) QS = qs_over;
+        QS = std::min(QS, qs_cap);
+        while (QS > 1 && (total(QS, nb1) > kRot3SmemBudget || ceil_div(nq, QS) < 2 * kSMs)) --QS;
+        G->QS = QS; G->gb1 = nb1;
+    } else {
+        int gb1 = 0;
+        for (int cand = nb1; cand >= 1; --cand) {
+            if (cand % G->GB) continue;
+            if (total(1, cand) <= kRot3SmemBudget) { gb1 = cand; break; }
+        }
+        if (gb1 == 0) {
+            if (total(1, 1) > (size_t)(227u << 10) - 1024) return false;
+            gb1 = 1;
+        }
+        // no larger than gives every consumer warp one item (smaller stages: deeper prefetch for the same memory)
+        const int want = std::max(G->GB, ceil_div(pe::kRot3Consumers, G->nmg) * G->GB);
+        gb1 = std::min(gb1, std::max(want, G->GB));
+        if (gb1_over > 0) gb1 = std::min(gb1_over, nb1);
+        G->QS = 1; G->gb1 = std::min(gb1, nb1);
+    }
+    G->smem = total(G->QS, G->gb1);
+    return G->smem <= (size_t)(227u << 10);
 }
 
 struct RateReq {           // f2: linewidth accumulation fused into the epilogue (nullptr = plain q_batch)
@@ -420,66 +521,18 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     const phoebe_elph_dims& d = c->dims;
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
     const int nq_sub = std::min(c->nq_sub, c->L.nq_sub);
-    // rotation kernel geometry
-    const int NT = ceil_div(d.nmodes, 8);
-    const bool use_mma = NT <= 6 && !c->rot_plain;
-    int gb1, rot_threads;
-    size_t rot_smem;
-    int QG = 1, rot_mtw = 1;
-    const bool use_v2 = use_mma && !c->rot_v1;
+    // rotation kernel geometry: rotate_v3 (FP64 tensor cores) for nm <= 48, else the plain DFMA kernel
+    const bool use_mma = d.nmodes <= 48 && !c->rot_plain;
     const bool fused_rates = rr != nullptr && use_mma;
     const bool polar = c->nG > 0;
-    if (use_v2) {
-        // k_rotate_epilogue_v2: same CTA shape as v1 (QG q-points, b1 groups of gb1 double-buffered), its own layout
-        const int KS = ceil_div(d.nmodes, 4), G = (KS == 1 || KS == 3) ? 2 : 1;
-        const size_t whole_q = pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, nb1, false, false).total - 16;
-        if (whole_q <= (64u << 10)) {
-            // several q per CTA only up to ~24 KB of shared memory: the kernel is latency-bound for small cells (prologue
-            // loads, one TMA wait per CTA) and 8 resident CTAs per SM hide more of it than a longer CTA does
-            // (measured, band-window: QG 1/2/4/8/16 -> 3.55/2.72/2.50/3.39/5.41 ms; si-like QG 1/2/4/8 -> 27/25/29/39 us)
-            gb1 = nb1;
-            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (24u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
-        } else {
-            gb1 = 0;
-            for (int cand = nb1 - 1; cand >= 1; --cand)           // largest group that leaves room for 2 CTAs per SM
-                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, cand, fused_rates, polar).total <= (112u << 10)) { gb1 = cand; break; }
-            if (gb1 == 0) {
-                if (pe::rot2_layout(1, d.nw, d.nmodes, nb1, nb2, 1, fused_rates, polar).total > (227u << 10))
-                    return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
-                gb1 = 1;
-            }
-            if (G == 2 && gb1 > 1) gb1 &= ~1;
-        }
-        if (c->rot_gb1 > 0) { gb1 = std::min(c->rot_gb1, nb1); if (gb1 < nb1) QG = 1; }
-        if (c->rot_qg > 0 && gb1 == nb1) QG = std::min(c->rot_qg, 16);
-        if (rr && rows_per_k > 0) while (rows_per_k % QG) --QG;     // stacked linewidths: a CTA's q-points share one k slot
-        // two m-tiles of b2 per warp item (a B fragment of a5 then feeds both) unless that leaves warps without an item
-        rot_mtw = (nb2 > 8 && QG * ceil_div(gb1, G) * ceil_div(ceil_div(nb2, 8), 2) >= 4) ? 2 : 1;
-        if (c->rot_mtw > 0) rot_mtw = (c->rot_mtw >= 2 && nb2 > 8) ? 2 : 1;
-        rot_smem = pe::rot2_layout(QG, d.nw, d.nmodes, nb1, nb2, gb1, fused_rates, polar).total;
-        rot_threads = 128;
-    } else if (use_mma) {
-        const int nwp = (d.nw + 3) & ~3, MT = ceil_div(nb2, 8);
-        const size_t slack = (size_t)(4 * d.nmodes + 8) * 16;
-        const size_t fixed_q = (size_t)8 * NT * 8 + ((size_t)nwp * (MT * 8 + 2) + (size_t)8 * NT * (NT * 8 + 1)) * 16;
-        const size_t per_b1 = (size_t)Y * 16;
-        const size_t whole_q = fixed_q + per_b1 * nb1 + slack;
-        const size_t budget = 100u << 10;
-        if (whole_q <= (64u << 10)) {
-            // small cell: every b1 of a q at once, several q per CTA (amortises the CTA prologue), but keep
-            // at least ~4 CTAs per SM in the grid
-            gb1 = nb1;
-            QG = (int)std::max<size_t>(1, std::min<size_t>({(size_t)8, (64u << 10) / whole_q, (size_t)nq / (4 * kSMs) + 1}));
-            if (rr && rows_per_k > 0) while (rows_per_k % QG) --QG;
-            rot_smem = 16 + whole_q * QG;
-        } else {
-            if (fixed_q + 2 * (per_b1 + slack) > (200u << 10))
-                return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
-            const size_t room = budget > fixed_q + 2 * slack ? budget - fixed_q - 2 * slack : 0;
-            gb1 = (int)std::max<size_t>(1, std::min<size_t>((size_t)nb1, room / (2 * per_b1)));
-            rot_smem = 16 + fixed_q + 2 * (per_b1 * gb1 + slack);
-        }
-        rot_threads = 128;
+    Rot3Geom G{};
+    int gb1 = nb1, rot_threads = pe::kRot3Threads;
+    size_t rot_smem = 0;
+    int P = d.nmodes, PB = d.nw * d.nmodes;                 // C layout (plain for the DFMA kernel)
+    if (use_mma) {
+        if (!rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), fused_rates, c->rot_qg, c->rot_gb1, c->rot_mtw, &G))
+            return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+        P = G.P; PB = G.PB; gb1 = G.gb1; rot_smem = G.smem;
     } else {
         const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;
         const size_t per_b1 = ((size_t)Y + (size_t)nb2 * d.nmodes) * 16;
@@ -489,33 +542,19 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const int work = gb1 * nb2 * d.nmodes;
         rot_threads = std::max(32, std::min(256, (int)align_up((size_t)work, 32)));
     }
-    if (fused_rates && !use_v2)       // omega, n, eps_kq, f' per q of the CTA + one row of sums per warp (follows Cs)
-        rot_smem += ((size_t)QG * (2 * 8 * NT + 2 * 8 * ceil_div(nb2, 8)) + ((4 * (size_t)nb1 + 1) & ~(size_t)1)) * 8;
-    if (polar && use_mma && !use_v2)  // P of the CTA's q-points and their overlaps O[b1][b2] (follow the rate arrays)
-        rot_smem += ((size_t)QG * 8 * NT + (size_t)QG * nb1 * 8 * ceil_div(nb2, 8)) * 16;
-    if (rot_smem > (227u << 10)) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+    const long long ldcq = (long long)nb1 * PB;            // complex elements of C per q-point
+    const pe::CMap cm = (P == d.nmodes && PB == d.nw * d.nmodes) ? pe::CMap{0, 0, 0, 0}
+                                                                   : pe::CMap{d.nmodes, d.nw, P, PB - d.nw * P};
     double2* Pbuf = reinterpret_cast<double2*>(c->ws + c->L.off_P);
     pe::PolarArgs pa{nullptr, c->Uk + (size_t)c->k_sel * d.nw * nb1, (c->conj_Ukq ? 0 : 1) | (c->conj_ev ? 2 : 0)};
-    if (rr && !use_mma && out == nullptr)      // the plain path sums from the stored |g|^2: keep it in the staging area
-        out = reinterpret_cast<double*>(c->ws + c->L.off_sout);
-    auto rot_kernel = [&]() -> const void* {
-        if (!use_mma) return (const void*)pe::k_rotate_epilogue;
-        if (use_v2) return rot2_kernel(ceil_div(d.nmodes, 4), rot_mtw, fused_rates);
-        switch (NT * 2 + (fused_rates ? 1 : 0)) {
-            case 2: return (const void*)pe::k_rotate_epilogue_mma<1, false>;
-            case 3: return (const void*)pe::k_rotate_epilogue_mma<1, true>;
-            case 4: return (const void*)pe::k_rotate_epilogue_mma<2, false>;
-            case 5: return (const void*)pe::k_rotate_epilogue_mma<2, true>;
-            case 6: return (const void*)pe::k_rotate_epilogue_mma<3, false>;
-            case 7: return (const void*)pe::k_rotate_epilogue_mma<3, true>;
-            case 8: return (const void*)pe::k_rotate_epilogue_mma<4, false>;
-            case 9: return (const void*)pe::k_rotate_epilogue_mma<4, true>;
-            case 10: return (const void*)pe::k_rotate_epilogue_mma<5, false>;
-            case 11: return (const void*)pe::k_rotate_epilogue_mma<5, true>;
-            case 12: return (const void*)pe::k_rotate_epilogue_mma<6, false>;
-            default: return (const void*)pe::k_rotate_epilogue_mma<6, true>;
-        }
-    }();
+    double* plain_scratch = nullptr;
+    if (rr && !use_mma && out == nullptr) {     // the plain path sums from the stored |g|^2: its own scratch behind C
+        if ((size_t)std::min(nq, nq_sub) * (size_t)ldcq * 16 + (size_t)std::min(nq, nq_sub) * nb1 * nb2 * d.nmodes * 8 >
+            (size_t)c->L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16)
+            return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates without out: not available for nmodes > 48 at this size");
+        plain_scratch = reinterpret_cast<double*>(c->C + (size_t)std::min(nq, nq_sub) * ldcq);
+    }
+    const void* rot_kernel = use_mma ? rot3_kernel(G.KS, G.GB, G.MTW, fused_rates) : (const void*)pe::k_rotate_epilogue;
     double* partial = reinterpret_cast<double*>(c->ws + c->L.off_part);
     pe::RateArgs ra{nullptr, nullptr, 0.0, 0.0, 0.0, partial, 0};
     if (rr && rows_per_k > 0) {
@@ -529,8 +568,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         ra.mu = rr->prm.mu;
         ra.inv_sigma2 = 1.0 / (rr->prm.sigma * rr->prm.sigma);
     }
-    if (rot_smem > (48u << 10))
-        PE_CUDA(c, cudaFuncSetAttribute(rot_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rot_smem));
+    PE_CUDA(c, ensure_smem_optin(rot_kernel, rot_smem));
 
     for (int qs = 0; qs < nq; qs += nq_sub) {
         const int nqs = std::min(nq_sub, nq - qs);
@@ -581,16 +619,13 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_CONTRACT);
-            GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, (long long)N, 0, nqs, N, d.nRp, c->L.Kpad, 1};
+            GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, ldcq, 0, nqs, N, d.nRp, c->L.Kpad, 1};
+            g.cm = cm;
             if (rows_per_k > 0) {
                 g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
             }
             if (use_pair) {
-                if (!c->pair_attr) {
-                    PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_pair, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                    (int)pe::PairCfg::kSmemBytes));
-                    c->pair_attr = true;
-                }
+                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs * c->pair_ctas);
                 const int slot = rows_per_k > 0 ? 0 : c->k_sel;
@@ -598,14 +633,10 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 while (panelW % 2 == 0 && (size_t)panelW * c->pair_Kr * pe::PairCfg::ROWB * 8 > (48u << 20)) panelW /= 2;
                 pe::k_contract_pair<<<grid, pe::PairCfg::kThreads, pe::PairCfg::kSmemBytes, c->stream>>>(
                     c->PtP, c->L.ldq, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64), (long long)c->L.g1P_stride,
-                    c->C, (long long)N, nqs, N, c->pair_Kr, c->pair_KrPad, rows_per_k, qs, panelW);
+                    c->C, ldcq, nqs, N, c->pair_Kr, c->pair_KrPad, rows_per_k, qs, panelW, cm);
                 PE_CUDA(c, cudaGetLastError());
             } else if (use_planar) {
-                if (!c->planar_attr) {
-                    PE_CUDA(c, cudaFuncSetAttribute(pe::k_contract_planar, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                    (int)pe::PlanarCfg::kSmemBytes));
-                    c->planar_attr = true;
-                }
+                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_planar, pe::PlanarCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs);
                 const int slot = rows_per_k > 0 ? 0 : c->k_sel;
@@ -615,11 +646,10 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 while (panelW % 2 == 0 && (size_t)panelW * d.nRp * pe::PlanarCfg::ROW * 8 > (48u << 20)) panelW /= 2;
                 pe::k_contract_planar<<<grid, pe::PlanarCfg::kThreads, pe::PlanarCfg::kSmemBytes, c->stream>>>(
                     c->PtP, c->L.ldq / 64, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64),
-                    (long long)c->L.g1P_stride, c->C, (long long)N, nqs, N, d.nRp, c->L.Kpad, rows_per_k, qs, panelW);
+                    (long long)c->L.g1P_stride, c->C, ldcq, nqs, N, d.nRp, c->L.Kpad, rows_per_k, qs, panelW, cm);
                 PE_CUDA(c, cudaGetLastError());
             } else if (c->m3) {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, true>(c->stream, g)));
-                else if (tile == 6432) PE_CUDA(c, (launch_contract<64, 32, 2, 2, 16, 3, true, 2>(c->stream, g)));
                 else PE_CUDA(c, (launch_contract<64, 64, 2, 4, 16, 4, true>(c->stream, g)));
             } else {
                 if (tile == 32) PE_CUDA(c, (launch_contract<32, 32, 2, 2, 16, 3, false>(c->stream, g)));
@@ -634,35 +664,52 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             PE_CUDA(c, cudaGetLastError());
             pa.P = Pbuf;
         }
+        if (rr) ra.eps_kq = rr->eps_kq + (size_t)qs * nb2;
+        double* op = out ? out + (size_t)qs * nb1 * nb2 * d.nmodes : nullptr;
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
-            dim3 grid = use_mma ? dim3(ceil_div(nqs, QG)) : dim3(ceil_div(nb1, gb1), nqs);
-            const double2* Cp = c->C; long long ldc = N; int ldc_i = N;
             const double2* Up = Ukq + (size_t)qs * d.nw * nb2;
             const double2* Zp = ev + (size_t)qs * d.nmodes * d.nmodes;
             const double* wp = omega + (size_t)qs * d.nmodes;
-            double* op = out ? out + (size_t)qs * nb1 * nb2 * d.nmodes : nullptr;
-            int nw_ = d.nw, nm_ = d.nmodes, nb1_ = nb1, nb2_ = nb2, gb1_ = gb1, nqs_ = nqs, QG_ = QG;
-            if (rr) ra.eps_kq = rr->eps_kq + (size_t)qs * nb2;
-            void* args_mma[] = {&Cp, &ldc, &Up, &Zp, &wp, &op, &nqs_, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &QG_, &ra, &pa};
-            void* args_pl[] = {&Cp, &ldc_i, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &pa};
-            PE_CUDA(c, cudaLaunchKernel(rot_kernel, grid, dim3(rot_threads), use_mma ? args_mma : args_pl, rot_smem,
-                                        c->stream));
+            if (use_mma) {
+                // persistent: one CTA per SM walks the groups of QS q-points
+                pe::Rot3Args ar{c->C, Up, Zp, wp, op, nqs, d.nw, d.nmodes, nb1, nb2, PB, G.QS, G.gb1, ra, pa};
+                if (rows_per_k > 0) ar.ra.eps_k = ra.eps_k + (size_t)(qs / rows_per_k) * nb1;   // (qs is 0 in the stacked rates form)
+                void* args[] = {&ar};
+                const int grid = std::min(ceil_div(nqs, G.QS), kSMs);
+                PE_CUDA(c, cudaLaunchKernel(rot_kernel, dim3(grid), dim3(rot_threads), args, rot_smem, c->stream));
+            } else {
+                if (plain_scratch) op = plain_scratch;
+                const double2* Cp = c->C; long long ldc = ldcq;
+                int nw_ = d.nw, nm_ = d.nmodes, nb1_ = nb1, nb2_ = nb2, gb1_ = gb1, P_ = P, PB_ = PB;
+                void* args[] = {&Cp, &ldc, &P_, &PB_, &Up, &Zp, &wp, &op, &nw_, &nm_, &nb1_, &nb2_, &gb1_, &pa};
+                for (int y0 = 0; y0 < nqs; y0 += 65535) {          // grid.y limit
+                    const int ny = std::min(65535, nqs - y0);
+                    const double2* Cy = c->C + (size_t)y0 * ldcq; const double2* Uy = Up + (size_t)y0 * d.nw * nb2;
+                    const double2* Zy = Zp + (size_t)y0 * d.nmodes * d.nmodes; const double* wy = wp + (size_t)y0 * d.nmodes;
+                    double* oy = op + (size_t)y0 * nb1 * nb2 * d.nmodes;
+                    pe::PolarArgs pay = pa;
+                    if (pay.P) pay.P += (size_t)y0 * d.nmodes;
+                    args[0] = &Cy; args[4] = &Uy; args[5] = &Zy; args[6] = &wy; args[7] = &oy; args[13] = &pay;
+                    PE_CUDA(c, cudaLaunchKernel(rot_kernel, dim3(ceil_div(nb1, gb1), ny), dim3(rot_threads), args, rot_smem,
+                                                c->stream));
+                }
+            }
         }
         if (rr) {
-            int nparts = ceil_div(nqs, QG);
+            int nparts = nqs * G.nmg;                   // rotate_v3: one partial row per (q, group of b2 tiles)
             if (!use_mma) {        // plain rotation path: sum from the stored |g|^2, 32 q per warp
                 const int QC = 32;
                 nparts = ceil_div(nqs, QC);
                 LaunchScope ls(c, PHOEBE_ELPH_K_ROTATE_EPI);
-                pe::k_rates_from_out<<<dim3(nparts, nb1), 32, 0, c->stream>>>(
-                    out + (size_t)qs * nb1 * nb2 * d.nmodes, omega + (size_t)qs * d.nmodes, nqs, d.nmodes, nb1, nb2, QC, ra);
+                pe::k_rates_from_out<<<dim3(nparts, nb1), 32, 0, c->stream>>>(op, omega + (size_t)qs * d.nmodes, nqs, d.nmodes,
+                                                                              nb1, nb2, QC, ra);
                 PE_CUDA(c, cudaGetLastError());
             }
             LaunchScope ls(c, PHOEBE_ELPH_K_RATE_REDUCE);
             const double scale = rr->prm.pref / (sqrt(3.14159265358979323846) * rr->prm.sigma);
             if (rows_per_k > 0)        // one (partial rows, rate[nb1]) block per k slot
-                pe::k_rate_reduce<<<dim3(nb1, nq / rows_per_k), 256, 0, c->stream>>>(partial, rows_per_k / QG, nb1, scale, rr->rate);
+                pe::k_rate_reduce<<<dim3(nb1, nq / rows_per_k), 256, 0, c->stream>>>(partial, rows_per_k * G.nmg, nb1, scale, rr->rate);
             else
                 pe::k_rate_reduce<<<nb1, 256, 0, c->stream>>>(partial, nparts, nb1, scale, rr->rate);
             PE_CUDA(c, cudaGetLastError());
@@ -811,6 +858,9 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
             up(c->pair_w, h_w.data(), h_w.size() * 8);
         }
     }
+    // the padding elements of the C layout (rotate_v3.cuh) are read, never written: they must hold finite values
+    if (e == cudaSuccess)
+        e = cudaMemsetAsync(c->C, 0, (size_t)L.nq_sub * c_elems_per_q(*dims, dims->nb1_max) * 16, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { delete c; return PHOEBE_ELPH_E_CUDA; }
     *ctx_out = c;
@@ -967,6 +1017,9 @@ int async_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_hos
     double* se1 = srate + d.nb1_max;
     double* se2 = reinterpret_cast<double*>(c->ws + c->L.off_seps) + (size_t)slot * d.nq_max * d.nb2_max;
     if (rh) {
+        // srate is the one buffer both the copy-in and the copy-out stream touch: the copy-out of the batch that last
+        // used this slot must have read it before the next initial values land
+        if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->s_in, c->ev_out[slot], 0));
         PE_CUDA(c, cudaMemcpyAsync(srate, rh->rate, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
         PE_CUDA(c, cudaMemcpyAsync(se1, rh->eps_k, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
         PE_CUDA(c, cudaMemcpyAsync(se2, rh->eps_kq, (size_t)nq * nb2 * 8, cudaMemcpyHostToDevice, c->s_in));
@@ -1220,12 +1273,14 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PHOEBE_ELPH_E_NULL;
     if (!strcmp(key, "nq_sub")) {
         if (value < 1) return fail(c, PHOEBE_ELPH_E_DIMS, "nq_sub must be >= 1");
-        c->nq_sub = (int)std::min<int64_t>(value, c->L.nq_sub);
+        // a multiple of the phase padding (128): sub-batch offsets then never split a contraction row tile (stacked
+        // forms: a tile must not straddle two k slots)
+        c->nq_sub = (int)std::min<int64_t>(std::max<int64_t>(kQPad, value / kQPad * kQPad), c->L.nq_sub);
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "tile")) {
-        if (value != 0 && value != 32 && value != 64 && value != 6432)
-            return fail(c, PHOEBE_ELPH_E_DIMS, "tile must be 0, 32, 64 or 6432");
+        if (value != 0 && value != 32 && value != 64)
+            return fail(c, PHOEBE_ELPH_E_DIMS, "tile must be 0, 32 or 64");
         c->tile = (int)value;
         return PHOEBE_ELPH_OK;
     }
@@ -1243,7 +1298,6 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
-    if (!strcmp(key, "rot_v1")) { c->rot_v1 = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_qg") || !strcmp(key, "rot_gb1") || !strcmp(key, "rot_mtw")) {
         if (value < 0 || value > 1024) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation geometry override out of range");
         (key[4] == 'q' ? c->rot_qg : key[4] == 'g' ? c->rot_gb1 : c->rot_mtw) = (int)value;

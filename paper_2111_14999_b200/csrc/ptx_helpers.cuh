@@ -69,4 +69,14 @@ __device__ __forceinline__ double neg(double x) {   // sign flip on the integer 
     return __hiloint2double(__double2hiint(x) ^ 0x80000000, __double2loint(x));
 }
 
+// ---- layout of the contraction result C[q][(b1, w2, ka)] (read by rotate_v3.cuh) -----------------------------
+// element (b1, w2, ka) of a q-point sits at b1*PB + w2*P + ka with P >= nm, PB = nw*P + padB; column n of the GEMM is
+// (b1*nw + w2)*nm + ka.  nm == 0: the plain layout (offset = n), also used by the a1 GEMM.
+struct CMap { int nm, nw, P, padB; };
+__device__ __forceinline__ long long cmap_off(int n, const CMap& m) {
+    if (m.nm == 0) return n;
+    const int r = n / m.nm, ka = n - r * m.nm;
+    return (long long)r * m.P + (long long)(r / m.nw) * m.padB + ka;
+}
+
 }  // namespace pe

@@ -138,7 +138,7 @@ template <int BM, int BN, int WARPS_M, int WARPS_N, int KC, int STAGES, bool M3,
 __global__ void __launch_bounds__((WARPS_M * WARPS_N + 1) * 32, MINB)
 k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ B, int ldb, long long strideB,
            double2* __restrict__ C, long long ldc, long long strideC, int M, int N, int K, int Kpad, int nbatch,
-           int rowsPerB, int rowOffset, long long strideBrow, int panelW)
+           int rowsPerB, int rowOffset, long long strideBrow, int panelW, CMap cm)
 {
     using Cfg = ContractCfg<BM, BN, WARPS_M, WARPS_N, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, LDA = Cfg::LDA, LDB = Cfg::LDB;
@@ -314,254 +314,40 @@ k_contract(const double2* __restrict__ At, int lda, const double2* __restrict__ 
 #pragma unroll
         for (int j = 0; j < TN; ++j) {
             const int n = n0 + wn * TN * 8 + j * 8 + 2 * t;
-            double2* dst = C + (size_t)z * strideC + (size_t)mm * ldc + n;
-            if (n < N) dst[0] = make_double2(cr[i][j][0], ci[i][j][0]);
-            if (n + 1 < N) dst[1] = make_double2(cr[i][j][1], ci[i][j][1]);
+            double2* dst = C + (size_t)z * strideC + (size_t)mm * ldc;
+            if (n < N) dst[cmap_off(n, cm)] = make_double2(cr[i][j][0], ci[i][j][0]);
+            if (n + 1 < N) dst[cmap_off(n + 1, cm)] = make_double2(cr[i][j][1], ci[i][j][1]);
         }
     }
     }   // tile loop
 }
 
 // ---------------------------------------------------------------------------
-// a5..a7 on the FP64 tensor cores, chained in registers.  A warp takes work items (q, b1, mt)
-// with mt an 8-row tile of b2:
-//   a5  D[b2][ka] = sum_w2 Uh[b2][w2] C[b1][w2][ka]      A = Uh (8x4 per k-step), B = C panel, K = nw
-//   a6  E[b2][nu] = sum_ka D[b2][ka] Z[ka][nu]            A = D straight from the a5 accumulators
-//   a7  out = |E|^2 * 1/(2 omega)
-// The DMMA accumulator of lane (g,t) holds D[g][2t], D[g][2t+1]; as the A operand of the next
-// product it must hold A[g][k-slot t].  The sum over ka may run in any order, so k-step (j,s) of
-// a6 is DEFINED to cover ka = 8j + 2t + s (t = 0..3): the accumulator registers are then the A
-// fragments as they stand and the B fragment is Z[8j + 2t + s][8n + g] -- no shuffles, no
-// shared-memory round trip.
-// Shared memory: Us[nwp][ldu] = conj(Ukq) zero padded (ldu = 2 mod 8 complex: conflict-free A
-// loads), Zs[8NT][ldz] zero padded (ldz = 1 mod 4), inv2w[8NT], Cs = the contiguous C panel of
-// a (q, b1 group) brought in by ONE TMA bulk copy, followed by zeroed slack so that the padded
-// k-steps / columns read finite values (they multiply zero rows of Us / Zs).
-// NT = ceil(nm / 8) <= 6.
+// Arguments shared by the rotation kernels (rotate_v3.cuh; the plain fallback below).
 //
-// RATES = true (Eq. 29 L229 with the Gaussian delta of Eq. 61): every
-// |g|^2 value is also multiplied by the occupation/energy-conservation bracket
+// RATES (Eq. 29 L229 with the Gaussian delta of Eq. 61): every |g|^2 value is also
+// multiplied by the occupation/energy-conservation bracket
 //   W = (1 - f' + n) G(eps_k[b1] - omega - eps_kq[q][b2]) + (f' + n) G(eps_k[b1] + omega - eps_kq[q][b2]),
 //   G(x) = exp(-x^2/sigma^2),  f' = 1/(e^{(eps_kq - mu)/kT} + 1),  n = 1/(e^{omega/kT} - 1)
-// and summed over (q, b2, nu) of the CTA in a fixed order: partial[blockIdx.x][b1].  k_rate_reduce adds
-// the partials (fixed order) times pref/(sqrt(pi) sigma) into rate[b1].  `out` may then be nullptr
-// (|g|^2 is not stored).  The extra shared arrays (omega, n, eps_kq, f', per-warp sums) follow Cs.
+// and summed over (b2, nu) in a fixed order into partial rows; k_rate_reduce adds the partial rows (fixed order) times
+// pref/(sqrt(pi) sigma) into rate[b1].  `out` may then be nullptr (|g|^2 is not stored).
 // ---------------------------------------------------------------------------
 struct RateArgs {
-    const double* eps_k;    // [nb1]; stacked form: [k slots][nb1], the slot of a CTA = (first q row of the CTA) / rows_per_k
+    const double* eps_k;    // [nb1]; stacked form: [k slots][nb1], the slot of a q-point = (its row) / rows_per_k
     const double* eps_kq;   // [nq][nb2] (of this launch)
     double inv_kT, mu, inv_sigma2;
-    double* partial;        // [gridDim.x][nb1]
-    int rows_per_k;         // > 0: the q lists of several k slots are stacked (host contract: a CTA never straddles two slots)
+    double* partial;        // rotate_v3: [nq][nmg][nb1], one row per (q, group of b2 tiles); plain path: [chunks][nb1]
+    int rows_per_k;         // > 0: the q lists of several k slots are stacked
 };
 
 // f4 (Eq. 14-15): when pa.P != nullptr the long-range amplitude P[q][nu] * O[q][b1][b2],
 // O = sum_w conj(Ukq[q][w][b2]) Uk[w][b1] (the overlap [U_kq^dagger U_k]_{b2 b1}), is added to E before |.|^2.
-// O of the CTA's q-points is formed once in shared memory from Us (already conjugated) and Uk.
+// rotate_v3 forms O on the tensor cores as one more column tile of a5 (B = U_k instead of the C panel).
 struct PolarArgs {
     const double2* P;     // [nq][nm] of this launch, or nullptr
     const double2* Uk;    // [nw][nb1]
     int conv;             // set_conventions: bit 0 = U_kq enters PLAIN (default: conjugated), bit 1 = ev enters CONJUGATED
 };
-
-template <int NT, bool RATES>
-__global__ void __launch_bounds__(128)
-k_rotate_epilogue_mma(const double2* __restrict__ C, long long ldc, const double2* __restrict__ Ukq,
-                      const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
-                      int nq, int nw, int nm, int nb1, int nb2, int gb1, int QG, RateArgs ra, PolarArgs pa)
-{
-    // One CTA = QG consecutive q-points; it walks the b1 groups (gb1 values of b1 each) with the C panels
-    // double-buffered: the TMA bulk copy of group i+1 runs while the warps do the DMMAs of group i.
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int nwp = (nw + 3) & ~3, MT = (nb2 + 7) >> 3;
-    const int ldu = MT * 8 + 2, ldz = NT * 8 + 1, Y = nw * nm;
-    const int slack = 4 * nm + 8;
-    const size_t panel = (size_t)gb1 * Y + slack;                       // complex elements of one (q, group) buffer
-    const int ngroups = (nb1 + gb1 - 1) / gb1;
-    const int nbuf = ngroups > 1 ? 2 : 1;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);                               // [2]
-    double* inv2w = reinterpret_cast<double*>(smem_raw + 16);                            // [QG][8 NT]
-    double2* Us = reinterpret_cast<double2*>(smem_raw + 16 + (size_t)QG * 8 * NT * sizeof(double));   // [QG][nwp][ldu]
-    double2* Zs = Us + (size_t)QG * nwp * ldu;                                           // [QG][8 NT][ldz]
-    double2* Cs = Zs + (size_t)QG * 8 * NT * ldz;                                        // [nbuf][QG][panel]
-    double* om_s = reinterpret_cast<double*>(Cs + (size_t)nbuf * QG * panel);            // [QG][8 NT]   (RATES only)
-    double* bose_s = om_s + QG * 8 * NT;                                                 // [QG][8 NT]
-    double* e2_s = bose_s + QG * 8 * NT;                                                 // [QG][8 MT]
-    double* f2_s = e2_s + QG * 8 * MT;                                                   // [QG][8 MT]
-    double* wsum = f2_s + QG * 8 * MT;                                                   // [4 warps][nb1]
-    // polar arrays follow the rate arrays when those exist, else Cs (host sizes the block the same way)
-    double2* Ps = reinterpret_cast<double2*>(RATES ? wsum + ((4 * nb1 + 1) & ~1) : om_s);   // [QG][8 NT]
-    double2* Os = Ps + QG * 8 * NT;                                                       // [QG][nb1][8 MT]
-    const bool polar = pa.P != nullptr;
-    const int q0 = blockIdx.x * QG;
-    const int nql = min(QG, nq - q0);
-    if (threadIdx.x == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); mbar_fence_init(); }
-    __syncthreads();
-    auto issue = [&](int grp) {             // thread 0: bring the C panels of group grp (all nql q-points) in
-        const int b10 = grp * gb1;
-        const int nb1l = min(gb1, nb1 - b10);
-        const uint32_t bytes = (uint32_t)((size_t)nb1l * Y * sizeof(double2));
-        uint64_t* fb = bar + (grp & 1);
-        mbar_arrive_expect_tx(fb, bytes * (uint32_t)nql);
-        for (int ql = 0; ql < nql; ++ql)
-            bulk_g2s(Cs + ((size_t)(grp & (nbuf - 1)) * QG + ql) * panel,
-                     C + (size_t)(q0 + ql) * ldc + (size_t)b10 * Y, bytes, fb);
-    };
-    if (threadIdx.x == 0) issue(0);
-    // while the first panels are in flight: conj(Ukq) -> Us, ev -> Zs, 1/(2 omega), zero padding / slack
-    for (int i = threadIdx.x; i < nql * nwp * ldu; i += blockDim.x) {
-        const int ql = i / (nwp * ldu), r = i - ql * nwp * ldu;
-        const int w2 = r / ldu, b2 = r - w2 * ldu;
-        double2 u = make_double2(0.0, 0.0);
-        if (w2 < nw && b2 < nb2) { u = Ukq[((size_t)(q0 + ql) * nw + w2) * nb2 + b2]; if (!(pa.conv & 1)) u.y = -u.y; }
-        Us[i] = u;
-    }
-    for (int i = threadIdx.x; i < nql * 8 * NT * ldz; i += blockDim.x) {
-        const int ql = i / (8 * NT * ldz), r = i - ql * 8 * NT * ldz;
-        const int ka = r / ldz, nu = r - ka * ldz;
-        double2 zv = (ka < nm && nu < nm) ? ev[((size_t)(q0 + ql) * nm + ka) * nm + nu] : make_double2(0.0, 0.0);
-        if (pa.conv & 2) zv.y = -zv.y;
-        Zs[i] = zv;
-    }
-    for (int i = threadIdx.x; i < nql * 8 * NT; i += blockDim.x) {
-        const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
-        const double w = (nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
-        inv2w[i] = (w > 0.0) ? 0.5 / w : 0.0;
-    }
-    for (int i = threadIdx.x; i < nbuf * QG * slack; i += blockDim.x) {
-        const int bq = i / slack, r = i - bq * slack;
-        Cs[(size_t)bq * panel + (size_t)gb1 * Y + r] = make_double2(0.0, 0.0);
-    }
-    if (RATES) {
-        for (int i = threadIdx.x; i < QG * 8 * NT; i += blockDim.x) {
-            const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
-            const double w = (ql < nql && nu < nm) ? omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
-            om_s[i] = w;
-            bose_s[i] = (w > 0.0) ? 1.0 / (exp(w * ra.inv_kT) - 1.0) : 0.0;
-        }
-        for (int i = threadIdx.x; i < QG * 8 * MT; i += blockDim.x) {
-            const int ql = i / (8 * MT), b2 = i - ql * 8 * MT;
-            const bool ok = ql < nql && b2 < nb2;
-            const double e2 = ok ? ra.eps_kq[(size_t)(q0 + ql) * nb2 + b2] : 0.0;
-            e2_s[i] = e2;
-            f2_s[i] = ok ? 1.0 / (exp((e2 - ra.mu) * ra.inv_kT) + 1.0) : 0.0;
-        }
-        for (int i = threadIdx.x; i < 4 * nb1; i += blockDim.x) wsum[i] = 0.0;
-    }
-    if (polar) {
-        for (int i = threadIdx.x; i < QG * 8 * NT; i += blockDim.x) {
-            const int ql = i / (8 * NT), nu = i - ql * 8 * NT;
-            Ps[i] = (ql < nql && nu < nm) ? pa.P[(size_t)(q0 + ql) * nm + nu] : make_double2(0.0, 0.0);
-        }
-        __syncthreads();                    // Us complete
-        for (int i = threadIdx.x; i < nql * nb1 * 8 * MT; i += blockDim.x) {
-            const int ql = i / (nb1 * 8 * MT), r = i - ql * nb1 * 8 * MT;
-            const int b1 = r / (8 * MT), b2 = r - b1 * 8 * MT;
-            double sr = 0.0, si = 0.0;
-            if (b2 < nb2) {
-                const double2* us = Us + (size_t)ql * nwp * ldu + b2;
-                for (int w = 0; w < nw; ++w) {
-                    const double2 u = us[(size_t)w * ldu], k = pa.Uk[(size_t)w * nb1 + b1];
-                    sr = fma(u.x, k.x, sr); sr = fma(-u.y, k.y, sr);
-                    si = fma(u.x, k.y, si); si = fma(u.y, k.x, si);
-                }
-            }
-            Os[i] = make_double2(sr, si);
-        }
-    }
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    const int g = lane >> 2, t = lane & 3;
-    const int nks = nwp >> 2;
-    for (int grp = 0; grp < ngroups; ++grp) {
-        __syncthreads();                    // everyone is done with the buffer group grp+1 will overwrite (and with the fills)
-        if (threadIdx.x == 0 && grp + 1 < ngroups) issue(grp + 1);
-        mbar_wait(bar + (grp & 1), (uint32_t)(grp >> 1) & 1u);
-        const int b10 = grp * gb1;
-        const int nb1l = min(gb1, nb1 - b10);
-        const int per_q = nb1l * MT;
-        for (int item = warp; item < nql * per_q; item += nwarps) {
-            const int ql = item / per_q, r = item - ql * per_q;
-            const int b1 = r / MT, mt = r - b1 * MT;
-            double dr[NT][2], di[NT][2];
-#pragma unroll
-            for (int j = 0; j < NT; ++j) { dr[j][0] = dr[j][1] = 0.0; di[j][0] = di[j][1] = 0.0; }
-            const double2* ua = Us + ((size_t)ql * nwp + t) * ldu + mt * 8 + g;
-            const double2* cb = Cs + ((size_t)(grp & (nbuf - 1)) * QG + ql) * panel + (size_t)b1 * Y + (size_t)t * nm + g;
-            for (int ks = 0; ks < nks; ++ks) {
-                const double2 a = ua[(size_t)ks * 4 * ldu];
-                const double nai = neg(a.y);
-#pragma unroll
-                for (int j = 0; j < NT; ++j) {
-                    const double2 b = cb[(size_t)ks * 4 * nm + j * 8];
-                    dmma884(dr[j][0], dr[j][1], a.x, b.x);
-                    dmma884(di[j][0], di[j][1], a.x, b.y);
-                    dmma884(dr[j][0], dr[j][1], nai, b.y);
-                    dmma884(di[j][0], di[j][1], a.y, b.x);
-                }
-            }
-            const int b2 = mt * 8 + g;
-            double* orow = out + (((size_t)(q0 + ql) * nb1 + b10 + b1) * nb2 + b2) * nm;
-            const double2* zq = Zs + (size_t)ql * 8 * NT * ldz;
-            const double* iw = inv2w + ql * 8 * NT;
-            double racc = 0.0, x12 = 0.0, f2 = 0.0;
-            if (RATES) {
-                x12 = ra.eps_k[(ra.rows_per_k > 0 ? (q0 / ra.rows_per_k) * nb1 : 0) + b10 + b1] - e2_s[ql * 8 * MT + b2];
-                f2 = f2_s[ql * 8 * MT + b2];
-            }
-#pragma unroll 1
-            for (int n = 0; n < NT; ++n) {       // not unrolled: keeps at most 2 NT fragments of Z in registers
-                double er[2] = {0.0, 0.0}, ei[2] = {0.0, 0.0};
-#pragma unroll
-                for (int j = 0; j < NT; ++j)
-#pragma unroll
-                    for (int sl = 0; sl < 2; ++sl) {
-                        const double2 z = zq[(size_t)(8 * j + 2 * t + sl) * ldz + 8 * n + g];
-                        const double ar = dr[j][sl], ai = di[j][sl];
-                        dmma884(er[0], er[1], ar, z.x);
-                        dmma884(ei[0], ei[1], ar, z.y);
-                        dmma884(er[0], er[1], neg(ai), z.y);
-                        dmma884(ei[0], ei[1], ai, z.x);
-                    }
-                const int nu = 8 * n + 2 * t;
-                if (polar) {
-                    const double2 o = Os[((size_t)ql * nb1 + b10 + b1) * 8 * MT + b2];
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const double2 pz = Ps[ql * 8 * NT + nu + h];
-                        er[h] += pz.x * o.x - pz.y * o.y;
-                        ei[h] += pz.x * o.y + pz.y * o.x;
-                    }
-                }
-                if (b2 < nb2) {
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        if (nu + h >= nm) continue;
-                        const double v = (er[h] * er[h] + ei[h] * ei[h]) * iw[nu + h];
-                        if (!RATES || out != nullptr) orow[nu + h] = v;
-                        if (RATES) {
-                            const double w = om_s[ql * 8 * NT + nu + h], bn = bose_s[ql * 8 * NT + nu + h];
-                            const double dm = x12 - w, dp = x12 + w;
-                            const double W = (1.0 - f2 + bn) * exp(-(dm * dm) * ra.inv_sigma2) +
-                                             (f2 + bn) * exp(-(dp * dp) * ra.inv_sigma2);
-                            racc = fma(v, W, racc);
-                        }
-                    }
-                }
-            }
-            if (RATES) {            // fixed-order sum over the warp, then into this warp's own row of wsum
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) racc += __shfl_xor_sync(0xffffffffu, racc, o);
-                if (lane == 0) wsum[warp * nb1 + b10 + b1] += racc;
-            }
-        }
-    }
-    if (RATES) {
-        __syncthreads();
-        for (int b = threadIdx.x; b < nb1; b += blockDim.x)
-            ra.partial[(size_t)blockIdx.x * nb1 + b] = ((wsum[b] + wsum[nb1 + b]) + wsum[2 * nb1 + b]) + wsum[3 * nb1 + b];
-    }
-}
 
 // Standalone form of the same sum for the plain rotation path (nm > 48): one warp per (chunk of QC
 // q-points, b1) reads the stored |g|^2 and writes partial[chunk][b1].
@@ -614,7 +400,7 @@ k_rate_reduce(const double* __restrict__ partial, int nparts, int nb1, double sc
 // smem: Uc[nw][nb2] (already conjugated), Z[nm][nm], Cs[gb1][nw*nm], Ds[gb1][nb2*nm]
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restrict__ Ukq,
+k_rotate_epilogue(const double2* __restrict__ C, long long ldc, int P, int PB, const double2* __restrict__ Ukq,
                   const double2* __restrict__ ev, const double* __restrict__ omega, double* __restrict__ out,
                   int nw, int nm, int nb1, int nb2, int gb1, PolarArgs pa)
 {
@@ -631,8 +417,11 @@ k_rotate_epilogue(const double2* __restrict__ C, int ldc, const double2* __restr
     for (int i = threadIdx.x; i < nw * nb2; i += blockDim.x) { double2 u = Uq[i]; Uc[i] = make_double2(u.x, (pa.conv & 1) ? u.y : -u.y); }
     const double2* Zq = ev + (size_t)iq * nm * nm;
     for (int i = threadIdx.x; i < nm * nm; i += blockDim.x) { double2 zv = Zq[i]; if (pa.conv & 2) zv.y = -zv.y; Z[i] = zv; }
-    const double2* Cq = C + (size_t)iq * ldc + (size_t)b10 * Y;
-    for (int i = threadIdx.x; i < nb1l * Y; i += blockDim.x) Cs[i] = Cq[i];
+    const double2* Cq = C + (size_t)iq * ldc + (size_t)b10 * PB;      // element (b1, w2, ka) at b1*PB + w2*P + ka
+    for (int i = threadIdx.x; i < nb1l * Y; i += blockDim.x) {
+        const int b1 = i / Y, r = i - b1 * Y, w2 = r / nm, ka = r - w2 * nm;
+        Cs[i] = Cq[(size_t)b1 * PB + (size_t)w2 * P + ka];
+    }
     __syncthreads();
     // a5
     const int nD = nb1l * nb2 * nm;

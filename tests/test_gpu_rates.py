@@ -186,9 +186,9 @@ def test_rates_async_pipelined_host_batches(env):
     ctx.close()
 
 
-@pytest.mark.parametrize("shape", [(8, 4, 4, 6, 192, {}), (12, 5, 12, 12, 128, {}), (5, 3, 4, 21, 64, {"rot_v1": 1}),
+@pytest.mark.parametrize("shape", [(8, 4, 4, 6, 192, {}), (12, 5, 12, 12, 128, {}), (5, 3, 4, 21, 64, {"rot_qg": 1}),
                                    (8, 4, 4, 6, 192, {"rot_qg": 5})],
-                         ids=["band_window_shape", "two_m_tiles", "first_form", "qg_not_dividing"])
+                         ids=["band_window_shape", "two_m_tiles", "one_q_per_stage", "qg_not_dividing"])
 def test_rates_multi_equals_oracle_per_k(env, shape):
     """phoebe_elph_q_batch_rates_multi: the q lists of all k slots of a set_k_batch stacked into one pass; every k slot's
     linewidths (and |g|^2 when stored) against the oracle, and against per-k q_batch_rates calls."""

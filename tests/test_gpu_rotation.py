@@ -1,7 +1,9 @@
-"""GPU parity of the second tensor-core form of steps a5-a7 (k_rotate_epilogue_v2: packed (b1, kappa) columns,
-three-multiply product): every k-step count KS = ceil(nm/4) in 1..12, one and two 8-row tiles of b2 per warp item,
-odd nb1 (the half-used b1 pair), ragged nb2 / nw, several b1 groups per q, and the fused linewidth sum --
-each element by element against the CPU oracle, and against the first form (tuning "rot_v1") on the same input.
+"""GPU parity of steps a5-a7 on the tensor cores (k_rotate_v3: persistent, producer warp + TMA rings, packed (b1, kappa)
+columns, three-multiply product): every k-step count KS = ceil(nm/4) in 1..12 and every residue of nm mod 4 (the padded
+row pitch of C for nm = 0 mod 4, the interleaved kappa order for nm = 2 mod 4), one and two 8-row tiles of b2 per warp
+item, every b1-per-item variant, odd nb1 (the half-used b1 pair), ragged nb2 / nw, several b1 groups per q (C panel
+larger than a stage), forced stage geometries, and the fused linewidth sum -- each element by element against the CPU
+oracle, and against the plain DFMA kernel (tuning "rot_plain") on the same input.
 Bar: max |out_gpu - out_oracle| <= 1e-10 * max(out_oracle)  (north_star, reading R10).
 """
 import numpy as np
@@ -40,12 +42,18 @@ CASES = [(5, 3, 4, nm, 37) for nm in (4, 5, 17, 21, 22, 25, 33, 37, 41, 48)] + \
     (32, 5, 12, 30, 9),       # several b1 groups per q (C panel of a q > 64 KB), KS = 8
     (40, 9, 20, 12, 7),       # several groups, KS = 3 (b1 pairs), three 8-row tiles of b2 (odd: one clamped)
     (16, 16, 16, 12, 130),    # the 4-atom cell's shape
-    (8, 4, 4, 6, 1100),       # the band-window shape, 8 q per CTA, ragged last CTA
+    (8, 4, 4, 6, 1100),       # the band-window shape, 8 q per stage, ragged last stage
+    (8, 8, 8, 6, 700),        # the si-like shape: two items per q
+    (9, 9, 3, 2, 900),        # KS = 1 with 8 b1 per item (+ one left over)
+    (20, 4, 20, 3, 300),       # KS = 1, two m-tiles, 4 b1 per item
+    (9, 2, 9, 8, 200),        # KS = 2, two m-tiles, 2 b1 per item, nm = 0 mod 8
+    (7, 6, 7, 16, 100),       # KS = 4, 2 b1 per item
+    (32, 32, 32, 30, 5),      # the large cell's shape: b1 groups, two rings
 ]
 
 
 @pytest.mark.parametrize("case", CASES, ids=lambda c: "nw%d_nb%d_%d_nm%d" % c[:4])
-def test_v2_matches_oracle_and_v1(env, case):
+def test_rotation_matches_oracle_and_plain_kernel(env, case):
     wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
     nw, nb1, nb2, nm, nq = case
     w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=(2, 1, 1), grid_p=(1, 2, 1), nq=nq, cfg_id=120 + nm)
@@ -55,7 +63,7 @@ def test_v2_matches_oracle_and_v1(env, case):
     ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
     d = harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])
     out2 = ctx.q_batch(*d).cpu().numpy()
-    ctx.set_tuning("rot_v1", 1)
+    ctx.set_tuning("rot_plain", 1)
     out1 = ctx.q_batch(*d).cpu().numpy()
     ctx.close()
     assert out2.shape == ref.shape
@@ -64,10 +72,30 @@ def test_v2_matches_oracle_and_v1(env, case):
     assert _relerr(out2, out1) <= TOL
 
 
+@pytest.mark.parametrize("knob", [{"rot_qg": 1}, {"rot_qg": 3}, {"rot_gb1": 2}, {"rot_gb1": 1}, {"rot_mtw": 1}],
+                         ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
+def test_rotation_forced_stage_geometry(env, knob):
+    """q-points per stage, b1 per C stage (the two-ring form on a small problem) and m-tiles per item forced."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=12, nb1=5, nb2=12, nm=10, grid_e=(2, 1, 1), grid_p=(1, 2, 1), nq=333, cfg_id=119)
+    a = _inputs(wl, w)
+    ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=w.nq)
+    for key, val in knob.items():
+        ctx.set_tuning(key, val)
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    d = harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])
+    out = ctx.q_batch(*d).cpu().numpy()
+    again = ctx.q_batch(*d).cpu().numpy()
+    ctx.close()
+    assert _relerr(out, ref) <= TOL
+    assert np.array_equal(out, again)
+
+
 @pytest.mark.parametrize("case", [(12, 5, 12, 12, 150), (12, 5, 12, 30, 40), (40, 9, 20, 12, 7), (5, 3, 4, 21, 300)],
                          ids=lambda c: "nw%d_nb%d_%d_nm%d" % c[:4])
-def test_v2_fused_rates(env, case):
-    """Eq. 29 linewidth sum inside the v2 epilogue (two m-tiles per item, b1 pairs, several groups)."""
+def test_rotation_fused_rates(env, case):
+    """Eq. 29 linewidth sum inside the epilogue (two m-tiles per item, b1 pairs, several groups)."""
     wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
     nw, nb1, nb2, nm, nq = case
     w = wl.custom(nw=nw, nb1=nb1, nb2=nb2, nm=nm, grid_e=(2, 1, 1), grid_p=(1, 2, 1), nq=nq, cfg_id=160 + nm)
