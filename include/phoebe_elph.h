@@ -309,7 +309,8 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
  *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the geometry of the tensor-core rotation kernel (rotate_v3.cuh):
  *               q-points per ring stage, b1 per C stage (forces the two-ring form), 8-row tiles of b2 per warp item
- *               (0 = automatic; measurement aids)                  */
+ *               (0 = automatic; measurement aids).  "rot_blk": how U_kq / ev reach shared memory: 0 = automatic,
+ *               1 = one bulk copy per row into padded rows, 2 = one bulk copy per q-point at the natural pitch      */
 int phoebe_elph_set_tuning(phoebe_elph_ctx* ctx, const char* key, int64_t value);
 int phoebe_elph_get_tuning(const phoebe_elph_ctx* ctx, const char* key, int64_t* value);
 

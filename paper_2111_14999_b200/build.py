@@ -21,22 +21,45 @@ def _deps():
             + glob.glob(os.path.join(ROOT, "include", "*.h")))
 
 
-def nvcc_cmd(verbose: bool = False):
+OBJ_DIR = os.path.join(HERE, "build")
+ROT3_SRC = os.path.join(HERE, "csrc", "rot3_instances.cu")
+ROT3_PARTS = 4
+
+
+def _nvcc_base(verbose: bool = False):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC",
-           "-o", LIB, SRC]
-    extra = os.environ.get("PHOEBE_ELPH_NVCC_FLAGS", "").split()      # e.g. -D switches of kernel experiments
-    cmd[1:1] = extra
+           "-Xcompiler", "-fPIC"]
+    cmd[1:1] = os.environ.get("PHOEBE_ELPH_NVCC_FLAGS", "").split()      # e.g. -D switches of kernel experiments
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     return cmd
 
 
+def nvcc_cmds(verbose: bool = False):
+    """-> (compile commands, link command): the C ABI + most kernels (phoebe_elph.cu) and the instantiations of the
+    rotation kernel in ROT3_PARTS translation units, compiled in parallel, linked into one shared library."""
+    base = _nvcc_base(verbose)
+    objs = [os.path.join(OBJ_DIR, "phoebe_elph.o")] + [os.path.join(OBJ_DIR, "rot3_part%d.o" % i) for i in range(ROT3_PARTS)]
+    compiles = [base + ["-c", SRC, "-o", objs[0]]]
+    compiles += [base + ["-DROT3_PART=%d" % i, "-c", ROT3_SRC, "-o", objs[1 + i]] for i in range(ROT3_PARTS)]
+    link = [base[0], "-shared", "-o", LIB] + objs
+    return compiles, link
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
-    subprocess.run(nvcc_cmd(verbose), check=True)
+    import concurrent.futures as cf
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    compiles, link = nvcc_cmds(verbose)
+    with cf.ThreadPoolExecutor(len(compiles)) as pool:
+        for r in pool.map(lambda c: subprocess.run(c, capture_output=True, text=True), compiles):
+            if verbose or r.returncode:
+                sys.stderr.write(r.stdout + r.stderr)
+            if r.returncode:
+                raise subprocess.CalledProcessError(r.returncode, r.args)
+    subprocess.run(link, check=True)
     return LIB
 
 

@@ -169,6 +169,7 @@ struct phoebe_elph_ctx {
     bool m3 = true;           // tuning "m3": three-multiply complex product (3 DMMA per tile and k-step instead of 4)
     int tile = 0;             // tuning "tile": 0 = automatic, 32 / 64 = force the contraction tile
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
+    int rot_blk = 0;          // tuning "rot_blk": U_kq / ev staging of the rotation kernel: 0 automatic, 1 row copies, 2 one block per q
     int rot_qg = 0, rot_gb1 = 0, rot_mtw = 0;   // tuning "rot_qg" / "rot_gb1" / "rot_mtw": override the v2 rotation geometry (0 = automatic)
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
@@ -430,44 +431,25 @@ int rot3_max_gb(int KS, int MTW)
     if (MTW == 1) return KS == 1 ? 8 : KS == 2 ? 4 : (KS == 3 || KS == 4) ? 2 : 1;
     return KS == 1 ? 4 : (KS == 2 || KS == 3) ? 2 : 1;
 }
-template <int KS, int GB, int MTW>
-const void* rot3_pick(bool rates)
+// the instantiations live in rot3_instances.cu (four translation units by KS range)
+extern "C" const void* pe_rot3_kernel_part0(int KS, int GB, int MTW, int mode);
+extern "C" const void* pe_rot3_kernel_part1(int KS, int GB, int MTW, int mode);
+extern "C" const void* pe_rot3_kernel_part2(int KS, int GB, int MTW, int mode);
+extern "C" const void* pe_rot3_kernel_part3(int KS, int GB, int MTW, int mode);
+const void* rot3_kernel(int KS, int GB, int MTW, int mode)     // mode: 0 plain, 1 linewidths (f2), 3 polar (f4)
 {
-    return rates ? (const void*)pe::k_rotate_v3<KS, GB, MTW, true> : (const void*)pe::k_rotate_v3<KS, GB, MTW, false>;
-}
-template <int KS>
-const void* rot3_kernel_ks(int GB, int MTW, bool rates)
-{
-    constexpr int g0 = (KS == 1 || KS == 3) ? 2 : 1;
-    constexpr int g1 = KS == 1 ? 8 : KS == 2 ? 4 : (KS == 3 || KS == 4) ? 2 : 1;      // rot3_max_gb(KS, 1)
-    constexpr int g2 = KS == 1 ? 4 : (KS == 2 || KS == 3) ? 2 : 1;                    // rot3_max_gb(KS, 2)
-    if (MTW == 1) return GB == g1 ? rot3_pick<KS, g1, 1>(rates) : rot3_pick<KS, g0, 1>(rates);
-    return GB == g2 ? rot3_pick<KS, g2, 2>(rates) : rot3_pick<KS, g0, 2>(rates);
-}
-const void* rot3_kernel(int KS, int GB, int MTW, bool rates)
-{
-    switch (KS) {
-        case 1: return rot3_kernel_ks<1>(GB, MTW, rates);
-        case 2: return rot3_kernel_ks<2>(GB, MTW, rates);
-        case 3: return rot3_kernel_ks<3>(GB, MTW, rates);
-        case 4: return rot3_kernel_ks<4>(GB, MTW, rates);
-        case 5: return rot3_kernel_ks<5>(GB, MTW, rates);
-        case 6: return rot3_kernel_ks<6>(GB, MTW, rates);
-        case 7: return rot3_kernel_ks<7>(GB, MTW, rates);
-        case 8: return rot3_kernel_ks<8>(GB, MTW, rates);
-        case 9: return rot3_kernel_ks<9>(GB, MTW, rates);
-        case 10: return rot3_kernel_ks<10>(GB, MTW, rates);
-        case 11: return rot3_kernel_ks<11>(GB, MTW, rates);
-        default: return rot3_kernel_ks<12>(GB, MTW, rates);
-    }
+    if (KS <= 2) return pe_rot3_kernel_part0(KS, GB, MTW, mode);
+    if (KS <= 5) return pe_rot3_kernel_part1(KS, GB, MTW, mode);
+    if (KS <= 9) return pe_rot3_kernel_part2(KS, GB, MTW, mode);
+    return pe_rot3_kernel_part3(KS, GB, MTW, mode);
 }
 
 // geometry of one rotation launch
-struct Rot3Geom { int KS, GB, MTW, P, PB, QS, gb1, nmg; size_t smem; };
+struct Rot3Geom { int KS, GB, MTW, P, PB, QS, gb1, nmg, blk; size_t smem; };
 constexpr size_t kRot3SmemBudget = 200u << 10;
 
 bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_over, int gb1_over, int mtw_over,
-                   Rot3Geom* G)
+                   int blk_over, Rot3Geom* G)
 {
     const int KS = ceil_div(nm, 4), NT = ceil_div(nm, 8), MT = ceil_div(nb2, 8);
     G->KS = KS;
@@ -479,8 +461,15 @@ bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_
     // fragment loads conflict-free
     const int raw = nw * G->P;
     G->PB = raw + ((G->GB >= 2 && (KS & 1)) ? ((4 - raw % 8) + 8) % 8 : 0);
-    auto total = [&](int QS, int gb1) { return (size_t)pe::rot3_layout(nw, nm, nb2, G->PB, QS, gb1, rates).total; };
-    const int qs_cap = std::max(1, 128 / (8 * std::max(NT, MT)));      // the producer lanes' register slots
+    // U_kq / ev as one block per q-point when their nw + nm row copies (~80 clocks of the TMA unit each) would weigh
+    // more than half of the q-point's tensor work (4 clocks per DMMA): the small cells
+    const long dmma_q = 3L * ceil_div(nb1, G->GB) * G->nmg * G->MTW *
+                        ((long)ceil_div(G->GB * KS, 2) * ceil_div(nw, 4) + (long)G->GB * KS * NT);
+    G->blk = blk_over > 0 ? blk_over - 1 : (long)(nw + nm) * 80 > 2 * dmma_q;
+    auto total = [&](int QS, int gb1) { return (size_t)pe::rot3_layout(nw, nm, nb2, G->PB, QS, gb1, rates, G->blk != 0).total; };
+    if (G->blk && nb1 * G->PB > 8192) G->blk = 0;                  // (block mode is for whole-q stages)
+    int qs_cap = std::max(1, 128 / (8 * std::max(NT, MT)));            // the producer lanes' register slots
+    if (G->blk) qs_cap = std::min(qs_cap, 32);                         // one lane per q-point's block copy
     if (total(1, nb1) <= kRot3SmemBudget && gb1_over <= 0) {
         // whole q-points per stage: enough of them that every consumer warp has an item, while the q list still
         // gives every SM several stages
@@ -530,7 +519,8 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     size_t rot_smem = 0;
     int P = d.nmodes, PB = d.nw * d.nmodes;                 // C layout (plain for the DFMA kernel)
     if (use_mma) {
-        if (!rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), fused_rates, c->rot_qg, c->rot_gb1, c->rot_mtw, &G))
+        // the polar kernels (mode 3) always carry the Eq. 29 arrays in their stages
+        if (!rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), fused_rates || polar, c->rot_qg, c->rot_gb1, c->rot_mtw, c->rot_blk, &G))
             return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
         P = G.P; PB = G.PB; gb1 = G.gb1; rot_smem = G.smem;
     } else {
@@ -554,7 +544,9 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates without out: not available for nmodes > 48 at this size");
         plain_scratch = reinterpret_cast<double*>(c->C + (size_t)std::min(nq, nq_sub) * ldcq);
     }
-    const void* rot_kernel = use_mma ? rot3_kernel(G.KS, G.GB, G.MTW, fused_rates) : (const void*)pe::k_rotate_epilogue;
+    const void* rot_kernel = use_mma ? rot3_kernel(G.KS, G.GB, G.MTW, polar ? 3 : fused_rates ? 1 : 0)
+                                     : (const void*)pe::k_rotate_epilogue;
+    if (!rot_kernel) return fail(c, PHOEBE_ELPH_E_DIMS, "no rotation kernel for this mode count");
     double* partial = reinterpret_cast<double*>(c->ws + c->L.off_part);
     pe::RateArgs ra{nullptr, nullptr, 0.0, 0.0, 0.0, partial, 0};
     if (rr && rows_per_k > 0) {
@@ -673,7 +665,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             const double* wp = omega + (size_t)qs * d.nmodes;
             if (use_mma) {
                 // persistent: one CTA per SM walks the groups of QS q-points
-                pe::Rot3Args ar{c->C, Up, Zp, wp, op, nqs, d.nw, d.nmodes, nb1, nb2, PB, G.QS, G.gb1, ra, pa};
+                pe::Rot3Args ar{c->C, Up, Zp, wp, op, nqs, d.nw, d.nmodes, nb1, nb2, PB, G.QS, G.gb1, G.blk, ra, pa};
                 if (rows_per_k > 0) ar.ra.eps_k = ra.eps_k + (size_t)(qs / rows_per_k) * nb1;   // (qs is 0 in the stacked rates form)
                 void* args[] = {&ar};
                 const int grid = std::min(ceil_div(nqs, G.QS), kSMs);
@@ -1298,6 +1290,11 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "rot_blk")) {
+        if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
+        c->rot_blk = (int)value;
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "rot_qg") || !strcmp(key, "rot_gb1") || !strcmp(key, "rot_mtw")) {
         if (value < 0 || value > 1024) return fail(c, PHOEBE_ELPH_E_DIMS, "rotation geometry override out of range");
         (key[4] == 'q' ? c->rot_qg : key[4] == 'g' ? c->rot_gb1 : c->rot_mtw) = (int)value;

@@ -16,8 +16,7 @@
 // operand sums (conj(U): as = ur - ui, T2 enters with the opposite sign), so the raw inputs are used as they land.
 //
 // Two rings: the Q ring (U_kq, ev, 1/(2 omega), Eq. 29 factors of QS q-points per stage) and the C ring (the C panels
-// of those q-points; for cells whose panel does not fit, groups of gb1 values of b1).  A stage is released one stage
-// late (see k_contract: an LDS still in flight must not race the next bulk copy), hence three stages per ring.
+// of those q-points; for cells whose panel does not fit, groups of gb1 values of b1), three stages each.
 //
 // C layout (written by the contraction kernels): element (b1, w2, ka) of a q at b1*PB + w2*P + ka.  P = nm except
 // for nm = 0 mod 4, where the row pitch is nm + 1: the four k rows (w2) of a B fragment then fall into distinct
@@ -25,12 +24,15 @@
 // column tile (ka = 8i + 2t' + h instead of 4s + t'): the order of the ka sum is free.
 #pragma once
 #include "ptx_helpers.cuh"
-#include "qbatch_kernels.cuh"
+#include "rot_args.cuh"
 
 namespace pe {
 
 constexpr int kRot3Consumers = 8;
-constexpr int kRot3Threads = (kRot3Consumers + 1) * 32;
+// three warpgroups: two of consumer warps, one that holds the producer warp (its other three warps exit at once).
+// The register file is re-split between them at kernel start (setmaxnreg): 12 warps x 168 = 8 x 232 + 4 x 40.
+constexpr int kRot3Threads = (kRot3Consumers + 4) * 32;
+constexpr int kRot3RegsConsumer = 232, kRot3RegsProducer = 40;
 constexpr int kRot3Stages = 3;
 
 struct Rot3Layout {
@@ -41,18 +43,22 @@ struct Rot3Layout {
 // row pitch of the C layout for nm modes, and the b1 block pitch (pad chosen by the host, see rot3_block_pad)
 __host__ __device__ inline int rot3_row_pitch(int nm) { return (nm & 3) == 0 ? nm + 1 : nm; }
 
-__host__ __device__ inline Rot3Layout rot3_layout(int nw, int nm, int nb2, int PB, int QS, int gb1, bool rates)
+// blk: U_kq / ev of a q-point land as ONE bulk copy each, rows at their natural pitch (small cells: a bulk copy per
+// 64..128-byte row costs the TMA unit more than the few bank conflicts of the unpadded rows cost the consumers);
+// otherwise row by row into padded rows.
+__host__ __device__ inline Rot3Layout rot3_layout(int nw, int nm, int nb2, int PB, int QS, int gb1, bool rates, bool blk)
 {
     Rot3Layout L;
     const int P = rot3_row_pitch(nm);
     L.KS = (nm + 3) >> 2; L.NT = (nm + 7) >> 3; L.MT = (nb2 + 7) >> 3;
     L.nwp = (nw + 3) & ~3;
     L.mapB = (nm & 3) == 2;
-    L.ldu = L.MT * 8 + 2;                       // complex; = 2 mod 8: the 4 k rows of an A fragment hit distinct bank groups
-    L.ldz = L.NT * 8 + (L.mapB ? 1 : 2);        // mapB reads rows 2t apart: an odd pitch spreads them
+    L.ldu = blk ? nb2 : L.MT * 8 + 2;           // complex; = 2 mod 8: the 4 k rows of an A fragment hit distinct bank groups
+    L.ldz = blk ? nm : L.NT * 8 + (L.mapB ? 1 : 2);    // mapB reads rows 2t apart: an odd pitch spreads them
     L.slack = 3 * P + 4 * L.KS + 4;             // what the padded k rows / columns behind the last panel may read
-    L.szU = (uint32_t)QS * L.nwp * L.ldu * 16;
-    L.szZ = (uint32_t)QS * 4 * L.KS * L.ldz * 16;
+    // (blk: the last rows' column padding reads up to 7 elements past a q-point's block)
+    L.szU = (uint32_t)(QS * L.nwp * L.ldu + (blk ? 8 : 0)) * 16;
+    L.szZ = (uint32_t)(QS * 4 * L.KS * L.ldz + (blk ? 8 : 0)) * 16;
     L.szW = (uint32_t)QS * 8 * L.NT * 8;
     L.szR = rates ? (uint32_t)QS * (2 * 8 * L.NT + 2 * 8 * L.MT) * 8 : 0u;
     L.szQ = L.szU + L.szZ + L.szW + L.szR;
@@ -71,6 +77,7 @@ struct Rot3Args {
     double* out;            // [nq][nb1][nb2][nm] or nullptr (RATES only)
     int nq, nw, nm, nb1, nb2;
     int PB, QS, gb1;
+    int blk;                // U_kq / ev as one block per q-point (rot3_layout)
     RateArgs ra;            // ra.partial: [nq][nmg][nb1]
     PolarArgs pa;
 };
@@ -83,17 +90,22 @@ __device__ __forceinline__ int rot3_kappa(int s, int tt, int mapB)
     return 4 * s + tt;
 }
 
-template <int KS, int GB, int MTW, bool RATES>
+// MODE: 0 = |g|^2 only, 1 = with the linewidth sums of Eq. 29 (f2), 3 = with the polar term of Eq. 14-15 (f4; the
+// linewidth sums are then a run-time choice: a.ra.eps_k != nullptr)
+template <int KS, int GB, int MTW, int MODE>
 __global__ void __launch_bounds__(kRot3Threads, 1)
 k_rotate_v3(const Rot3Args a)
 {
+    constexpr bool RSM = (MODE & 1) != 0;                 // the Eq. 29 arrays exist in the Q stages
+    constexpr bool POLAR = (MODE & 2) != 0;
+    const bool rates = RSM && (MODE != 3 || a.ra.eps_k != nullptr);
     constexpr int TJ = (GB * KS + 1) / 2;                 // a5 column tiles per item
     constexpr int NT = (KS + 1) / 2;
     constexpr int NS = kRot3Stages;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int nw = a.nw, nm = a.nm, nb1 = a.nb1, nb2 = a.nb2, PB = a.PB, QS = a.QS, gb1 = a.gb1;
     const int P = rot3_row_pitch(nm);
-    const Rot3Layout L = rot3_layout(nw, nm, nb2, PB, QS, gb1, RATES);
+    const Rot3Layout L = rot3_layout(nw, nm, nb2, PB, QS, gb1, RSM, a.blk != 0);
     const int MT = L.MT, ldu = L.ldu, ldz = L.ldz, nwp = L.nwp, mapB = L.mapB;
     const int ngroups = (nb1 + gb1 - 1) / gb1;
     uint64_t* qfull = reinterpret_cast<uint64_t*>(smem_raw);
@@ -119,7 +131,9 @@ k_rotate_v3(const Rot3Args a)
     const int nqg = (a.nq + QS - 1) / QS;
     const long long ldcq = (long long)nb1 * PB;
 
-    if (warp == kRot3Consumers) {
+    if (warp >= kRot3Consumers) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRot3RegsProducer));
+        if (warp > kRot3Consumers) return;
         // ================= producer warp =================
         int sq = 0, sc = 0; uint32_t phq = 0, phc = 0;
         const int nW = 8 * NT, nE = 8 * MT;
@@ -127,14 +141,14 @@ k_rotate_v3(const Rot3Args a)
             const int q0 = qg * QS, nql = min(QS, a.nq - q0);
             // omega (and eps_kq) of this stage: loads issued BEFORE the wait for a free stage
             constexpr int WR = 4;                            // register slots per lane (QS * 8NT <= 32 * WR by host contract)
-            double wv[WR], ev2[RATES ? WR : 1];
+            double wv[WR], ev2[RSM ? WR : 1];
 #pragma unroll
             for (int r = 0; r < WR; ++r) {
                 const int i = lane + 32 * r, ql = i / nW, nu = i - ql * nW;
                 wv[r] = (ql < nql && nu < nm) ? a.omega[(size_t)(q0 + ql) * nm + nu] : 0.0;
-                if (RATES) {
+                if (RSM) {
                     const int qe = i / nE, b2 = i - qe * nE;
-                    ev2[r] = (qe < nql && b2 < nb2) ? a.ra.eps_kq[(size_t)(q0 + qe) * nb2 + b2] : 0.0;
+                    ev2[r] = (rates && qe < nql && b2 < nb2) ? a.ra.eps_kq[(size_t)(q0 + qe) * nb2 + b2] : 0.0;
                 }
             }
             mbar_wait(qempty + sq, phq ^ 1u);
@@ -142,21 +156,37 @@ k_rotate_v3(const Rot3Args a)
             double2* Us = reinterpret_cast<double2*>(Q);
             double2* Zs = reinterpret_cast<double2*>(Q + L.szU);
             double* iw = reinterpret_cast<double*>(Q + L.szU + L.szZ);
-            for (int i = lane; i < nql * nw; i += 32) {          // U_kq rows: [q][w2][nb2] -> Us[ql][w2][ldu]
-                const int ql = i / nw, w2 = i - ql * nw;
-                bulk_g2s(Us + ((size_t)ql * nwp + w2) * ldu, a.Ukq + ((size_t)(q0 + ql) * nw + w2) * nb2,
-                         (uint32_t)nb2 * 16u, qfull + sq);
-            }
-            for (int i = lane; i < nql * nm; i += 32) {          // ev rows: [q][ka][nm] -> Zs[ql][ka][ldz]
-                const int ql = i / nm, ka = i - ql * nm;
-                bulk_g2s(Zs + ((size_t)ql * 4 * KS + ka) * ldz, a.ev + ((size_t)(q0 + ql) * nm + ka) * nm,
-                         (uint32_t)nm * 16u, qfull + sq);
+            if (a.blk) {
+                // one copy per q-point (all q-points at once when there are no padding rows between their blocks)
+                if (nwp == nw) {
+                    if (lane == 0) bulk_g2s(Us, a.Ukq + (size_t)q0 * nw * nb2, (uint32_t)(nql * nw * nb2) * 16u, qfull + sq);
+                } else if (lane < nql) {
+                    bulk_g2s(Us + (size_t)lane * nwp * ldu, a.Ukq + (size_t)(q0 + lane) * nw * nb2, (uint32_t)(nw * nb2) * 16u,
+                             qfull + sq);
+                }
+                if (4 * KS == nm) {
+                    if (lane == 1) bulk_g2s(Zs, a.ev + (size_t)q0 * nm * nm, (uint32_t)(nql * nm * nm) * 16u, qfull + sq);
+                } else if (lane < nql) {
+                    bulk_g2s(Zs + (size_t)lane * 4 * KS * ldz, a.ev + (size_t)(q0 + lane) * nm * nm, (uint32_t)(nm * nm) * 16u,
+                             qfull + sq);
+                }
+            } else {
+                for (int i = lane; i < nql * nw; i += 32) {          // U_kq rows: [q][w2][nb2] -> Us[ql][w2][ldu]
+                    const int ql = i / nw, w2 = i - ql * nw;
+                    bulk_g2s(Us + ((size_t)ql * nwp + w2) * ldu, a.Ukq + ((size_t)(q0 + ql) * nw + w2) * nb2,
+                             (uint32_t)nb2 * 16u, qfull + sq);
+                }
+                for (int i = lane; i < nql * nm; i += 32) {          // ev rows: [q][ka][nm] -> Zs[ql][ka][ldz]
+                    const int ql = i / nm, ka = i - ql * nm;
+                    bulk_g2s(Zs + ((size_t)ql * 4 * KS + ka) * ldz, a.ev + ((size_t)(q0 + ql) * nm + ka) * nm,
+                             (uint32_t)nm * 16u, qfull + sq);
+                }
             }
 #pragma unroll
             for (int r = 0; r < WR; ++r) {
                 const int i = lane + 32 * r;
                 if (i < QS * nW) iw[i] = (wv[r] > 0.0) ? 0.5 / wv[r] : 0.0;
-                if (RATES) {
+                if (RSM) {
                     double* om_s = iw + QS * nW;
                     double* bose_s = om_s + QS * nW;
                     double* e2_s = bose_s + QS * nW;
@@ -192,14 +222,19 @@ k_rotate_v3(const Rot3Args a)
     }
 
     // ================= consumer warps =================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRot3RegsConsumer));
     const int g = lane >> 2, t = lane & 3;
-    const bool polar = a.pa.P != nullptr;
     const double nsU = (a.pa.conv & 1) ? -1.0 : 1.0;      // MINUS the sign Im U enters with (default: conjugated)
     const double nsZ = (a.pa.conv & 2) ? 1.0 : -1.0;      // MINUS the sign Im Z enters with (default: plain)
     const int nks = nwp >> 2;
+    int zrow[KS];                                        // Z row (times its pitch) of this lane in k-step s of a6
+#pragma unroll
+    for (int s = 0; s < KS; ++s) zrow[s] = rot3_kappa<KS>(s, t, mapB) * ldz + g;
     const int nmg = (MT + MTW - 1) / MTW;
-    const bool st2 = (nm & 1) == 0;                      // two consecutive outputs of a lane are one aligned 16-byte store
-    int sq = 0, sc = 0, prev_q = -1, prev_c = -1; uint32_t phq = 0, phc = 0;
+    const int so_b1 = nb2 * nm, so_mt = 8 * nm;          // strides of out in b1 and in tiles of b2
+    // two consecutive outputs of a lane are one aligned 16-byte store
+    const bool st2 = (nm & 1) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0;
+    int sq = 0, sc = 0; uint32_t phq = 0, phc = 0;
     for (int qg = blockIdx.x; qg < nqg; qg += gridDim.x) {
         const int q0 = qg * QS, nql = min(QS, a.nq - q0);
         mbar_wait(qfull + sq, phq);
@@ -232,6 +267,7 @@ k_rotate_v3(const Rot3Args a)
                     for (int j = 0; j < TJ; ++j) {
                         t1[mi][j][0] = t1[mi][j][1] = 0.0; t2[mi][j][0] = t2[mi][j][1] = 0.0; t3[mi][j][0] = t3[mi][j][1] = 0.0;
                     }
+                // running fragment pointers (one add per k-step each)
                 const double2* ua[MTW];
 #pragma unroll
                 for (int mi = 0; mi < MTW; ++mi)
@@ -244,33 +280,34 @@ k_rotate_v3(const Rot3Args a)
                     const int bl = p / KS, s = p - bl * KS;
                     cb[j] = pbase + (size_t)min(b1a + bl, nb1l - 1) * PB + rot3_kappa<KS>(s, g >> 1, mapB);
                 }
-                double2 an[MTW], bn[TJ];
-#pragma unroll
-                for (int mi = 0; mi < MTW; ++mi) an[mi] = ua[mi][0];
-#pragma unroll
-                for (int j = 0; j < TJ; ++j) bn[j] = cb[j][0];
                 // f4: the overlap O[b2][b1] = sum_w Uh[b2][w] Uk[w][b1] as one more column tile per two b1 (columns
                 // alternate between the two b1, so every lane ends up with O of both in its accumulator pair)
-                constexpr int TO = (GB + 1) / 2;
+                constexpr int TO = POLAR ? (GB + 1) / 2 : 1;
                 double o1[MTW][TO][2], o2[MTW][TO][2], o3[MTW][TO][2];
+                const double2* kb[TO];
+                if (POLAR) {
 #pragma unroll
-                for (int mi = 0; mi < MTW; ++mi)
+                    for (int mi = 0; mi < MTW; ++mi)
 #pragma unroll
-                    for (int jo = 0; jo < TO; ++jo) {
-                        o1[mi][jo][0] = o1[mi][jo][1] = 0.0; o2[mi][jo][0] = o2[mi][jo][1] = 0.0; o3[mi][jo][0] = o3[mi][jo][1] = 0.0;
-                    }
-                for (int ks = 0; ks < nks; ++ks) {
-                    double2 av[MTW], bv[TJ];
+                        for (int jo = 0; jo < TO; ++jo) {
+                            o1[mi][jo][0] = o1[mi][jo][1] = 0.0; o2[mi][jo][0] = o2[mi][jo][1] = 0.0; o3[mi][jo][0] = o3[mi][jo][1] = 0.0;
+                        }
+#pragma unroll
+                    for (int jo = 0; jo < TO; ++jo) kb[jo] = a.pa.Uk + min(b10 + b1a + 2 * jo + (g & 1), nb1 - 1);
+                }
+                // one k-step (4 values of w2): fragments (av, bv) are consumed, those of the next step land in (an, bn)
+                auto kstep = [&](const double2 (&av)[MTW], const double2 (&bv)[TJ], double2 (&an)[MTW], double2 (&bn)[TJ],
+                                 int ks, bool more) {
                     double as[MTW], bs[TJ];
 #pragma unroll
-                    for (int mi = 0; mi < MTW; ++mi) { av[mi] = an[mi]; as[mi] = fma(-nsU, av[mi].y, av[mi].x); }
+                    for (int mi = 0; mi < MTW; ++mi) as[mi] = fma(-nsU, av[mi].y, av[mi].x);
 #pragma unroll
-                    for (int j = 0; j < TJ; ++j) { bv[j] = bn[j]; bs[j] = bv[j].x + bv[j].y; }
-                    if (ks + 1 < nks) {
+                    for (int j = 0; j < TJ; ++j) bs[j] = bv[j].x + bv[j].y;
+                    if (more) {
 #pragma unroll
-                        for (int mi = 0; mi < MTW; ++mi) an[mi] = ua[mi][(size_t)(ks + 1) * 4 * ldu];
+                        for (int mi = 0; mi < MTW; ++mi) { ua[mi] += 4 * ldu; an[mi] = *ua[mi]; }
 #pragma unroll
-                        for (int j = 0; j < TJ; ++j) bn[j] = cb[j][(size_t)(ks + 1) * 4 * P];
+                        for (int j = 0; j < TJ; ++j) { cb[j] += 4 * P; bn[j] = *cb[j]; }
                     }
 #pragma unroll
                     for (int mi = 0; mi < MTW; ++mi)
@@ -280,11 +317,10 @@ k_rotate_v3(const Rot3Args a)
                             dmma884(t2[mi][j][0], t2[mi][j][1], av[mi].y, bv[j].y);
                             dmma884(t3[mi][j][0], t3[mi][j][1], as[mi], bs[j]);
                         }
-                    if (polar) {
+                    if (POLAR) {
 #pragma unroll
                         for (int jo = 0; jo < TO; ++jo) {
-                            const int b1o = min(b10 + b1a + 2 * jo + (g & 1), nb1 - 1);
-                            const double2 kv = a.pa.Uk[(size_t)min(4 * ks + t, nw - 1) * nb1 + b1o];
+                            const double2 kv = kb[jo][(size_t)min(4 * ks + t, nw - 1) * nb1];
                             const double ksum = kv.x + kv.y;
 #pragma unroll
                             for (int mi = 0; mi < MTW; ++mi) {
@@ -293,6 +329,17 @@ k_rotate_v3(const Rot3Args a)
                                 dmma884(o3[mi][jo][0], o3[mi][jo][1], as[mi], ksum);
                             }
                         }
+                    }
+                };
+                {
+                    double2 fa0[MTW], fb0[TJ], fa1[MTW], fb1[TJ];      // two fragment sets used alternately: no register moves
+#pragma unroll
+                    for (int mi = 0; mi < MTW; ++mi) fa0[mi] = *ua[mi];
+#pragma unroll
+                    for (int j = 0; j < TJ; ++j) fb0[j] = *cb[j];
+                    for (int ks = 0; ks < nks; ks += 2) {
+                        kstep(fa0, fb0, fa1, fb1, ks, ks + 1 < nks);
+                        if (ks + 1 < nks) kstep(fa1, fb1, fa0, fb0, ks + 1, ks + 2 < nks);
                     }
                 }
                 // D = (T1 -+ T2) + i (T3 - T1 -+ T2); kept as (Re, Im, Re + Im): the three A planes of a6
@@ -306,7 +353,7 @@ k_rotate_v3(const Rot3Args a)
                             const double re = fma(nsU, x2, x1), im = fma(nsU, x2, x3 - x1);
                             t1[mi][j][h] = re; t2[mi][j][h] = im; t3[mi][j][h] = re + im;
                         }
-                if (polar) {
+                if (POLAR) {
 #pragma unroll
                     for (int mi = 0; mi < MTW; ++mi)
 #pragma unroll
@@ -318,12 +365,22 @@ k_rotate_v3(const Rot3Args a)
                             }
                 }
                 // ---- a6 + a7 ----
-                const double2* zq = Zs + (size_t)ql * 4 * KS * ldz + g;
+                const double2* zq = Zs + (size_t)ql * 4 * KS * ldz;
                 const double* iw = iwq + ql * 8 * NT;
                 const int qabs = q0 + ql;
-                double racc[GB];
+                double racc[GB], e1k[GB];
+                bool okb[GB], okm[MTW];
 #pragma unroll
-                for (int bl = 0; bl < GB; ++bl) racc[bl] = 0.0;
+                for (int bl = 0; bl < GB; ++bl) {
+                    racc[bl] = 0.0;
+                    okb[bl] = b1a + bl < nb1l;
+                    e1k[bl] = rates ? a.ra.eps_k[(a.ra.rows_per_k > 0 ? (qabs / a.ra.rows_per_k) * nb1 : 0) +
+                                                 min(b10 + b1a + bl, nb1 - 1)] : 0.0;
+                }
+#pragma unroll
+                for (int mi = 0; mi < MTW; ++mi) okm[mi] = mt0 + mi < MT && (mt0 + mi) * 8 + g < nb2;
+                // out[q][b1][b2][nu] of this lane's first value; + bl * so_b1 + mi * so_mt + 8 n for the others
+                double* obase = a.out + (((size_t)qabs * nb1 + b10 + b1a) * nb2 + (size_t)mt0 * 8 + g) * nm + 2 * t;
 #pragma unroll 1
                 for (int n = 0; n < NT; ++n) {
                     double e1[GB][MTW][2], e2[GB][MTW][2], e3[GB][MTW][2];
@@ -335,7 +392,7 @@ k_rotate_v3(const Rot3Args a)
                         }
 #pragma unroll
                     for (int s = 0; s < KS; ++s) {
-                        const double2 z = zq[(size_t)rot3_kappa<KS>(s, t, mapB) * ldz + 8 * n];
+                        const double2 z = zq[zrow[s] + 8 * n];
                         const double zs = fma(-nsZ, z.y, z.x);
 #pragma unroll
                         for (int bl = 0; bl < GB; ++bl) {
@@ -348,29 +405,27 @@ k_rotate_v3(const Rot3Args a)
                             }
                         }
                     }
+                    // branch-free: every lane computes its two values, only the stores are predicated
                     const int nu = 8 * n + 2 * t;
                     const double2 iw2 = *reinterpret_cast<const double2*>(iw + nu);      // 1/(2 omega) of this lane's two columns
-                    const bool okh[2] = {nu < nm, nu + 1 < nm};
+                    const bool ok0 = nu < nm, ok1 = nu + 1 < nm;
                     double2 pz[2] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
-                    if (polar) {
-                        if (okh[0]) pz[0] = a.pa.P[(size_t)qabs * nm + nu];
-                        if (okh[1]) pz[1] = a.pa.P[(size_t)qabs * nm + nu + 1];
+                    if (POLAR) {
+                        if (ok0) pz[0] = a.pa.P[(size_t)qabs * nm + nu];
+                        if (ok1) pz[1] = a.pa.P[(size_t)qabs * nm + nu + 1];
                     }
 #pragma unroll
                     for (int bl = 0; bl < GB; ++bl) {
-                        if (b1a + bl >= nb1l) continue;
-                        const int b1 = b10 + b1a + bl;
 #pragma unroll
                         for (int mi = 0; mi < MTW; ++mi) {
-                            const int b2 = (mt0 + mi) * 8 + g;
-                            if (mt0 + mi >= MT || b2 >= nb2) continue;
+                            const bool okr = okb[bl] && okm[mi];            // this lane's (b1, b2) exists
                             double er[2], ei[2];
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
                                 er[h] = fma(nsZ, e2[bl][mi][h], e1[bl][mi][h]);
                                 ei[h] = fma(nsZ, e2[bl][mi][h], e3[bl][mi][h] - e1[bl][mi][h]);
                             }
-                            if (polar) {
+                            if (POLAR) {
                                 const double ox = o1[mi][bl >> 1][bl & 1], oy = o2[mi][bl >> 1][bl & 1];
 #pragma unroll
                                 for (int h = 0; h < 2; ++h) {
@@ -380,29 +435,31 @@ k_rotate_v3(const Rot3Args a)
                             }
                             const double v0 = (er[0] * er[0] + ei[0] * ei[0]) * iw2.x;
                             const double v1 = (er[1] * er[1] + ei[1] * ei[1]) * iw2.y;
-                            if (!RATES || a.out != nullptr) {
-                                double* orow = a.out + (((size_t)qabs * nb1 + b1) * nb2 + b2) * nm + nu;
-                                if (st2 && okh[1]) *reinterpret_cast<double2*>(orow) = make_double2(v0, v1);
-                                else { if (okh[0]) orow[0] = v0; if (okh[1]) orow[1] = v1; }
+                            if (!RSM || a.out != nullptr) {
+                                double* orow = obase + (size_t)bl * so_b1 + (size_t)mi * so_mt + 8 * n;
+                                if (st2) { if (okr && ok1) *reinterpret_cast<double2*>(orow) = make_double2(v0, v1); }
+                                else { if (okr && ok0) orow[0] = v0; if (okr && ok1) orow[1] = v1; }
+                                if (st2 && okr && ok0 && !ok1) orow[0] = v0;
                             }
-                            if (RATES) {
-                                const double x12 = a.ra.eps_k[(a.ra.rows_per_k > 0 ? (qabs / a.ra.rows_per_k) * nb1 : 0) + b1] -
-                                                   e2_s[ql * 8 * MT + b2];
-                                const double f2 = f2_s[ql * 8 * MT + b2];
+                            if (rates) {
+                                const int b2c = min((mt0 + mi) * 8 + g, 8 * MT - 1);
+                                const double x12 = e1k[bl] - e2_s[ql * 8 * MT + b2c];
+                                const double f2 = f2_s[ql * 8 * MT + b2c];
 #pragma unroll
                                 for (int h = 0; h < 2; ++h) {
-                                    if (!okh[h]) continue;
                                     const double w = om_s[ql * 8 * NT + nu + h], bn_ = bose_s[ql * 8 * NT + nu + h];
                                     const double dm = x12 - w, dp = x12 + w;
                                     const double W = (1.0 - f2 + bn_) * exp(-(dm * dm) * a.ra.inv_sigma2) +
                                                      (f2 + bn_) * exp(-(dp * dp) * a.ra.inv_sigma2);
-                                    racc[bl] = fma(h ? v1 : v0, W, racc[bl]);
+                                    // padded rows / columns: omega = 0 there gives v = 0 exactly (1/(2 omega) := 0), rows
+                                    // b2 >= nb2 are masked
+                                    racc[bl] = fma((okr && (h ? ok1 : ok0)) ? (h ? v1 : v0) : 0.0, W, racc[bl]);
                                 }
                             }
                         }
                     }
                 }
-                if (RATES) {        // fixed-order sum over the warp: partial[q][mg][b1] is owned by this item
+                if (rates) {        // fixed-order sum over the warp: partial[q][mg][b1] is owned by this item
 #pragma unroll
                     for (int bl = 0; bl < GB; ++bl) {
                         double rsum = racc[bl];
@@ -413,15 +470,17 @@ k_rotate_v3(const Rot3Args a)
                     }
                 }
             }
-            // release the PREVIOUS stage of each ring (one stage late, see k_contract)
+            // Release the stage.  Every shared-memory load of an item has been consumed by the time its last store
+            // issues (the stores depend on all of its DMMAs, those on all of its fragment loads); the fence keeps the
+            // arrive behind those stores and orders every lane's reads before lane 0's release.
+            __threadfence_block();
             __syncwarp();
-            if (lane == 0 && prev_c >= 0) mbar_arrive(cempty + prev_c);
-            prev_c = sc;
+            if (lane == 0) mbar_arrive(cempty + sc);
             if (++sc == NS) { sc = 0; phc ^= 1u; }
         }
+        __threadfence_block();
         __syncwarp();
-        if (lane == 0 && prev_q >= 0) mbar_arrive(qempty + prev_q);
-        prev_q = sq;
+        if (lane == 0) mbar_arrive(qempty + sq);
         if (++sq == NS) { sq = 0; phq ^= 1u; }
     }
 }

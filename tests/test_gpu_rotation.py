@@ -72,7 +72,8 @@ def test_rotation_matches_oracle_and_plain_kernel(env, case):
     assert _relerr(out2, out1) <= TOL
 
 
-@pytest.mark.parametrize("knob", [{"rot_qg": 1}, {"rot_qg": 3}, {"rot_gb1": 2}, {"rot_gb1": 1}, {"rot_mtw": 1}],
+@pytest.mark.parametrize("knob", [{"rot_qg": 1}, {"rot_qg": 3}, {"rot_gb1": 2}, {"rot_gb1": 1}, {"rot_mtw": 1},
+                                  {"rot_blk": 1}, {"rot_blk": 2}, {"rot_blk": 2, "rot_gb1": 2}, {"rot_blk": 2, "rot_qg": 3}],
                          ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
 def test_rotation_forced_stage_geometry(env, knob):
     """q-points per stage, b1 per C stage (the two-ring form on a small problem) and m-tiles per item forced."""
