@@ -474,7 +474,7 @@ bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_
         // whole q-points per stage: enough of them that every consumer warp has an item, while the q list still
         // gives every SM several stages
         const int per_q = ceil_div(nb1, G->GB) * G->nmg;
-        int QS = ceil_div(pe::kRot3Consumers, per_q);
+        int QS = ceil_div(pe::rot3_consumers(G->MTW), per_q);
         if (qs_over > 0) QS = qs_over;
         QS = std::min(QS, qs_cap);
         while (QS > 1 && (total(QS, nb1) > kRot3SmemBudget || ceil_div(nq, QS) < 2 * kSMs)) --QS;
@@ -490,7 +490,7 @@ bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_
             gb1 = 1;
         }
         // no larger than gives every consumer warp one item (smaller stages: deeper prefetch for the same memory)
-        const int want = std::max(G->GB, ceil_div(pe::kRot3Consumers, G->nmg) * G->GB);
+        const int want = std::max(G->GB, ceil_div(pe::rot3_consumers(G->MTW), G->nmg) * G->GB);
         gb1 = std::min(gb1, std::max(want, G->GB));
         if (gb1_over > 0) gb1 = std::min(gb1_over, nb1);
         G->QS = 1; G->gb1 = std::min(gb1, nb1);
@@ -515,14 +515,14 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     const bool fused_rates = rr != nullptr && use_mma;
     const bool polar = c->nG > 0;
     Rot3Geom G{};
-    int gb1 = nb1, rot_threads = pe::kRot3Threads;
+    int gb1 = nb1, rot_threads = 0;
     size_t rot_smem = 0;
     int P = d.nmodes, PB = d.nw * d.nmodes;                 // C layout (plain for the DFMA kernel)
     if (use_mma) {
         // the polar kernels (mode 3) always carry the Eq. 29 arrays in their stages
         if (!rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), fused_rates || polar, c->rot_qg, c->rot_gb1, c->rot_mtw, c->rot_blk, &G))
             return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
-        P = G.P; PB = G.PB; gb1 = G.gb1; rot_smem = G.smem;
+        P = G.P; PB = G.PB; gb1 = G.gb1; rot_smem = G.smem; rot_threads = pe::rot3_threads(G.MTW);
     } else {
         const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;
         const size_t per_b1 = ((size_t)Y + (size_t)nb2 * d.nmodes) * 16;

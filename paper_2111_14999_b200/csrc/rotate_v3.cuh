@@ -28,11 +28,13 @@
 
 namespace pe {
 
-constexpr int kRot3Consumers = 8;
-// three warpgroups: two of consumer warps, one that holds the producer warp (its other three warps exit at once).
-// The register file is re-split between them at kernel start (setmaxnreg): 12 warps x 168 = 8 x 232 + 4 x 40.
-constexpr int kRot3Threads = (kRot3Consumers + 4) * 32;
-constexpr int kRot3RegsConsumer = 232, kRot3RegsProducer = 40;
+// Warpgroups of consumer warps plus one that holds the producer warp (its other three warps exit at once); the
+// register file is re-split between them at kernel start (setmaxnreg).  Items with two tiles of b2 (MTW = 2) need
+// ~230 registers: 8 consumer warps (8 x 232 + 4 x 40 = 12 x 168); items with one tile fit 160: 12 consumer warps
+// (12 x 160 + 4 x 32 = 16 x 128), three per scheduler -- more warps to overlap one item's DMMA phases with another's
+// operand sums / epilogue.
+__host__ __device__ constexpr int rot3_consumers(int MTW) { return MTW == 2 ? 8 : 12; }
+__host__ __device__ constexpr int rot3_threads(int MTW) { return (rot3_consumers(MTW) + 4) * 32; }
 constexpr int kRot3Stages = 3;
 
 struct Rot3Layout {
@@ -93,9 +95,11 @@ __device__ __forceinline__ int rot3_kappa(int s, int tt, int mapB)
 // MODE: 0 = |g|^2 only, 1 = with the linewidth sums of Eq. 29 (f2), 3 = with the polar term of Eq. 14-15 (f4; the
 // linewidth sums are then a run-time choice: a.ra.eps_k != nullptr)
 template <int KS, int GB, int MTW, int MODE>
-__global__ void __launch_bounds__(kRot3Threads, 1)
+__global__ void __launch_bounds__(rot3_threads(MTW), 1)
 k_rotate_v3(const Rot3Args a)
 {
+    constexpr int NCW = rot3_consumers(MTW), NTHREADS = rot3_threads(MTW);
+    constexpr int REGS_C = MTW == 2 ? 232 : 160, REGS_P = MTW == 2 ? 40 : 32;
     constexpr bool RSM = (MODE & 1) != 0;                 // the Eq. 29 arrays exist in the Q stages
     constexpr bool POLAR = (MODE & 2) != 0;
     const bool rates = RSM && (MODE != 3 || a.ra.eps_k != nullptr);
@@ -116,12 +120,16 @@ k_rotate_v3(const Rot3Args a)
 
     // the rings are zeroed ONCE: the bulk copies only ever write the real rows / columns, so the padding the fragment
     // loads touch (U rows >= nw, Z rows >= nm, row tails, the slack behind the panels) stays zero for the whole kernel
-    for (uint32_t i = L.off_Q / 16 + threadIdx.x; i < L.total / 16; i += kRot3Threads)
+    for (uint32_t i = L.off_Q / 16 + threadIdx.x; i < L.total / 16; i += NTHREADS)
         reinterpret_cast<double2*>(smem_raw)[i] = make_double2(0.0, 0.0);
+    // Warp w takes the items w, w + NCW, ... of the CTA's whole item SEQUENCE (not of each stage), so a stage with
+    // fewer items than warps does not leave the same warps idle every time, and the warps drift apart across the
+    // stages of the ring instead of marching through them in step.  Every warp observes every stage (waits for its
+    // full barrier, arrives on its empty barrier) in order, with or without items in it: barrier phases stay in step.
     if (threadIdx.x == 0) {
         for (int s = 0; s < NS; ++s) {
-            mbar_init(qfull + s, 1); mbar_init(qempty + s, kRot3Consumers);
-            mbar_init(cfull + s, 1); mbar_init(cempty + s, kRot3Consumers);
+            mbar_init(qfull + s, 1); mbar_init(qempty + s, NCW);
+            mbar_init(cfull + s, 1); mbar_init(cempty + s, NCW);
         }
         mbar_fence_init();
     }
@@ -131,9 +139,9 @@ k_rotate_v3(const Rot3Args a)
     const int nqg = (a.nq + QS - 1) / QS;
     const long long ldcq = (long long)nb1 * PB;
 
-    if (warp >= kRot3Consumers) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRot3RegsProducer));
-        if (warp > kRot3Consumers) return;
+    if (warp >= NCW) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_P));
+        if (warp > NCW) return;
         // ================= producer warp =================
         int sq = 0, sc = 0; uint32_t phq = 0, phc = 0;
         const int nW = 8 * NT, nE = 8 * MT;
@@ -222,7 +230,7 @@ k_rotate_v3(const Rot3Args a)
     }
 
     // ================= consumer warps =================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRot3RegsConsumer));
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_C));
     const int g = lane >> 2, t = lane & 3;
     const double nsU = (a.pa.conv & 1) ? -1.0 : 1.0;      // MINUS the sign Im U enters with (default: conjugated)
     const double nsZ = (a.pa.conv & 2) ? 1.0 : -1.0;      // MINUS the sign Im Z enters with (default: plain)
@@ -234,10 +242,12 @@ k_rotate_v3(const Rot3Args a)
     const int so_b1 = nb2 * nm, so_mt = 8 * nm;          // strides of out in b1 and in tiles of b2
     // two consecutive outputs of a lane are one aligned 16-byte store
     const bool st2 = (nm & 1) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0;
-    int sq = 0, sc = 0; uint32_t phq = 0, phc = 0;
-    for (int qg = blockIdx.x; qg < nqg; qg += gridDim.x) {
+    int Sq = 0, Sc = 0;              // stages of the two rings consumed so far (slot = S % NS, phase = (S / NS) & 1)
+    int rem = 0;                     // (items of all earlier stages) % NCW
+    for (int qg = blockIdx.x; qg < nqg; qg += gridDim.x, ++Sq) {
         const int q0 = qg * QS, nql = min(QS, a.nq - q0);
-        mbar_wait(qfull + sq, phq);
+        const int sq = Sq % NS;
+        mbar_wait(qfull + sq, (uint32_t)(Sq / NS) & 1u);
         const unsigned char* Q = smem_raw + L.off_Q + (size_t)sq * L.szQ;
         const double2* Us = reinterpret_cast<const double2*>(Q);
         const double2* Zs = reinterpret_cast<const double2*>(Q + L.szU);
@@ -246,14 +256,18 @@ k_rotate_v3(const Rot3Args a)
         const double* bose_s = om_s + QS * 8 * NT;
         const double* e2_s = bose_s + QS * 8 * NT;
         const double* f2_s = e2_s + QS * 8 * MT;
-        for (int grp = 0; grp < ngroups; ++grp) {
-            mbar_wait(cfull + sc, phc);
+        for (int grp = 0; grp < ngroups; ++grp, ++Sc) {
+            const int sc = Sc % NS;
             const double2* Cs = reinterpret_cast<const double2*>(smem_raw + L.off_C + (size_t)sc * L.szC);
             const int b10 = grp * gb1;
             const int nb1l = min(gb1, nb1 - b10);
             const int nbg = (nb1l + GB - 1) / GB;
             const int per_q = nbg * nmg;
-            for (int item = warp; item < nql * per_q; item += kRot3Consumers) {
+            const int ni = nql * per_q;
+            int item = warp - rem; if (item < 0) item += NCW;           // this warp's first item of the stage
+            rem = (rem + ni) % NCW;
+            mbar_wait(cfull + sc, (uint32_t)(Sc / NS) & 1u);
+            for (; item < ni; item += NCW) {
                 int ql = 0, r = item;
                 if (per_q > 1) { ql = item / per_q; r = item - ql * per_q; } else { ql = item; r = 0; }
                 int bg = r, mg = 0;
@@ -470,18 +484,16 @@ k_rotate_v3(const Rot3Args a)
                     }
                 }
             }
-            // Release the stage.  Every shared-memory load of an item has been consumed by the time its last store
+            // Release the stage: every shared-memory load of an item has been consumed by the time its last store
             // issues (the stores depend on all of its DMMAs, those on all of its fragment loads); the fence keeps the
             // arrive behind those stores and orders every lane's reads before lane 0's release.
             __threadfence_block();
             __syncwarp();
             if (lane == 0) mbar_arrive(cempty + sc);
-            if (++sc == NS) { sc = 0; phc ^= 1u; }
         }
         __threadfence_block();
         __syncwarp();
         if (lane == 0) mbar_arrive(qempty + sq);
-        if (++sq == NS) { sq = 0; phq ^= 1u; }
     }
 }
 
