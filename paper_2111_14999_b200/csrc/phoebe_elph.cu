@@ -453,7 +453,10 @@ bool rot3_geometry(int nw, int nm, int nb1, int nb2, int nq, bool rates, int qs_
 {
     const int KS = ceil_div(nm, 4), NT = ceil_div(nm, 8), MT = ceil_div(nb2, 8);
     G->KS = KS;
-    G->MTW = (mtw_over > 0) ? ((mtw_over >= 2 && MT >= 2) ? 2 : 1) : (MT >= 2 ? 2 : 1);
+    // two tiles of b2 per item (8 consumer warps with ~230 registers) when an item has many a5 column tiles to share
+    // each A fragment over (KS >= 5: the large cell 7.28 vs 7.78 ms per launch); else one tile and 12 consumer warps
+    // (the 4-atom cell: 3.27 vs 3.57 ms)
+    G->MTW = (mtw_over > 0) ? ((mtw_over >= 2 && MT >= 2) ? 2 : 1) : ((MT >= 2 && KS >= 5) ? 2 : 1);
     G->GB = nb1 >= rot3_max_gb(KS, G->MTW) ? rot3_max_gb(KS, G->MTW) : rot3_min_gb(KS);
     G->nmg = ceil_div(MT, G->MTW);
     G->P = pe::rot3_row_pitch(nm);

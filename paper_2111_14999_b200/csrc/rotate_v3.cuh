@@ -240,6 +240,16 @@ k_rotate_v3(const Rot3Args a)
     for (int s = 0; s < KS; ++s) zrow[s] = rot3_kappa<KS>(s, t, mapB) * ldz + g;
     const int nmg = (MT + MTW - 1) / MTW;
     const int so_b1 = nb2 * nm, so_mt = 8 * nm;          // strides of out in b1 and in tiles of b2
+    // this lane's B column of a5 tile j: which b1 of the item (cbl) and where in the C panel (cof, without the b1 term)
+    int cbl[TJ], cof[TJ];
+#pragma unroll
+    for (int j = 0; j < TJ; ++j) {
+        const int p = min(2 * j + (g & 1), GB * KS - 1);        // pair of the column (clamped: unused half tile)
+        const int bl = p / KS, sp = p - bl * KS;
+        cbl[j] = bl;
+        cof[j] = t * P + rot3_kappa<KS>(sp, g >> 1, mapB);
+    }
+    const int uof = t * ldu + g;                         // A fragment of a5: row t of a k-step, column g of a tile of b2
     // two consecutive outputs of a lane are one aligned 16-byte store
     const bool st2 = (nm & 1) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0;
     int Sq = 0, Sc = 0;              // stages of the two rings consumed so far (slot = S % NS, phase = (S / NS) & 1)
@@ -269,9 +279,9 @@ k_rotate_v3(const Rot3Args a)
             mbar_wait(cfull + sc, (uint32_t)(Sc / NS) & 1u);
             for (; item < ni; item += NCW) {
                 int ql = 0, r = item;
-                if (per_q > 1) { ql = item / per_q; r = item - ql * per_q; } else { ql = item; r = 0; }
+                if (nql > 1) { ql = (int)((unsigned)item / (unsigned)per_q); r = item - ql * per_q; }
                 int bg = r, mg = 0;
-                if (nmg > 1) { bg = r / nmg; mg = r - bg * nmg; }
+                if (nmg > 1) { bg = (int)((unsigned)r / (unsigned)nmg); mg = r - bg * nmg; }
                 const int b1a = bg * GB, mt0 = mg * MTW;
                 // ---- a5: T1, T2, T3 of D[b2][(b1,ka)] ----
                 double t1[MTW][TJ][2], t2[MTW][TJ][2], t3[MTW][TJ][2];
@@ -285,15 +295,11 @@ k_rotate_v3(const Rot3Args a)
                 const double2* ua[MTW];
 #pragma unroll
                 for (int mi = 0; mi < MTW; ++mi)
-                    ua[mi] = Us + ((size_t)ql * nwp + t) * ldu + min(mt0 + mi, MT - 1) * 8 + g;
-                const double2* pbase = Cs + (size_t)ql * (gb1 * PB) + (size_t)t * P;
+                    ua[mi] = Us + ql * (nwp * ldu) + uof + min(mt0 + mi, MT - 1) * 8;
+                const double2* pbase = Cs + ql * (gb1 * PB);
                 const double2* cb[TJ];
 #pragma unroll
-                for (int j = 0; j < TJ; ++j) {
-                    const int p = min(2 * j + (g & 1), GB * KS - 1);        // pair of this lane's B column (clamped: unused half tile)
-                    const int bl = p / KS, s = p - bl * KS;
-                    cb[j] = pbase + (size_t)min(b1a + bl, nb1l - 1) * PB + rot3_kappa<KS>(s, g >> 1, mapB);
-                }
+                for (int j = 0; j < TJ; ++j) cb[j] = pbase + min(b1a + cbl[j], nb1l - 1) * PB + cof[j];
                 // f4: the overlap O[b2][b1] = sum_w Uh[b2][w] Uk[w][b1] as one more column tile per two b1 (columns
                 // alternate between the two b1, so every lane ends up with O of both in its accumulator pair)
                 constexpr int TO = POLAR ? (GB + 1) / 2 : 1;
