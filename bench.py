@@ -111,7 +111,8 @@ class ClockSampler:
         return out
 
 
-from paper_2111_14999_b200.sharding import dist_env as _dist_env, max_over_ranks, shard_k  # noqa: E402
+from paper_2111_14999_b200.sharding import (allreduce_g1, dist_env as _dist_env, max_over_ranks, pool_set_k,  # noqa: E402
+                                            pool_set_k_batch, shard_k, shard_range)
 
 
 def _k_inputs(w, ik):
@@ -125,40 +126,45 @@ def _k_inputs(w, ik):
 
 # ----------------------------------------------------------------------------- CPU oracle legs
 def time_oracle(w, budget_s: float = 20.0):
-    """The oracle as it stands, timed on the host cores on a bounded sample of workload w.
-    Returns (pairs_per_s, cores, sample_description).  set_k is timed on a subset of the Rp slabs and
-    scaled by nRp/slabs (it is a plain sum over independent slabs); q_batch is timed on a subset of the
-    q list against a g1' of the right shape, and scaled by nq/sample."""
+    """The oracle as it stands, timed on the host cores on a bounded sample of workload w (SURVEY 8(d) "Oracle timed
+    beside it": every k-point of the workload x min(256, nq) of its q-points; set_k on as many Rp slabs of g_W as the
+    budget allows).  Returns (pairs_per_s, cores, sample_description, (t_setk, t_q)) for the WHOLE workload:
+    set_k is a plain sum over independent slabs and is scaled by nRp/slabs, q_batch is linear in nq and is scaled by
+    nq/sample -- the value is an EXTRAPOLATION from the sample, and says so."""
     import oracle
     cores = oracle.num_threads()
     Re, Rp = wl.Re_vectors(w), wl.Rp_vectors(w)
-    k, Uk = wl.k_points(w)[0], wl.U_k(w, 0)
-    slab_flop = 8.0 * w.nRe * w.X
+    ks = wl.k_points(w)
+    nk_s = min(w.nk, 16)                                   # k-points actually run (band-window: 16 of its 256)
+    slab_flop = 8.0 * w.nRe * w.X * nk_s
     # assume >= 0.3 GFLOP/s/core for sizing; the measured time is what is reported
-    n_slab = int(max(cores, min(w.nRp, (0.3 * budget_s * 0.3e9 * cores) / slab_flop)))
+    n_slab = int(max(1, min(w.nRp, (0.4 * budget_s * 0.3e9 * cores) / slab_flop)))
     n_slab = max(1, min(w.nRp, n_slab, int(2e9 // (16 * w.nRe * w.X))))      # <= 2 GB of g_W on the host
     slabs = np.empty((n_slab, w.nRe, w.nw, w.nw, w.nm), dtype=np.complex128)
     import concurrent.futures as cf
     with cf.ThreadPoolExecutor(min(16, os.cpu_count() or 4)) as pool:
         list(pool.map(lambda p: wl.gW_slab(w, p, slabs[p]), range(n_slab)))
     t0 = time.perf_counter()
-    g1_part = oracle.setk(slabs, Re, None, k, Uk)
-    t_setk = (time.perf_counter() - t0) * (w.nRp / n_slab)
+    g1_part = None
+    for ik in range(nk_s):
+        g1_part = oracle.setk(slabs, Re, None, ks[ik], wl.U_k(w, ik))
+    t_setk = (time.perf_counter() - t0) * (w.nRp / n_slab) * (w.nk / nk_s)
     # q part: g1' of the right shape (values are irrelevant for timing): tile what set_k produced
     reps = -(-w.nRp // n_slab)
     g1 = np.ascontiguousarray(np.concatenate([g1_part] * reps)[: w.nRp])
-    q_flop = 8.0 * w.nRp * w.N + 8.0 * w.nb1 * w.nb2 * w.nm * (w.nw + w.nm)
-    nq_s = int(max(cores, min(w.nq, (0.7 * budget_s * 0.4e9 * cores) / q_flop)))
-    nq_s = min(w.nq, nq_s)
-    q, Ukq, ev, om = wl.q_inputs(w, 0)
-    idx = wl.sample_indices(w.nq, nq_s)
-    qa, Ua, ea, oa = q[idx], np.ascontiguousarray(Ukq[idx]), np.ascontiguousarray(ev[idx]), om[idx]
-    t0 = time.perf_counter()
-    oracle.qbatch(g1, Rp, None, qa, Ua, ea, oa)
-    t_q = (time.perf_counter() - t0) * (w.nq / nq_s)
-    pairs_per_s = w.nq / (t_setk + t_q)
-    sample = (f"1 k-point of {w.nk}: set_k on {n_slab}/{w.nRp} Rp slabs (scaled x{w.nRp / n_slab:.2f}), "
-              f"q_batch on {nq_s}/{w.nq} q (scaled x{w.nq / nq_s:.2f}); gcc -O2 -fopenmp, {cores} threads")
+    nq_s = min(w.nq, 256)
+    ws = w.with_(nq=nq_s)                                  # same recipe and distributions, nq_s q-points per k
+    t_q = 0.0
+    for ik in range(nk_s):
+        qa, Ua, ea, oa = wl.q_inputs(ws, ik)
+        t0 = time.perf_counter()
+        oracle.qbatch(g1, Rp, None, qa, Ua, ea, oa)
+        t_q += time.perf_counter() - t0
+    t_q *= (w.nq / nq_s) * (w.nk / nk_s)
+    pairs_per_s = w.nk * w.nq / (t_setk + t_q)
+    sample = (f"{nk_s} of {w.nk} k-points: set_k on {n_slab}/{w.nRp} Rp slabs (scaled x{w.nRp / n_slab:.2f}), "
+              f"q_batch on {nq_s}/{w.nq} q per k (scaled x{w.nq / nq_s:.2f}); EXTRAPOLATED to the whole workload; "
+              f"gcc -O2 -fopenmp, {cores} threads")
     return pairs_per_s, cores, sample, (t_setk, t_q)
 
 
@@ -170,7 +176,7 @@ def run_reference(args):
     vals = []
     sample = ""
     cores = 0
-    budget = max(2.0, min(20.0, 90.0 / max(1, args.steps + args.warmup)))
+    budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for i in range(args.warmup + args.steps):
         v, cores, sample, _ = time_oracle(w, budget)
         if i >= args.warmup:
@@ -178,22 +184,52 @@ def run_reference(args):
     value = float(np.mean(vals))
     ms_per_step = 1e3 * (w.nk * w.nq) / value
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "extrapolated": True, "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": _config_dict(w, args.gpus),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "config": _config_dict(w, world),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "extrapolated": True},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
 
 
-def _config_dict(w, n_gpus):
+def _config_dict(w, n_gpus, scaling="weak", pool=1):
+    if pool > 1:
+        par = (f"{max(1, n_gpus // pool)} Re-pools of {pool} ranks: g_W sharded over Re inside a pool, one NCCL all-reduce of g1' per "
+               f"set_k_batch, q lists shared out inside the pool, k-points {scaling}-sharded over the pools")
+    else:
+        par = f"k-sharded x{n_gpus} ({scaling}), g_W replicated, no collective"
     return {"workload": w.name, "nw": w.nw, "nb1": w.nb1, "nb2": w.nb2, "nmodes": w.nm, "nRe": w.nRe, "nRp": w.nRp,
             "nk": w.nk, "nq_per_k": w.nq, "gW_GB": round(w.gW_bytes / 1e9, 3),
             "cache": "inputs larger than L2 (g_W is streamed from HBM every step)",
-            "parallelism": f"k-sharded x{n_gpus}, g_W replicated, no collective"}
+            "parallelism": par}
+
+
+def cublas_ceilings(torch, dev, M, N, K):
+    """cuBLAS FP64 GEMM throughput at the contraction's shape [M x K].[K x N] (through torch.matmul), as CEILINGS for
+    the roofline: DGEMM in real flops (2 M N K), ZGEMM in the four-multiply convention (8 M N K)."""
+    out = {}
+    for name, dt, fl in (("cublas_dgemm_tflops", torch.float64, 2.0), ("cublas_zgemm_8flop_tflops", torch.complex128, 8.0)):
+        a = torch.randn((M, K), dtype=dt, device=dev)
+        b = torch.randn((K, N), dtype=dt, device=dev)
+        c = torch.empty((M, N), dtype=dt, device=dev)
+        for _ in range(2):
+            torch.matmul(a, b, out=c)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = 1e30
+        for _ in range(4):
+            e0.record()
+            torch.matmul(a, b, out=c)
+            e1.record()
+            e1.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        out[name] = fl * M * N * K / (best * 1e-3) / 1e12
+        del a, b, c
+    out["cublas_shape"] = [M, N, K]
+    return out
 
 
 def _with_kbatch(cfg, kb):
@@ -208,6 +244,76 @@ def _with_multi(cfg, multi):
     return cfg
 
 
+# ----------------------------------------------------------------------------- N ranks on one node
+def _free_port():
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        return so.getsockname()[1]
+
+
+def spawn_ranks(args, argv):
+    """`python bench.py --gpus N` started WITHOUT torchrun: re-exec under torch.distributed.run with one process per
+    GPU (the launch line the driver itself uses), relay its output, return its exit code."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")         # the communicator line ("... nranks N ...") shows every rank joined
+    env.setdefault("OMP_NUM_THREADS", "4")
+    return subprocess.call(cmd, env=env)
+
+
+def rank_plan(w, rank, world, scaling, pool):
+    """What one rank does (no arithmetic of the method): its pool, its k-points, its slice of the Re list (Re-pool,
+    PAPER.md L576) and of every q list.  pool = P > 1: ranks [j*P, (j+1)*P) form pool j; the pools share out the
+    k-points (weak: nk per pool; strong: the workload's nk dealt over the pools), the ranks of a pool share out Re for
+    step 1 (one all-reduce of g1') and the q list for step 2."""
+    assert pool >= 1 and world % pool == 0, "--pool must divide the number of ranks"
+    npools, ipool, prank = world // pool, rank // pool, rank % pool
+    k_ids = shard_k(w.nk, ipool, npools, scaling)
+    re_lo, re_hi = shard_range(w.nRe, prank, pool)
+    # q slices in multiples of 64 rows (the contraction's row tile), the last rank takes the ragged rest
+    per = -(-w.nq // pool)
+    per = -(-per // 64) * 64
+    q_lo, q_hi = min(w.nq, prank * per), min(w.nq, (prank + 1) * per)
+    return dict(rank=rank, pool=ipool, pool_rank=prank, pool_size=pool, k_ids=k_ids, re=(re_lo, re_hi), q=(q_lo, q_hi),
+                pairs=len(k_ids) * (q_hi - q_lo))
+
+
+def run_dry(args):
+    """--dry-run: the N-rank plumbing without a GPU (the world-2 gloo test drives the spawn path through this): process
+    group, pool sub-groups, the plan of every rank, one all-reduce over the pool through the same helper the Re-pool
+    uses, barrier + max-over-ranks of a per-rank time.  No CUDA, no kernels, no oracle."""
+    import torch
+    import torch.distributed as dist
+    rank, world, local = _dist_env()
+    if world > 1:
+        dist.init_process_group(args.backend if args.backend != "nccl" else "gloo")
+    w = wl.CONFIGS[args.workload]
+    plan = rank_plan(w, rank, world, args.scaling, args.pool)
+    group = None
+    if world > 1 and args.pool > 1:
+        for j in range(world // args.pool):
+            g = dist.new_group(list(range(j * args.pool, (j + 1) * args.pool)))
+            if j == plan["pool"]:
+                group = g
+    t = torch.full((4,), float(rank + 1), dtype=torch.float64)
+    if world > 1:
+        from paper_2111_14999_b200.sharding import allreduce_g1
+        allreduce_g1(t, dist, group)
+        dist.barrier()
+    plan["pool_sum"] = float(t[0])
+    ms = max_over_ranks(10.0 + rank, dist if world > 1 else None)
+    plans = [plan]
+    if world > 1:
+        plans = [None] * world
+        dist.all_gather_object(plans, plan)
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "metric": METRIC, "n_gpus": world, "scaling": args.scaling, "pool": args.pool,
+                          "ms_max_over_ranks": ms, "pairs_per_step": sum(p_["pairs"] for p_ in plans), "plans": plans}))
+
+
 # ----------------------------------------------------------------------------- GPU leg
 def run_ours(args):
     import torch
@@ -218,6 +324,18 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    w = wl.CONFIGS[args.workload]
+    if args.pool_emulate:     # one GPU plays rank 0 of a pool of --pool ranks; nothing is summed over the pool
+        assert world == 1, "--pool-emulate is a single-GPU smoke test of the Re-pool code path"
+        plan = rank_plan(w, 0, args.pool, args.scaling, args.pool)
+    else:
+        plan = rank_plan(w, rank, world, args.scaling, args.pool)
+    pool_group = None
+    if dist is not None and args.pool > 1:
+        for j in range(world // args.pool):      # every rank creates every group (collective call), keeps its own
+            g_ = dist.new_group(list(range(j * args.pool, (j + 1) * args.pool)))
+            if j == plan["pool"]:
+                pool_group = g_
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -228,11 +346,17 @@ def run_ours(args):
         dist.barrier()
     binding.load_library()
 
-    w = wl.CONFIGS[args.workload]
     t_gen = time.perf_counter()
-    gW = harness.upload_gW(w, dev)
-    k_ids = shard_k(w.nk, rank, world, "weak")
-    host_inputs = [_k_inputs(w, ik) for ik in k_ids]
+    pooled = args.pool > 1
+    re_lo, re_hi = plan["re"]
+    q_lo, q_hi = plan["q"]
+    nq_l = q_hi - q_lo                           # q-points per k on this rank (the whole list unless pooled)
+    gW = harness.upload_gW(w, dev, re_range=(re_lo, re_hi) if pooled else None)
+    k_ids = plan["k_ids"]
+    host_inputs = []
+    for ik in k_ids:
+        k_, Uk_, qin = _k_inputs(w, ik)
+        host_inputs.append((k_, Uk_, tuple(np.ascontiguousarray(x[q_lo:q_hi]) for x in qin)))
     dev_inputs = []
     for k, Uk, (q, Ukq, ev, om) in host_inputs:
         dev_inputs.append((k, harness.to_device([Uk], dev)[0], harness.to_device([q, Ukq, ev, om], dev)))
@@ -242,16 +366,17 @@ def run_ours(args):
     # (phoebe_elph_q_batch_multi) whenever the stacked C fits 8 GB: for band windows one k-point's list alone is too
     # small a GEMM for 148 SMs (57 % -> 92 % of peak), for the 4-atom cell it removes the ragged last round of tiles and
     # the launch gaps (93.8 % -> 95.1 %)
-    multi = (kb > 1 and args.q_multi != 0 and w.nq % 64 == 0 and len(host_inputs) % kb == 0
-             and (args.q_multi == 1 or kb * w.nq * w.N * 16 <= (8 << 30)))
-    ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0, nq_max=kb * w.nq if multi else None)
+    multi = (kb > 1 and args.q_multi != 0 and nq_l % 64 == 0 and len(host_inputs) % kb == 0
+             and (args.q_multi == 1 or kb * nq_l * w.N * 16 <= (8 << 30)))
+    ctx = harness.make_context(w, gW, nk_max=kb if kb > 1 else 0, nq_max=kb * nq_l if multi else nq_l,
+                               re_range=(re_lo, re_hi) if pooled else None)
     ctx.set_tuning("m3", args.m3)
     if args.tile:
         ctx.set_tuning("tile", args.tile)
     for kv in args.tune:                      # kernel-variant experiments: --tune rot_qg=4 (see include/phoebe_elph.h, set_tuning)
         key, val = kv.split("=")
         ctx.set_tuning(key, int(val))
-    out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+    out = torch.empty((nq_l, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
     # k-points grouped into batches of kb: one pass over g_W per batch (set_k_batch)
     groups = [list(range(i, min(i + kb, len(host_inputs)))) for i in range(0, len(host_inputs), kb)]
     ks_np = [np.stack([host_inputs[i][0] for i in g]) for g in groups]
@@ -260,21 +385,36 @@ def run_ours(args):
 
     if multi:
         stacks = [[torch.stack([dev_inputs[i][2][j] for i in g]).contiguous() for j in range(4)] for g in groups]
-        out_multi = torch.empty((kb, w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+        out_multi = torch.empty((kb, nq_l, w.nb1, w.nb2, w.nm), dtype=torch.float64, device=dev)
+
+    def set_k_batch(ks, Uk_d):
+        # Re-pool: every rank of the pool holds the partial g1' of its Re shard; ONE in-place all-reduce completes it
+        # (sharding.pool_set_k_batch).  NCCL runs on torch's current stream = the library's stream.
+        if pooled:
+            pool_set_k_batch(ctx, ks, Uk_d, dist, pool_group)
+        else:
+            ctx.set_k_batch(ks, Uk_d)
+
+    def step_three_call():
+        # north_star's boundary as it stands: set_k, then q_batch, for every k-point
+        for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
+            if pooled:
+                pool_set_k(ctx, k, Uk_d, dist, pool_group)
+            else:
+                ctx.set_k(k, Uk_d)
+            ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
 
     def step():
         if multi:
             for ks, Uk_d, (q_s, Ukq_s, ev_s, om_s) in zip(ks_np, Uks_d, stacks):
-                ctx.set_k_batch(ks, Uk_d)
+                set_k_batch(ks, Uk_d)
                 ctx.q_batch_multi(q_s, Ukq_s, ev_s, om_s, out_multi)
             return
         if kb == 1:
-            for k, Uk_d, (q_d, Ukq_d, ev_d, om_d) in dev_inputs:
-                ctx.set_k(k, Uk_d)
-                ctx.q_batch(q_d, Ukq_d, ev_d, om_d, out)
+            step_three_call()
             return
         for g, ks, Uk_d in zip(groups, ks_np, Uks_d):
-            ctx.set_k_batch(ks, Uk_d)
+            set_k_batch(ks, Uk_d)
             for j, i in enumerate(g):
                 ctx.select_k(j)
                 q_d, Ukq_d, ev_d, om_d = dev_inputs[i][2]
@@ -306,7 +446,11 @@ def run_ours(args):
     ms_total = maxreduce(e0.elapsed_time(e1))
     clocks = sampler.stop() if rank == 0 else {}
     gpu_launches = sum(ctx.launch_counts().values()) - launches0
-    pairs_per_step_all = world * w.nk * w.nq
+    pairs_per_step_all = plan["pairs"]
+    if dist is not None:
+        t_pairs = torch.tensor([plan["pairs"]], dtype=torch.int64, device=dev)
+        dist.all_reduce(t_pairs)
+        pairs_per_step_all = int(t_pairs.item())
     value = pairs_per_step_all * args.steps / (ms_total * 1e-3)
 
     # ---- per-kernel durations (CUDA events inside the library, on its stream) ---
@@ -318,7 +462,10 @@ def run_ours(args):
     ctx.profile(False)
     m3 = bool(ctx.get_tuning("m3"))
     pair_rows = ctx.get_tuning("pair_rows")     # > 0: a4 runs the +R / -R pair form (4 real flop per MAC)
-    counts = harness.algorithmic_counts(w, m3=m3, pair_rows=pair_rows)
+    counts = harness.algorithmic_counts(w, nq=nq_l, m3=m3, pair_rows=pair_rows)
+    if pooled:       # a rank of a Re-pool streams only its share of g_W
+        for key in ("setk_bytes", "setk_stream_bytes", "setk_flop", "setk_stream_flop", "setk_gemm_flop"):
+            counts[key] = counts[key] * (re_hi - re_lo) // w.nRe
     peaks, peak_src = _measured_peaks()
     hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
     kernels = {}
@@ -370,16 +517,99 @@ def run_ours(args):
         except Exception:
             fp64_probe = None
 
+    # ---- FP64 ceilings measured in the same run (SURVEY 8(d) "Peaks"): the two in-library probes above and cuBLAS
+    # (through torch.matmul: the product library links no cuBLAS) at the contraction's own shape -- ceilings only ----
+    ceilings = None
+    if rank == 0:
+        ceilings = {"derived_tflops": FP64_PEAK_TFLOPS}
+        if fp64_probe:
+            ceilings.update(dmma_probe_tflops=fp64_probe["dmma_tflops"], dfma_probe_tflops=fp64_probe["dfma_tflops"])
+        try:
+            ceilings.update(cublas_ceilings(torch, dev, min(16384, max(1024, len(dev_inputs) * nq_l)), w.N, w.nRp))
+        except Exception as exc:          # a ceiling that cannot be measured is reported as such, never guessed
+            ceilings["cublas_error"] = str(exc)[:200]
+        best = max(v for k_, v in ceilings.items() if k_ in ("derived_tflops", "dmma_probe_tflops", "cublas_dgemm_tflops"))
+        ceilings["max_tflops"] = best
+        for kk in kernels.values():
+            if kk.get("bound") == "alu":
+                kk["frac_of_max_ceiling"] = kk["achieved"] / best
+
+    # ---- Re-pool check (f3): g1' of the pooled path against the unsharded path, element by element, on this rank ----
+    pool_check = None
+    if pooled:
+        free_b, _ = torch.cuda.mem_get_info()
+        if free_b > w.gW_bytes + (16 << 30):
+            gW_full = harness.upload_gW(w, dev)
+            ctx_full = harness.make_context(w, gW_full, nk_max=kb if kb > 1 else 0, nq_max=64)
+            worst = 0.0
+            ks0, Uk0 = ks_np[0], Uks_d[0]
+            if kb > 1:
+                ctx_full.set_k_batch(ks0, Uk0)
+                set_k_batch(ks0, Uk0)
+            else:
+                ctx_full.set_k(ks0[0], Uk0[0])
+                pool_set_k(ctx, ks0[0], Uk0[0], dist, pool_group)
+            for j in range(len(groups[0])):
+                a_ = ctx.g1_view(j)
+                b_ = ctx_full.g1_view(j)
+                worst = max(worst, float(((a_ - b_).abs().max() / b_.abs().max()).item()))
+            ctx_full.close()
+            del gW_full
+            torch.cuda.empty_cache()
+            pool_check = {"what": "max |g1'(Re-pool, all-reduced) - g1'(unsharded)| / max |g1'| over the first k batch, "
+                                  "worst rank", "max_rel_err": maxreduce(worst), "ok": maxreduce(worst) < 1e-12}
+        else:
+            pool_check = {"skipped": "not enough free device memory for the unsharded g_W beside the shard"}
+
+    # ---- the north-star boundary as it stands: set_k + q_batch per k-point (no set_k_batch, no stacking) ----
+    three_call = None
+    if not args.no_three_call and kb > 1:
+        for _ in range(2):
+            step_three_call()
+        barrier()
+        n3 = max(1, min(args.steps, 3))
+        e0.record()
+        for _ in range(n3):
+            step_three_call()
+        e1.record()
+        barrier()
+        ms3 = maxreduce(e0.elapsed_time(e1))
+        ctx.profile(True)
+        step_three_call()
+        prof3 = ctx.profile_read()
+        ctx.profile(False)
+        c1 = harness.algorithmic_counts(w, nq=nq_l, m3=m3, pair_rows=ctx.get_tuning("pair_rows"))
+        k3 = {kind: {"ms_total": ms_, "launches_per_step": n_, "avg_ms": ms_ / n_} for kind, (ms_, n_) in prof3.items() if n_}
+        share = (re_hi - re_lo) / w.nRe if pooled else 1.0
+        for kind, bound, work in (("setk_stream", "hbm", c1["setk_stream_bytes"] * share), ("contract", "alu", c1["contract_flop"]),
+                                  ("rotate_epilogue", "alu" if rot_alu else "hbm", c1["rotate_flop"] if rot_alu else c1["rotate_bytes"])):
+            if kind in k3:
+                dur = k3[kind]["avg_ms"] * 1e-3
+                peak_ = FP64_PEAK_TFLOPS if bound == "alu" else hbm_peak
+                ach = work / dur / (1e12 if bound == "alu" else 1e9)
+                k3[kind].update(bound=bound, achieved=ach, peak=peak_, unit="TFLOP/s" if bound == "alu" else "GB/s", frac=ach / peak_)
+        three_call = {"what": "phoebe_elph_set_k + phoebe_elph_q_batch per k-point (north_star's three-call boundary; g_W is "
+                              "re-read for every k-point)", "value": pairs_per_step_all * n3 / (ms3 * 1e-3), "unit": UNIT,
+                      "ms_per_step": ms3 / n3, "kernels": k3}
+
     # ---- end to end: host buffers through the C ABI, copies inside the timed region ----
     pinned = []
     for k, Uk, (q, Ukq, ev, om) in host_inputs:
         pin = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (Uk, q, Ukq, ev, om)]
         pinned.append((k, pin))
     Uks_pin = [torch.from_numpy(u).pin_memory() for u in Uks_np]
-    out_hosts = [torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory() for _ in range(2)]
+    out_hosts = [torch.empty((nq_l, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory() for _ in range(2)]
     out_host = out_hosts[0]
     h2d = sum(sum(t.numel() * t.element_size() for t in pin) + 24 for _, pin in pinned)
     d2h = len(pinned) * out_host.numel() * 8
+
+    def set_k_host(ks, Uk_p):
+        if kb == 1:
+            ctx.set_k_host(ks[0], Uk_p.numpy()[0])
+        else:
+            ctx.set_k_batch_host(ks, Uk_p.numpy())
+        if pooled:
+            allreduce_g1(ctx.g1_view(-1), dist, pool_group)
 
     def step_e2e():
         # every k-point: inputs host->device, |g|^2 device->host (into two alternating pinned buffers, as a consumer
@@ -387,10 +617,7 @@ def run_ours(args):
         # copies with the kernels; the step ends when the last result is on the host (phoebe_elph_wait)
         n = 0
         for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
-            if kb == 1:
-                ctx.set_k_host(ks[0], Uk_p.numpy()[0])
-            else:
-                ctx.set_k_batch_host(ks, Uk_p.numpy())
+            set_k_host(ks, Uk_p)
             for j, i in enumerate(g):
                 ctx.select_k(j)
                 _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
@@ -418,7 +645,7 @@ def run_ours(args):
     rates = None
     if not args.no_rates:
         P = wl.RATE_PARAMS
-        eps_np = [wl.band_energies(w, ik) for ik in k_ids]
+        eps_np = [(e1_, np.ascontiguousarray(e2_[q_lo:q_hi])) for e1_, e2_ in (wl.band_energies(w, ik) for ik in k_ids)]
         eps_d = [harness.to_device([e1, e2], dev) for e1, e2 in eps_np]
         rate_d = torch.zeros((len(dev_inputs), w.nb1), dtype=torch.float64, device=dev)
 
@@ -430,14 +657,17 @@ def run_ours(args):
         def step_rates():
             if multi:
                 for ig, (ks, Uk_d, (q_s, Ukq_s, ev_s, om_s)) in enumerate(zip(ks_np, Uks_d, stacks)):
-                    ctx.set_k_batch(ks, Uk_d)
+                    set_k_batch(ks, Uk_d)
                     ctx.q_batch_rates_multi(q_s, Ukq_s, ev_s, om_s, eps_k_s[ig], eps_kq_s[ig], rate_s[ig], **P)
                 return
             for g, ks, Uk_d in zip(groups, ks_np, Uks_d):
                 if kb == 1:
-                    ctx.set_k(ks[0], Uk_d[0])
+                    if pooled:
+                        pool_set_k(ctx, ks[0], Uk_d[0], dist, pool_group)
+                    else:
+                        ctx.set_k(ks[0], Uk_d[0])
                 else:
-                    ctx.set_k_batch(ks, Uk_d)
+                    set_k_batch(ks, Uk_d)
                 for j, i in enumerate(g):
                     ctx.select_k(j)
                     q_d, Ukq_d, ev_d, om_d = dev_inputs[i][2]
@@ -456,10 +686,7 @@ def run_ours(args):
 
         def step_rates_e2e():
             for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
-                if kb == 1:
-                    ctx.set_k_host(ks[0], Uk_p.numpy()[0])
-                else:
-                    ctx.set_k_batch_host(ks, Uk_p.numpy())
+                set_k_host(ks, Uk_p)
                 for j, i in enumerate(g):
                     ctx.select_k(j)
                     _, (_, q_p, Ukq_p, ev_p, om_p) = pinned[i]
@@ -487,14 +714,14 @@ def run_ours(args):
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, cores, sample, _ = time_oracle(w, 20.0)
-        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "extrapolated": True}
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": _with_multi(_with_kbatch(_config_dict(w, world), kb), multi),
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": _with_multi(_with_kbatch(_config_dict(w, world, args.scaling, args.pool), kb), multi),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else "q_batch_host_async + wait"},
@@ -502,16 +729,20 @@ def run_ours(args):
             "roofline": roofline,
             "kernels": kernels,
             "fp64_probe": fp64_probe,
+            "fp64_ceilings": ceilings,
+            "three_call": three_call,
+            "pool_check": pool_check,
             "cpu_baseline": cpu_baseline,
             "rates_fused": rates,
             "fp64_tflops_whole_path_4m_equivalent": (counts["setk_flop"] + counts["contract_flop_4m"] + counts["rotate_flop"]) * w.nk * world
             * args.steps / (ms_total * 1e-3) / 1e12,
             "input_gen_s": round(t_gen, 1),
         }
-        print(json.dumps(line))
     ctx.close()
     if dist is not None:
         dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)     # the last thing on stdout, behind NCCL's shutdown messages
 
 
 def main():
@@ -532,8 +763,24 @@ def main():
                     help="phoebe_elph_set_tuning knob for kernel-variant experiments (repeatable)")
     ap.add_argument("--k-batch", type=int, default=32,
                     help="k-points per pass over g_W (phoebe_elph_set_k_batch); 1 = one set_k per k")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank (pool) runs the workload's nk k-points of its own; strong = the workload's "
+                         "nk k-points are dealt over the ranks (the paper's axis: MPI loop over k, PAPER.md L556, L705)")
+    ap.add_argument("--pool", type=int, default=1,
+                    help="Re-pool size P (PAPER.md L576): P ranks share one g_W, sharded over Re; one all-reduce of g1' per "
+                         "set_k_batch, then the q lists are shared out.  Must divide the number of ranks")
+    ap.add_argument("--pool-emulate", action="store_true",
+                    help="single-GPU smoke test of the Re-pool code path: this rank acts as rank 0 of a pool of --pool ranks "
+                         "and the all-reduce is skipped, so g1' stays partial and pool_check must report the mismatch")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="process-group backend (gloo: --dry-run only)")
+    ap.add_argument("--dry-run", action="store_true", help="N-rank plumbing only (no GPU): prints every rank's plan")
+    ap.add_argument("--no-three-call", action="store_true", help="skip the extra set_k + q_batch per k measurement")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args, sys.argv[1:]))
+    if args.dry_run:
+        run_dry(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

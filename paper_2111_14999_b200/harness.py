@@ -13,13 +13,16 @@ from . import binding
 from . import workloads as wl
 
 
-def upload_gW(w: wl.Workload, device="cuda:0", threads: int | None = None):
+def upload_gW(w: wl.Workload, device="cuda:0", threads: int | None = None, re_range=None):
     """g_W as a CUDA complex128 tensor [nRp][nRe][nw][nw][nm], generated slab by slab
     on the host (bit-identical to workloads.gW_slab) and copied through a small ring
-    of pinned buffers, so the 57.8 GB workload never exists on the host at once."""
+    of pinned buffers, so the 57.8 GB workload never exists on the host at once.
+    re_range = (lo, hi): only the electron lattice vectors lo..hi-1 (the shard of one rank of a
+    Re-pool): [nRp][hi-lo][nw][nw][nm]."""
     import torch
 
-    gW = torch.empty((w.nRp, w.nRe, w.nw, w.nw, w.nm), dtype=torch.complex128, device=device)
+    lo, hi = (0, w.nRe) if re_range is None else re_range
+    gW = torch.empty((w.nRp, hi - lo, w.nw, w.nw, w.nm), dtype=torch.complex128, device=device)
     threads = threads or min(32, os.cpu_count() or 8)
     slab_shape = (w.nRe, w.nw, w.nw, w.nm)
     nbuf = threads * 2
@@ -49,7 +52,7 @@ def upload_gW(w: wl.Workload, device="cuda:0", threads: int | None = None):
                 p, slot = fut.result()
                 del pending[fut]
                 with torch.cuda.stream(stream):
-                    gW[p].copy_(pinned[slot], non_blocking=True)
+                    gW[p].copy_(pinned[slot][lo:hi], non_blocking=True)
                     ev = torch.cuda.Event()
                     ev.record(stream)
                 events[slot] = ev
@@ -60,8 +63,13 @@ def upload_gW(w: wl.Workload, device="cuda:0", threads: int | None = None):
 
 
 def make_context(w: wl.Workload, gW, *, nq_max=None, deg_e=None, deg_p=None, hbm_budget_bytes=None,
-                 nb1_max=None, nb2_max=None, nk_max=0) -> binding.ElphContext:
-    return binding.ElphContext(gW, wl.Re_vectors(w), wl.Rp_vectors(w), deg_e, deg_p,
+                 nb1_max=None, nb2_max=None, nk_max=0, re_range=None) -> binding.ElphContext:
+    """re_range = (lo, hi): gW holds only these electron lattice vectors (one rank of a Re-pool)."""
+    Re = wl.Re_vectors(w)
+    if re_range is not None:
+        Re = np.ascontiguousarray(Re[re_range[0]:re_range[1]])
+        deg_e = None if deg_e is None else np.ascontiguousarray(deg_e[re_range[0]:re_range[1]])
+    return binding.ElphContext(gW, Re, wl.Rp_vectors(w), deg_e, deg_p,
                                nb1_max=nb1_max or w.nb1, nb2_max=nb2_max or w.nb2,
                                nq_max=nq_max or w.nq, nk_max=nk_max, hbm_budget_bytes=hbm_budget_bytes)
 

@@ -148,3 +148,44 @@ def test_shard_range_properties():
             assert max(sizes) - min(sizes) <= 1
     t = torch.ones(3, dtype=torch.complex128)
     assert sharding.allreduce_g1(t) is t
+
+
+def _run_bench_dry(*flags):
+    """bench.py --gpus 2 started WITHOUT torchrun: it must re-exec itself under torch.distributed.run with two ranks
+    (the launch line the driver uses) and rank 0 must print ONE JSON line for the whole job."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry-run", "--backend", "gloo",
+                        *flags], capture_output=True, text=True, timeout=300, env=env, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    return json.loads(lines[0])
+
+
+@pytest.mark.parametrize("scaling", ["weak", "strong"])
+def test_bench_gpus2_spawns_two_ranks(scaling):
+    d = _run_bench_dry("--workload", "4-atom", "--scaling", scaling)
+    w = wl.CONFIGS["4-atom"]
+    assert d["n_gpus"] == 2 and d["scaling"] == scaling and d["ms_max_over_ranks"] == 11.0
+    ks = sorted(sum((p["k_ids"] for p in d["plans"]), []))
+    assert ks == (list(range(2 * w.nk)) if scaling == "weak" else list(range(w.nk)))
+    assert d["pairs_per_step"] == (2 if scaling == "weak" else 1) * w.nk * w.nq
+    assert all(p["re"] == [0, w.nRe] and p["q"] == [0, w.nq] for p in d["plans"])      # no pool: g_W replicated
+
+
+def test_bench_gpus2_re_pool_plan():
+    """--pool 2: the two ranks form one Re-pool: same k-points, disjoint Re shards that cover the list, disjoint q
+    slices in multiples of the contraction's 64-row tile, and the pool's all-reduce (through sharding.allreduce_g1,
+    the helper the GPU path uses) sums over both ranks."""
+    d = _run_bench_dry("--workload", "band-window", "--pool", "2", "--scaling", "strong")
+    w = wl.CONFIGS["band-window"]
+    p0, p1 = d["plans"]
+    assert p0["k_ids"] == p1["k_ids"] == list(range(w.nk)) and p0["pool"] == p1["pool"] == 0
+    assert p0["re"][0] == 0 and p0["re"][1] == p1["re"][0] and p1["re"][1] == w.nRe
+    assert p0["q"][0] == 0 and p0["q"][1] == p1["q"][0] and p1["q"][1] == w.nq and p0["q"][1] % 64 == 0
+    assert p0["pool_sum"] == p1["pool_sum"] == 3.0
+    assert d["pairs_per_step"] == w.nk * w.nq
