@@ -14,12 +14,17 @@ LIB = os.path.join(HERE, "liboracle_elph.so")
 
 
 def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB)
+    """ORACLE_SANITIZE=1 in the environment builds with -fsanitize=address,undefined (run the CPU pins with
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so); see profiles/r2_sanitizers.md)."""
+    san = os.environ.get("ORACLE_SANITIZE") == "1"
+    if (not force and not san and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
     # -O2, no -ffast-math: the oracle is meant to be plain, not tuned.
     cmd = ["gcc", "-std=c99", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall",
            "-o", LIB, SRC, "-lm"]
+    if san:
+        cmd[1:1] = ["-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -129,7 +129,7 @@ class ElphContext:
     """
 
     def __init__(self, gW, Re, Rp, deg_e=None, deg_p=None, *, nb1_max=None, nb2_max=None, nq_max, nk_max=0,
-                 hbm_budget_bytes=None, stream=None):
+                 hbm_budget_bytes=None, stream=None, poison_workspace=False):
         import numpy as np
         import torch
 
@@ -153,6 +153,8 @@ class ElphContext:
         self.nq_batch = nqb
         self.workspace_nbytes = nbytes
         self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        if poison_workspace:      # test aid: every double of the workspace starts as a NaN (tests/test_gpu_guards.py)
+            self._ws.fill_(0xFF)
         ws_ptr = (self._ws.data_ptr() + 255) // 256 * 256
         Re = np.ascontiguousarray(Re, dtype=np.float64); Rp = np.ascontiguousarray(Rp, dtype=np.float64)
         assert Re.shape == (nRe, 3) and Rp.shape == (nRp, 3)
