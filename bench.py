@@ -611,7 +611,22 @@ def run_ours(args):
         if pooled:
             allreduce_g1(ctx.g1_view(-1), dist, pool_group)
 
+    if multi:     # k-stacked pinned arrays of every k batch (the layout of phoebe_elph_q_batch_multi_host_async)
+        stacks_pin = [[torch.from_numpy(np.ascontiguousarray(np.stack([host_inputs[i][2][j] for i in g]))).pin_memory()
+                       for j in range(4)] for g in groups]
+        out_multi_hosts = [torch.empty((kb, nq_l, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory() for _ in range(2)]
+
+    def step_e2e_multi():
+        # one call per k batch: the stacked inputs host->device, the stacked |g|^2 device->host (two alternating pinned
+        # buffers); copies of neighbouring batches and the next set_k_batch overlap this batch's kernels
+        for n, (ks, Uk_p, st_p) in enumerate(zip(ks_np, Uks_pin, stacks_pin)):
+            set_k_host(ks, Uk_p)
+            ctx.q_batch_multi_host_async(*[t.numpy() for t in st_p], out_multi_hosts[n & 1].numpy())
+        ctx.wait()
+
     def step_e2e():
+        if multi and not args.e2e_sync:
+            return step_e2e_multi()
         # every k-point: inputs host->device, |g|^2 device->host (into two alternating pinned buffers, as a consumer
         # that reads batch n while batch n+1 is computed would hold them); phoebe_elph_q_batch_host_async overlaps the
         # copies with the kernels; the step ends when the last result is on the host (phoebe_elph_wait)
@@ -684,7 +699,19 @@ def run_ours(args):
         eps_pin = [[torch.from_numpy(np.ascontiguousarray(x)).pin_memory() for x in e] for e in eps_np]
         rate_h = torch.zeros((len(dev_inputs), w.nb1), dtype=torch.float64).pin_memory().numpy()
 
+        if multi:
+            eps_k_pin = [torch.from_numpy(np.stack([eps_np[i][0] for i in g])).pin_memory() for g in groups]
+            eps_kq_pin = [torch.from_numpy(np.ascontiguousarray(np.stack([eps_np[i][1] for i in g]))).pin_memory() for g in groups]
+            rate_hm = [torch.zeros((len(g), w.nb1), dtype=torch.float64).pin_memory() for g in groups]
+
         def step_rates_e2e():
+            if multi:
+                for n, (ks, Uk_p, st_p) in enumerate(zip(ks_np, Uks_pin, stacks_pin)):
+                    set_k_host(ks, Uk_p)
+                    ctx.q_batch_rates_multi_host_async(*[t.numpy() for t in st_p], eps_k_pin[n].numpy(), eps_kq_pin[n].numpy(),
+                                                       rate_hm[n].numpy(), **P)
+                ctx.wait()
+                return
             for g, ks, Uk_p in zip(groups, ks_np, Uks_pin):
                 set_k_host(ks, Uk_p)
                 for j, i in enumerate(g):
@@ -724,7 +751,8 @@ def run_ours(args):
             "config": _with_multi(_with_kbatch(_config_dict(w, world, args.scaling, args.pool), kb), multi),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else "q_batch_host_async + wait"},
+                    "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else
+                    ("set_k_batch_host + q_batch_multi_host_async + wait" if multi else "q_batch_host_async + wait")},
             "gpu_launches": int(gpu_launches),
             "roofline": roofline,
             "kernels": kernels,

@@ -218,6 +218,23 @@ int phoebe_elph_q_batch_rates_multi(phoebe_elph_ctx* ctx, int32_t nk, int32_t nq
                                     const double* eps_k_dev, const double* eps_kq_dev, const phoebe_elph_rate_params* prm,
                                     double* rate_dev, double* out_dev);
 
+/* Pipelined HOST forms of the two stacked calls (a single small call is latency-bound, so batch; L707: the
+ * results go back to the CPU): the k-stacked arrays of a whole set_k_batch in PINNED host memory, same layout as the device
+ * forms.  Like q_batch_host_async they return at once: the copy-in of batch n+1 (its own stream) and the copy-out of batch
+ * n-1 (its own stream) overlap the kernels of batch n -- and so does the next set_k_batch, which runs on the compute stream
+ * behind this batch's kernels while its results are still being copied out.  Host arrays (and rate_host, out_host) must
+ * stay valid and untouched until phoebe_elph_wait; at most two batches are in flight.
+ * Errors: as the device forms. */
+int phoebe_elph_q_batch_multi_host_async(phoebe_elph_ctx* ctx, int32_t nk, int32_t nq, int32_t nb2, const double* q_host,
+                                         const void* Ukq_host, const void* ev_host, const double* omega_host,
+                                         double* out_host);
+int phoebe_elph_q_batch_rates_multi_host_async(phoebe_elph_ctx* ctx, int32_t nk, int32_t nq, int32_t nb2,
+                                               const double* q_host, const void* Ukq_host, const void* ev_host,
+                                               const double* omega_host, const double* eps_k_host,
+                                               const double* eps_kq_host, const phoebe_elph_rate_params* prm,
+                                               double* rate_host /* [nk][nb1], accumulated into */,
+                                               double* out_host /* [nk][nq][nb1][nb2][nmodes] or NULL */);
+
 /* Same with HOST buffers (rate_host [nb1] is read, accumulated into and written back; out_host may be
  * NULL, and then only nb1 doubles come back); SYNCHRONISES the stream before returning. */
 int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* ctx, int32_t nq, int32_t nb2,

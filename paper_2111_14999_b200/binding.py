@@ -22,7 +22,7 @@ EXPORTS = [
     "phoebe_elph_set_k_batch", "phoebe_elph_set_k_batch_host", "phoebe_elph_select_k",
     "phoebe_elph_q_batch", "phoebe_elph_q_batch_multi", "phoebe_elph_q_batch_host", "phoebe_elph_q_batch_host_async", "phoebe_elph_wait",
     "phoebe_elph_q_batch_rates", "phoebe_elph_q_batch_rates_host", "phoebe_elph_q_batch_rates_host_async",
-    "phoebe_elph_q_batch_rates_multi",
+    "phoebe_elph_q_batch_rates_multi", "phoebe_elph_q_batch_multi_host_async", "phoebe_elph_q_batch_rates_multi_host_async",
     "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_set_conventions", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
@@ -74,6 +74,9 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_q_batch_multi.argtypes = [c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
     lib.phoebe_elph_q_batch_host_async.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_q_batch_multi_host_async.argtypes = [c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 5
+    lib.phoebe_elph_q_batch_rates_multi_host_async.argtypes = ([c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 6 +
+                                                               [POINTER(RateParams), c_void_p, c_void_p])
     lib.phoebe_elph_wait.argtypes = [c_void_p]
     lib.phoebe_elph_q_batch_rates.argtypes = [c_void_p, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
     lib.phoebe_elph_q_batch_rates_multi.argtypes = [c_void_p, c_int32, c_int32, c_int32] + [c_void_p] * 6 + [POINTER(RateParams), c_void_p, c_void_p]
@@ -109,6 +112,19 @@ def workspace_bytes(dims: Dims, hbm_budget_bytes: int):
     if rc:
         raise PhoebeElphError(rc, "phoebe_elph_workspace_bytes")
     return int(nbytes.value), int(nqb.value)
+
+
+def _chk_host(**arrays):
+    """The host entry points read raw memory: every array must be C-contiguous with the dtype the C ABI expects
+    (complex128 for Ukq / ev, float64 otherwise)."""
+    import numpy as np
+    for name, a in arrays.items():
+        if a is None:
+            continue
+        want = np.complex128 if name in ("Ukq", "ev") else np.float64
+        if a.dtype != want or not a.flags.c_contiguous:
+            raise TypeError(f"{name}: expected a C-contiguous {np.dtype(want).name} array, got {a.dtype}"
+                            f"{'' if a.flags.c_contiguous else ' (not contiguous)'}")
 
 
 def _host_ptr(a):
@@ -149,6 +165,9 @@ class ElphContext:
             hbm_budget_bytes = int(free * 0.9)
         nbytes, nqb = workspace_bytes(self.dims, hbm_budget_bytes)
         if nqb < nq_max:
+            import warnings
+            warnings.warn(f"workspace budget {hbm_budget_bytes} B fits only {nqb} of the requested {nq_max} q-points per "
+                          "batch: dims.nq_max lowered, larger q_batch calls will fail with E_DIMS", RuntimeWarning)
             self.dims.nq_max = nqb
         self.nq_batch = nqb
         self.workspace_nbytes = nbytes
@@ -264,6 +283,7 @@ class ElphContext:
 
     def q_batch_host(self, q, Ukq, ev, omega, out):
         """NumPy arrays (or pinned CPU tensors via .numpy()); synchronises before returning."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, out=out)
         nq, nw, nb2 = Ukq.shape
         self._check(self._lib.phoebe_elph_q_batch_host(self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data,
                                                        ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
@@ -272,11 +292,34 @@ class ElphContext:
 
     def q_batch_host_async(self, q, Ukq, ev, omega, out):
         """Pipelined q_batch_host: NumPy views of PINNED memory; returns at once -- call wait() before reading out."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, out=out)
         nq, nw, nb2 = Ukq.shape
         self._check(self._lib.phoebe_elph_q_batch_host_async(self._ctx, nq, nb2, q.ctypes.data, Ukq.ctypes.data,
                                                              ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
                     "phoebe_elph_q_batch_host_async")
         return out
+
+    def q_batch_multi_host_async(self, q, Ukq, ev, omega, out):
+        """Pipelined q_batch_multi over PINNED host arrays stacked over k (q [nk][nq][3], ...); call wait() before
+        reading out [nk][nq][nb1][nb2][nm]."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, out=out)
+        nk, nq, nw, nb2 = Ukq.shape
+        self._check(self._lib.phoebe_elph_q_batch_multi_host_async(self._ctx, nk, nq, nb2, q.ctypes.data, Ukq.ctypes.data,
+                                                                   ev.ctypes.data, omega.ctypes.data, out.ctypes.data),
+                    "phoebe_elph_q_batch_multi_host_async")
+        return out
+
+    def q_batch_rates_multi_host_async(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):
+        """Pipelined q_batch_rates_multi over PINNED host arrays stacked over k; rate [nk][nb1] is accumulated into;
+        call wait() before reading rate / out."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, eps_k=eps_k, eps_kq=eps_kq, rate=rate, out=out)
+        nk, nq, nw, nb2 = Ukq.shape
+        prm = RateParams(kT, mu, sigma, pref)
+        self._check(self._lib.phoebe_elph_q_batch_rates_multi_host_async(
+            self._ctx, nk, nq, nb2, q.ctypes.data, Ukq.ctypes.data, ev.ctypes.data, omega.ctypes.data, eps_k.ctypes.data,
+            eps_kq.ctypes.data, byref(prm), rate.ctypes.data, None if out is None else out.ctypes.data),
+            "phoebe_elph_q_batch_rates_multi_host_async")
+        return rate, out
 
     def wait(self):
         self._check(self._lib.phoebe_elph_wait(self._ctx), "phoebe_elph_wait")
@@ -325,6 +368,7 @@ class ElphContext:
 
     def q_batch_rates_host(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):
         """NumPy arrays; rate [nb1] is accumulated into in place; synchronises before returning."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, eps_k=eps_k, eps_kq=eps_kq, rate=rate, out=out)
         nq, nw, nb2 = Ukq.shape
         prm = RateParams(kT, mu, sigma, pref)
         self._check(self._lib.phoebe_elph_q_batch_rates_host(
@@ -336,6 +380,7 @@ class ElphContext:
     def q_batch_rates_host_async(self, q, Ukq, ev, omega, eps_k, eps_kq, rate, *, kT, mu, sigma, pref, out=None):
         """Pipelined q_batch_rates_host (NumPy views of PINNED memory; one rate array per call in flight); returns at
         once -- call wait() before reading rate / out."""
+        _chk_host(q=q, Ukq=Ukq, ev=ev, omega=omega, eps_k=eps_k, eps_kq=eps_kq, rate=rate, out=out)
         nq, nw, nb2 = Ukq.shape
         prm = RateParams(kT, mu, sigma, pref)
         self._check(self._lib.phoebe_elph_q_batch_rates_host_async(

@@ -114,7 +114,7 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_C = take((size_t)L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16);
     // f2: linewidth partials [nq][groups of b2 tiles][nb1], staging of rate / eps_k / eps_kq for the host entry point
     L.off_part = take((size_t)nq_max * ceil_div(d.nb2_max, 8) * d.nb1_max * 8);
-    L.off_rate = take((size_t)2 * 2 * d.nb1_max * 8);                 // two slots of (rate, eps_k)
+    L.off_rate = take((size_t)2 * 2 * L.nk_slots * d.nb1_max * 8);    // two slots of (rate, eps_k), each [k slots][nb1]
     L.off_seps = take((size_t)2 * nq_max * d.nb2_max * 8);            // two slots of eps_kq
     // f4: G list and Born charges of the polar term, its (q, nu) amplitudes
     L.off_G = take((size_t)kMaxG * 3 * 8);
@@ -506,9 +506,10 @@ struct RateReq {           // f2: linewidth accumulation fused into the epilogue
     const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate;
 };
 
-// rows_per_k > 0: the q lists of the k slots 0.. are stacked (nq = slots * rows_per_k rows); row block j uses the g1' of slot j
+// rows_per_k > 0: the q lists of the k slots slot0, slot0+1, .. are stacked (nq = slots * rows_per_k rows); row block j uses
+// the g1' of slot slot0 + j
 int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const double2* Ukq, const double2* ev,
-                const double* omega, double* out, const RateReq* rr = nullptr, int rows_per_k = 0)
+                const double* omega, double* out, const RateReq* rr = nullptr, int rows_per_k = 0, int slot0 = 0)
 {
     const phoebe_elph_dims& d = c->dims;
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
@@ -617,13 +618,14 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             GemmArgs g{c->Pt, c->L.ldq, c->g1, N, 0, c->C, ldcq, 0, nqs, N, d.nRp, c->L.Kpad, 1};
             g.cm = cm;
             if (rows_per_k > 0) {
-                g.B = c->g1_base; g.rowsPerB = rows_per_k; g.rowOffset = qs; g.strideBrow = (long long)c->L.g1_stride;
+                g.B = c->g1_base + (size_t)slot0 * c->L.g1_stride; g.rowsPerB = rows_per_k; g.rowOffset = qs;
+                g.strideBrow = (long long)c->L.g1_stride;
             }
             if (use_pair) {
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs * c->pair_ctas);
-                const int slot = rows_per_k > 0 ? 0 : c->k_sel;
+                const int slot = rows_per_k > 0 ? slot0 : c->k_sel;
                 int panelW = grid;      // as for the planar form: the panel of pair rows (width x Kr x 1024 B) stays in L2
                 while (panelW % 2 == 0 && (size_t)panelW * c->pair_Kr * pe::PairCfg::ROWB * 8 > (48u << 20)) panelW /= 2;
                 pe::k_contract_pair<<<grid, pe::PairCfg::kThreads, pe::PairCfg::kSmemBytes, c->stream>>>(
@@ -634,7 +636,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_planar, pe::PlanarCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs);
-                const int slot = rows_per_k > 0 ? 0 : c->k_sel;
+                const int slot = rows_per_k > 0 ? slot0 : c->k_sel;
                 // panel width: a divisor of the grid (each CTA keeps its column tile for a whole panel) small enough
                 // that the panel of g1P (width x K x 1536 B) stays L2-resident next to the streaming phase rows and C
                 int panelW = grid;
@@ -975,9 +977,11 @@ int phoebe_elph_q_batch_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const 
 namespace {
 struct RateHost { const double* eps_k; const double* eps_kq; phoebe_elph_rate_params prm; double* rate; };
 
-// one pipelined host batch: copy-in stream -> compute stream -> copy-out stream over staging slot (n mod 2)
+// one pipelined host batch: copy-in stream -> compute stream -> copy-out stream over staging slot (n mod 2).
+// nk_stack > 0: the arrays hold the q lists of nk_stack k slots, k slowest (nq = rows of ALL of them): the stacked forms
 int async_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_host, const void* Ukq_host,
-                const void* ev_host, const double* omega_host, double* out_host, const RateHost* rh)
+                const void* ev_host, const double* omega_host, double* out_host, const RateHost* rh, int nk_stack = 0,
+                int slot0 = 0)
 {
     if (!c->async_ready) {
         PE_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
@@ -1008,15 +1012,16 @@ int async_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_hos
     PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->s_in));
     PE_CUDA(c, cudaMemcpyAsync(sZ, ev_host, (size_t)nq * d.nmodes * d.nmodes * 16, cudaMemcpyHostToDevice, c->s_in));
     PE_CUDA(c, cudaMemcpyAsync(sw, omega_host, (size_t)nq * d.nmodes * 8, cudaMemcpyHostToDevice, c->s_in));
-    double* srate = reinterpret_cast<double*>(c->ws + c->L.off_rate) + (size_t)slot * 2 * d.nb1_max;
-    double* se1 = srate + d.nb1_max;
+    const size_t nrate = (size_t)std::max(1, nk_stack) * c->nb1;       // rate / eps_k values of this batch
+    double* srate = reinterpret_cast<double*>(c->ws + c->L.off_rate) + (size_t)slot * 2 * c->L.nk_slots * d.nb1_max;
+    double* se1 = srate + (size_t)c->L.nk_slots * d.nb1_max;
     double* se2 = reinterpret_cast<double*>(c->ws + c->L.off_seps) + (size_t)slot * d.nq_max * d.nb2_max;
     if (rh) {
         // srate is the one buffer both the copy-in and the copy-out stream touch: the copy-out of the batch that last
         // used this slot must have read it before the next initial values land
         if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->s_in, c->ev_out[slot], 0));
-        PE_CUDA(c, cudaMemcpyAsync(srate, rh->rate, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
-        PE_CUDA(c, cudaMemcpyAsync(se1, rh->eps_k, (size_t)c->nb1 * 8, cudaMemcpyHostToDevice, c->s_in));
+        PE_CUDA(c, cudaMemcpyAsync(srate, rh->rate, nrate * 8, cudaMemcpyHostToDevice, c->s_in));
+        PE_CUDA(c, cudaMemcpyAsync(se1, rh->eps_k, nrate * 8, cudaMemcpyHostToDevice, c->s_in));
         PE_CUDA(c, cudaMemcpyAsync(se2, rh->eps_kq, (size_t)nq * nb2 * 8, cudaMemcpyHostToDevice, c->s_in));
     }
     PE_CUDA(c, cudaEventRecord(c->ev_in[slot], c->s_in));
@@ -1024,17 +1029,18 @@ int async_batch(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, const double* q_hos
     PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in[slot], 0));
     if (reuse) PE_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out[slot], 0));
     int rc;
+    const int rows_per_k = nk_stack > 0 ? nq / nk_stack : 0;
     if (rh) {
         RateReq rr{se1, se2, rh->prm, srate};
-        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, out_host ? so : nullptr, &rr);
+        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, out_host ? so : nullptr, &rr, rows_per_k, slot0);
     } else {
-        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so);
+        rc = run_q_batch(c, nq, nb2, sq, sU, sZ, sw, so, nullptr, rows_per_k, slot0);
     }
     if (rc) return rc;
     PE_CUDA(c, cudaEventRecord(c->ev_done[slot], c->stream));
     // copy-out stream
     PE_CUDA(c, cudaStreamWaitEvent(c->s_out, c->ev_done[slot], 0));
-    if (rh) PE_CUDA(c, cudaMemcpyAsync(rh->rate, srate, (size_t)c->nb1 * 8, cudaMemcpyDeviceToHost, c->s_out));
+    if (rh) PE_CUDA(c, cudaMemcpyAsync(rh->rate, srate, nrate * 8, cudaMemcpyDeviceToHost, c->s_out));
     if (out_host)
         PE_CUDA(c, cudaMemcpyAsync(out_host, so, (size_t)nq * c->nb1 * nb2 * d.nmodes * 8, cudaMemcpyDeviceToHost, c->s_out));
     PE_CUDA(c, cudaEventRecord(c->ev_out[slot], c->s_out));
@@ -1072,6 +1078,76 @@ int phoebe_elph_q_batch_rates_host_async(phoebe_elph_ctx* c, int32_t nq, int32_t
     if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_host_async: kT and sigma must be > 0");
     RateHost rh{eps_k_host, eps_kq_host, *prm, rate_host};
     return async_batch(c, nq, nb2, q_host, Ukq_host, ev_host, omega_host, out_host, &rh);
+}
+
+namespace {
+int check_multi(phoebe_elph_ctx* c, const char* who, int32_t nk, int32_t nq, int32_t nb2)
+{
+    if (!c->have_k) return fail(c, PHOEBE_ELPH_E_NO_K, "stacked q_batch before set_k_batch");
+    if (nk <= 0 || nk > c->nk_have) return fail(c, PHOEBE_ELPH_E_DIMS, "stacked q_batch: nk exceeds the k slots of the last set_k_batch");
+    if (nq < 0 || (nq % 64) != 0) return fail(c, PHOEBE_ELPH_E_DIMS, "stacked q_batch: nq must be a multiple of 64");
+    if ((long long)nk * nq > c->dims.nq_max) return fail(c, PHOEBE_ELPH_E_DIMS, "stacked q_batch: nk*nq exceeds nq_max");
+    if (nb2 <= 0 || nb2 > c->dims.nb2_max) return fail(c, PHOEBE_ELPH_E_DIMS, "stacked q_batch: nb2 out of range");
+    if (c->nG > 0) return fail(c, PHOEBE_ELPH_E_DIMS, "stacked q_batch: not available while the polar term is on");
+    (void)who;
+    return PHOEBE_ELPH_OK;
+}
+// k slots per pipelined chunk of a stacked host call: the fewest whose stacked rows still fill the GPU for ~8 rounds of
+// contraction tiles (a chunk is one contraction launch) -- many small chunks keep the un-overlapped first copy-in and last
+// copy-out of a call short (4-atom workload, 16 slots: chunks of 4 -> 1.63 M pairs/s end to end, chunks of 1 -> see bench)
+int multi_chunk_slots(const phoebe_elph_ctx* c, int nk, int nq)
+{
+    const long ntn = ceil_div(c->nb1 * c->dims.nw * c->dims.nmodes, 64);
+    const long min_rows = std::max<long>(64, (8L * kSMs + ntn - 1) / ntn * 64);      // rows of ~8 rounds of 64 x 64 tiles
+    int kc = 1;
+    while (kc < nk && (long)kc * nq < min_rows) ++kc;
+    return kc;
+}
+}  // namespace
+
+int phoebe_elph_q_batch_multi_host_async(phoebe_elph_ctx* c, int32_t nk, int32_t nq, int32_t nb2, const double* q_host,
+                                         const void* Ukq_host, const void* ev_host, const double* omega_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !out_host) return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_multi_host_async: null pointer");
+    if (int rc = check_multi(c, "q_batch_multi_host_async", nk, nq, nb2)) return rc;
+    if (nq == 0) return PHOEBE_ELPH_OK;
+    const phoebe_elph_dims& d = c->dims;
+    const int kc = multi_chunk_slots(c, nk, nq);
+    for (int j0 = 0; j0 < nk; j0 += kc) {          // chunks of k slots: the copies of one chunk overlap the kernels of its neighbours
+        const int nkc = std::min(kc, nk - j0);
+        const size_t r0 = (size_t)j0 * nq;
+        int rc = async_batch(c, nkc * nq, nb2, q_host + r0 * 3, static_cast<const char*>(Ukq_host) + r0 * d.nw * nb2 * 16,
+                             static_cast<const char*>(ev_host) + r0 * d.nmodes * d.nmodes * 16, omega_host + r0 * d.nmodes,
+                             out_host + r0 * c->nb1 * nb2 * d.nmodes, nullptr, nkc, j0);
+        if (rc) return rc;
+    }
+    return PHOEBE_ELPH_OK;
+}
+
+int phoebe_elph_q_batch_rates_multi_host_async(phoebe_elph_ctx* c, int32_t nk, int32_t nq, int32_t nb2, const double* q_host,
+                                               const void* Ukq_host, const void* ev_host, const double* omega_host,
+                                               const double* eps_k_host, const double* eps_kq_host,
+                                               const phoebe_elph_rate_params* prm, double* rate_host, double* out_host)
+{
+    if (!c) return PHOEBE_ELPH_E_NULL;
+    if (!q_host || !Ukq_host || !ev_host || !omega_host || !eps_k_host || !eps_kq_host || !prm || !rate_host)
+        return fail(c, PHOEBE_ELPH_E_NULL, "q_batch_rates_multi_host_async: null pointer");
+    if (int rc = check_multi(c, "q_batch_rates_multi_host_async", nk, nq, nb2)) return rc;
+    if (!(prm->kT > 0.0) || !(prm->sigma > 0.0)) return fail(c, PHOEBE_ELPH_E_DIMS, "q_batch_rates_multi_host_async: kT and sigma must be > 0");
+    if (nq == 0) return PHOEBE_ELPH_OK;
+    const phoebe_elph_dims& d = c->dims;
+    const int kc = multi_chunk_slots(c, nk, nq);
+    for (int j0 = 0; j0 < nk; j0 += kc) {
+        const int nkc = std::min(kc, nk - j0);
+        const size_t r0 = (size_t)j0 * nq;
+        RateHost rh{eps_k_host + (size_t)j0 * c->nb1, eps_kq_host + r0 * nb2, *prm, rate_host + (size_t)j0 * c->nb1};
+        int rc = async_batch(c, nkc * nq, nb2, q_host + r0 * 3, static_cast<const char*>(Ukq_host) + r0 * d.nw * nb2 * 16,
+                             static_cast<const char*>(ev_host) + r0 * d.nmodes * d.nmodes * 16, omega_host + r0 * d.nmodes,
+                             out_host ? out_host + r0 * c->nb1 * nb2 * d.nmodes : nullptr, &rh, nkc, j0);
+        if (rc) return rc;
+    }
+    return PHOEBE_ELPH_OK;
 }
 
 int phoebe_elph_wait(phoebe_elph_ctx* c)
@@ -1151,7 +1227,7 @@ int phoebe_elph_q_batch_rates_host(phoebe_elph_ctx* c, int32_t nq, int32_t nb2, 
     double* sw = reinterpret_cast<double*>(c->ws + c->L.off_som);
     double* so = reinterpret_cast<double*>(c->ws + c->L.off_sout);
     double* srate = reinterpret_cast<double*>(c->ws + c->L.off_rate);
-    double* se1 = srate + d.nb1_max;
+    double* se1 = srate + (size_t)c->L.nk_slots * d.nb1_max;
     double* se2 = reinterpret_cast<double*>(c->ws + c->L.off_seps);
     PE_CUDA(c, cudaMemcpyAsync(sq, q_host, (size_t)nq * 24, cudaMemcpyHostToDevice, c->stream));
     PE_CUDA(c, cudaMemcpyAsync(sU, Ukq_host, (size_t)nq * d.nw * nb2 * 16, cudaMemcpyHostToDevice, c->stream));

@@ -224,3 +224,69 @@ def test_rates_multi_equals_oracle_per_k(env, shape):
         rk, _ = ctx.q_batch_rates(*dk, **P)
         assert _relerr(rk.cpu().numpy(), ref) <= TOL
     ctx.close()
+
+
+def test_stacked_host_async_pipelines_k_batches(env):
+    """phoebe_elph_q_batch_multi_host_async / _rates_multi_host_async: four k batches of three k-points each, the
+    k-stacked pinned arrays of a batch per call, batches pipelined over the two staging slots with the NEXT
+    set_k_batch_host issued while the previous batch's results are still being copied out; |g|^2 and linewidths of
+    every (batch, k) against the oracle after wait()."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    nk, nbatch, nq = 3, 4, 128
+    w = wl.custom(nw=5, nb1=4, nb2=5, nm=6, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nk=nk * nbatch, nq=nq, cfg_id=98)
+    gW_np, ks = wl.gW_full(w), wl.k_points(w)
+    ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=nk * nq, nk_max=nk)
+    P = dict(wl.RATE_PARAMS)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    cases = [_case(wl, w, ik) for ik in range(nk * nbatch)]
+    st = lambda b, key: pin(np.stack([cases[b * nk + j][key] for j in range(nk)]))
+    held = []
+    for b in range(nbatch):
+        Uks = np.stack([cases[b * nk + j]["Uk"] for j in range(nk)])
+        ctx.set_k_batch_host(ks[b * nk:(b + 1) * nk], Uks)
+        ins = [st(b, key) for key in ("q", "Ukq", "ev", "om")]
+        out = torch.empty((nk, nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory()
+        if b % 2 == 0:
+            ctx.q_batch_multi_host_async(*[t.numpy() for t in ins], out.numpy())
+            held.append((b, ins, out, None))
+        else:
+            eps = [st(b, "eps_k"), st(b, "eps_kq")]
+            rate = torch.zeros((nk, w.nb1), dtype=torch.float64).pin_memory()
+            ctx.q_batch_rates_multi_host_async(*[t.numpy() for t in ins], eps[0].numpy(), eps[1].numpy(), rate.numpy(),
+                                               out=out.numpy() if b == 1 else None, **P)
+            held.append((b, ins + eps, out if b == 1 else None, rate))
+    ctx.wait()
+    for b, _, out, rate in held:
+        for j in range(nk):
+            rref, oref = _oracle_rates(oracle, cases[b * nk + j], P)
+            if out is not None:
+                assert _relerr(out.numpy()[j], oref) <= TOL
+            if rate is not None:
+                assert _relerr(rate.numpy()[j], rref) <= TOL
+    ctx.close()
+
+
+def test_rates_async_copy_out_outlasts_copy_in(env):
+    """Six pipelined q_batch_rates_host_async batches WITH |g|^2 copied out (3 MB per batch against 0.3 MB copied in):
+    the copy-out of batch n-2 is still running when the inputs of batch n arrive.  Each call has its own initial rate
+    values; a copy-in that overtook the copy-out of the rate staging buffer would hand back the wrong batch's sums."""
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    w = wl.custom(nw=8, nb1=8, nb2=8, nm=6, grid_e=(2, 2, 1), grid_p=(3, 3, 1), nk=1, nq=1024, cfg_id=99)
+    a = _case(wl, w, 0)
+    P = dict(wl.RATE_PARAMS)
+    ctx = harness.make_context(w, torch.from_numpy(a["gW"]).cuda(), nq_max=w.nq)
+    ctx.set_k_host(a["k"], a["Uk"])
+    pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+    ins = [pin(a[key]) for key in ("q", "Ukq", "ev", "om", "eps_k", "eps_kq")]
+    rref, oref = _oracle_rates(oracle, a, P)
+    held = []
+    for n in range(6):
+        rate = pin(np.full(w.nb1, 1e-3 * (n + 1)))
+        out = torch.empty((w.nq, w.nb1, w.nb2, w.nm), dtype=torch.float64).pin_memory()
+        ctx.q_batch_rates_host_async(*[t.numpy() for t in ins], rate.numpy(), out=out.numpy(), **P)
+        held.append((n, rate, out))
+    ctx.wait()
+    for n, rate, out in held:
+        assert _relerr(rate.numpy() - 1e-3 * (n + 1), rref) <= 1e-9
+        assert _relerr(out.numpy(), oref) <= TOL
+    ctx.close()
