@@ -336,15 +336,6 @@ int phoebe_elph_destroy(phoebe_elph_ctx* ctx);
 /* Text of the last error on this context ("" if none); valid until the next call on ctx. */
 const char* phoebe_elph_last_error(const phoebe_elph_ctx* ctx);
 
-/* FP64 ceiling probes used for the roofline denominators: runs a
- * register-resident loop of dependent-free FP64 FMAs (kind 0: DFMA, kind 1: mma.sync
- * m8n8k4 DMMA) on every SM for `iters` iterations and writes the achieved TFLOP/s.
- * Synchronises the stream.  Errors: E_NULL, E_DIMS, E_CUDA. */
-int phoebe_elph_probe_fp64(int32_t kind, int32_t iters, void* cuda_stream, double* tflops_out);
-
-/* HBM read-stream probe: sums `bytes` of DEVICE memory with 128-bit loads; writes GB/s. */
-int phoebe_elph_probe_hbm_read(const void* buf_dev, size_t bytes, void* cuda_stream, double* gbs_out);
-
 const char* phoebe_elph_version(void);
 
 #ifdef __cplusplus

@@ -25,7 +25,7 @@ EXPORTS = [
     "phoebe_elph_q_batch_rates_multi", "phoebe_elph_q_batch_multi_host_async", "phoebe_elph_q_batch_rates_multi_host_async",
     "phoebe_elph_copy_g1", "phoebe_elph_g1_buffer", "phoebe_elph_set_polar", "phoebe_elph_set_conventions", "phoebe_elph_launch_counts",
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
-    "phoebe_elph_destroy", "phoebe_elph_last_error", "phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read",
+    "phoebe_elph_destroy", "phoebe_elph_last_error",
     "phoebe_elph_version",
 ]
 
@@ -94,8 +94,6 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_destroy.argtypes = [c_void_p]
     lib.phoebe_elph_last_error.argtypes = [c_void_p]
     lib.phoebe_elph_last_error.restype = c_char_p
-    lib.phoebe_elph_probe_fp64.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
-    lib.phoebe_elph_probe_hbm_read.argtypes = [c_void_p, c_size_t, c_void_p, POINTER(c_double)]
     lib.phoebe_elph_version.restype = c_char_p
     _lib = lib
     return lib
@@ -455,11 +453,29 @@ class ElphContext:
         return int(v.value)
 
 
+#: every symbol declared in include/phoebe_elph_probes.h (libphoebe_elph_probes.so: measurement aids, not the product)
+PROBE_EXPORTS = ["phoebe_elph_probe_fp64", "phoebe_elph_probe_hbm_read"]
+PROBES_LIB_PATH = os.path.join(HERE, "libphoebe_elph_probes.so")
+_probes = None
+
+
+def load_probes() -> ctypes.CDLL:
+    global _probes
+    if _probes is None:
+        if not os.path.exists(PROBES_LIB_PATH):
+            raise FileNotFoundError(f"{PROBES_LIB_PATH} not built; run `python -m paper_2111_14999_b200.build`")
+        lib = ctypes.CDLL(PROBES_LIB_PATH)
+        lib.phoebe_elph_probe_fp64.argtypes = [c_int32, c_int32, c_void_p, POINTER(c_double)]
+        lib.phoebe_elph_probe_hbm_read.argtypes = [c_void_p, c_size_t, c_void_p, POINTER(c_double)]
+        _probes = lib
+    return _probes
+
+
 def probe_fp64(kind: str = "dmma", iters: int = 20000, stream=None) -> float:
     """FP64 ceiling in TFLOP/s measured on this device (kind: 'dfma' | 'dmma')."""
     t = c_double(0.0)
     st = None if stream is None else stream.cuda_stream
-    rc = load_library().phoebe_elph_probe_fp64({"dfma": 0, "dmma": 1}[kind], iters, st, byref(t))
+    rc = load_probes().phoebe_elph_probe_fp64({"dfma": 0, "dmma": 1}[kind], iters, st, byref(t))
     if rc:
         raise PhoebeElphError(rc, "phoebe_elph_probe_fp64")
     return float(t.value)
@@ -469,7 +485,7 @@ def probe_hbm_read(buf, stream=None) -> float:
     """HBM read-stream bandwidth in GB/s over a CUDA tensor."""
     t = c_double(0.0)
     st = None if stream is None else stream.cuda_stream
-    rc = load_library().phoebe_elph_probe_hbm_read(buf.data_ptr(), buf.numel() * buf.element_size(), st, byref(t))
+    rc = load_probes().phoebe_elph_probe_hbm_read(buf.data_ptr(), buf.numel() * buf.element_size(), st, byref(t))
     if rc:
         raise PhoebeElphError(rc, "phoebe_elph_probe_hbm_read")
     return float(t.value)

@@ -14,6 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = os.path.join(HERE, "csrc", "phoebe_elph.cu")
 LIB = os.path.join(HERE, "libphoebe_elph.so")
+PROBES_SRC = os.path.join(HERE, "csrc", "probes.cu")
+PROBES_LIB = os.path.join(HERE, "libphoebe_elph_probes.so")      # measurement aids of bench.py, not the product
 
 
 def _deps():
@@ -43,12 +45,14 @@ def nvcc_cmds(verbose: bool = False):
     objs = [os.path.join(OBJ_DIR, "phoebe_elph.o")] + [os.path.join(OBJ_DIR, "rot3_part%d.o" % i) for i in range(ROT3_PARTS)]
     compiles = [base + ["-c", SRC, "-o", objs[0]]]
     compiles += [base + ["-DROT3_PART=%d" % i, "-c", ROT3_SRC, "-o", objs[1 + i]] for i in range(ROT3_PARTS)]
+    compiles.append(base + ["-shared", "-o", PROBES_LIB, PROBES_SRC])
     link = [base[0], "-shared", "-o", LIB] + objs
     return compiles, link
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
+    if (not force and os.path.exists(LIB) and os.path.exists(PROBES_LIB)
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps())):
         return LIB
     import concurrent.futures as cf
     os.makedirs(OBJ_DIR, exist_ok=True)

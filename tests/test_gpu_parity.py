@@ -432,3 +432,56 @@ def test_q_batch_multi_equals_per_k_calls(env, knob):
             ctx.q_batch_multi(*bad)
         assert e.value.code == -2
     ctx.close()
+
+
+def test_two_contexts_on_two_threads(env):
+    """Two contexts, each on its own host thread and CUDA stream, through the whole path at the same time (different
+    shapes, so different kernel instantiations and shared-memory opt-ins race for the per-device attribute table):
+    both against the oracle, repeated so that first-use initialisation overlaps."""
+    import threading
+    wl, oracle, torch, harness = env["wl"], env["oracle"], env["torch"], env["harness"]
+    shapes = [dict(nw=6, nb1=5, nb2=6, nm=9, grid_e=(3, 2, 2), grid_p=(3, 3, 2), nq=300, cfg_id=181),
+              dict(nw=16, nb1=16, nb2=16, nm=12, grid_e=(2, 2, 1), grid_p=(3, 3, 1), nq=200, cfg_id=182)]
+    cases = []
+    for sh in shapes:
+        w = wl.custom(**sh)
+        a = _inputs(wl, w)
+        a["w"] = w
+        a["ref"] = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+        cases.append(a)
+    errs, excs = [None, None], []
+    start = threading.Barrier(2)
+
+    def worker(i):
+        try:
+            a = cases[i]
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                gW = torch.from_numpy(a["gW"]).cuda()
+                d = harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])
+                (Uk_d,) = harness.to_device([a["Uk"]])
+                st.synchronize()
+                start.wait()
+                worst = 0.0
+                for rep in range(5):
+                    ctx = harness.make_context(a["w"], gW, nq_max=a["w"].nq)      # binds torch's current stream (st)
+                    ctx.set_k(a["k"], Uk_d)
+                    out = ctx.q_batch(*d)
+                    st.synchronize()
+                    worst = max(worst, _relerr(out.cpu().numpy(), a["ref"]))
+                    ctx.close()
+                errs[i] = worst
+        except Exception as exc:          # surfaced in the main thread
+            excs.append(exc)
+            try:
+                start.abort()
+            except Exception:
+                pass
+
+    ts = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join(120)
+    assert not excs, excs
+    assert errs[0] is not None and errs[0] <= TOL and errs[1] is not None and errs[1] <= TOL, errs

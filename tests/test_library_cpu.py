@@ -25,6 +25,17 @@ def test_every_declared_symbol_is_exported(lib):
     assert declared == set(binding.EXPORTS)
     for name in declared:
         assert getattr(lib, name) is not None
+    # ... and nothing else: the product ABI is the hot path's calls, measurement aids live in their own library
+    import subprocess
+    syms = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    exported = set(re.findall(r" T (phoebe_elph_[a-z0-9_]+)", syms))
+    assert exported == declared, exported ^ declared
+    probes = binding.load_probes()
+    pheader = open(os.path.join(ROOT, "include", "phoebe_elph_probes.h")).read()
+    pdecl = set(re.findall(r"\b(phoebe_elph_[a-z0-9_]+)\s*\(", pheader))
+    assert pdecl == set(binding.PROBE_EXPORTS)
+    for name in pdecl:
+        assert getattr(probes, name) is not None
 
 
 def test_version(lib):
@@ -97,7 +108,7 @@ def test_no_cpu_fallback(lib):
     rc = lib.phoebe_elph_setup(ctypes.byref(ctx), 0x1000, Re, Re, None, None, ctypes.byref(d), 0x10000, 1 << 30, None)
     assert rc == -6 and not ctx.value
     t = ctypes.c_double(0)
-    assert lib.phoebe_elph_probe_fp64(1, 10, None, ctypes.byref(t)) == -6
+    assert binding.load_probes().phoebe_elph_probe_fp64(1, 10, None, ctypes.byref(t)) == -6
     import numpy as np
     with pytest.raises(binding.PhoebeElphError) as e:
         binding.ElphContext(torch.zeros((1, 1, 1, 1, 1), dtype=torch.complex128), np.zeros((1, 3)), np.zeros((1, 3)),
