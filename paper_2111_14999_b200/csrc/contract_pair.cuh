@@ -57,39 +57,50 @@ k_pack_pair(const double2* __restrict__ src, long long ld, long long strideS, in
         const int ib = pb[r];
         const double2 b = ib >= 0 ? s[(size_t)ib * ld] : make_double2(0.0, 0.0);
         if (kind[r] == 0) v = make_double2(a.x + b.x, a.y + b.y);
-        else v = make_double2(-(a.y - b.y), a.x - b.x);
+        else if (kind[r] == 1) v = make_double2(-(a.y - b.y), a.x - b.x);
+        else v = make_double2(0.0, 0.0);                       // padding row between the cosine and the sine block
     }
     double* d = dst + (size_t)slot * strideD + ((size_t)r * gridDim.x + tile) * PairCfg::ROWB + c;
     d[0] = v.x; d[64] = v.y;
 }
 
-// A rows: AtR[r][q] = w[r] * (trig[r] ? sgn * sin : cos)(2 pi q . Rrow[r]); zero for r >= Kr or q >= nq.
-// Rows come in (cos, sin) pairs of the same lattice vector for r < 2*K2 and as single cos rows behind them (host
-// contract, phoebe_elph_setup): one sincospi serves both rows of a pair.  blockIdx.y strides over row PAIRS.
+// Row order of the pair form (host contract, phoebe_elph_setup): a COSINE block -- one row per (+R, -R) pair or
+// partner-less vector (K2 of them), then one per self-inverse vector (R = 0), zero rows up to a multiple of 4 (Kc4) --
+// followed by the SINE block, one row per pair in the same order: row Kc4 + sl belongs to cosine row sl.  The cosine
+// rows are even in q and the sine rows odd, which is what the q <-> -q fold below uses.
+//
+// A rows: AtR[r][col] = w[r] * cos(2 pi q . R[r]) (r < Kc) or w * sgn * sin(2 pi q . R[r - Kc4]); zero for padding rows and
+// for columns >= nq.  One sincospi serves both rows of a pair.  blockIdx.y strides over cosine rows.
+// qidx != nullptr: column col takes q-point qidx[col] (the representatives of the q <-> -q fold), and the number of
+// columns is *ncol_dev; `run` (device flag, may be nullptr) == 0 makes the launch a no-op.
 __global__ void __launch_bounds__(256)
-k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rrow /* [Kr][3] */,
-              const double* __restrict__ wrow, int K2, int nq, int Kr, int KrPad, int ldq,
-              double sgn, double* __restrict__ AtR /* [KrPad][ldq] */)
+k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restrict__ Rrow /* [Kc][3] */,
+              const double* __restrict__ wrow, int K2, int Kc, int Kc4, int nq, int Kr, int KrPad, int ldq,
+              double sgn, double* __restrict__ AtR /* [KrPad][ldq] */, const int* __restrict__ qidx,
+              const int* __restrict__ ncol_dev, const int* __restrict__ run, int run_when)
 {
-    const int iq = blockIdx.x * blockDim.x + threadIdx.x;
-    if (iq >= ldq) return;
+    if (run != nullptr && (*run != 0) != (run_when != 0)) return;
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= ldq) return;
+    if (ncol_dev != nullptr) nq = *ncol_dev;
     double q0 = 0.0, q1 = 0.0, q2 = 0.0;
-    const bool valid = iq < nq;
-    if (valid) { q0 = q[3 * (size_t)iq]; q1 = q[3 * (size_t)iq + 1]; q2 = q[3 * (size_t)iq + 2]; }
-    const int nslots = K2 + (KrPad - 2 * K2);            // K2 two-row slots, then one slot per remaining (single or padding) row
-    for (int sl = blockIdx.y; sl < nslots; sl += gridDim.y) {
-        const bool two = sl < K2;
-        const int r = two ? 2 * sl : sl + K2;
+    const bool valid = col < nq;
+    if (valid) {
+        const size_t iq = qidx != nullptr ? (size_t)qidx[col] : (size_t)col;
+        q0 = q[3 * iq]; q1 = q[3 * iq + 1]; q2 = q[3 * iq + 2];
+    }
+    for (int r = blockIdx.y; r < Kc4; r += gridDim.y) {
         double vc = 0.0, vs = 0.0;
-        if (valid && r < Kr) {
+        if (valid && r < Kc) {
             const double x = q0 * Rrow[3 * r] + q1 * Rrow[3 * r + 1] + q2 * Rrow[3 * r + 2];
             double sn, cs;
             sincospi(2.0 * x, &sn, &cs);
             vc = wrow[r] * cs; vs = wrow[r] * sgn * sn;
         }
-        AtR[(size_t)r * ldq + iq] = vc;
-        if (two) AtR[(size_t)(r + 1) * ldq + iq] = vs;
+        AtR[(size_t)r * ldq + col] = vc;
+        if (r < K2) AtR[(size_t)(Kc4 + r) * ldq + col] = vs;
     }
+    for (int r = Kr + blockIdx.y; r < KrPad; r += gridDim.y) AtR[(size_t)r * ldq + col] = 0.0;
 }
 
 // AtR, BP2 as above (BP2 of k slot 0; slot j at + j*strideBslot doubles); C [M][ldc] complex; K = Kr, Kpad = KrPad.

@@ -104,10 +104,10 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_Tpart = take((size_t)std::max(L.S_alloc, L.nk_slots) * d.nRp * X * 16);
     L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
     // planar blocked copies ([rows][tiles of 64][3][64] doubles) of g1' and of the phases for k_contract_planar
-    L.g1P_stride = (size_t)d.nRp * ceil_div((int)N, 64) * 192;
+    L.g1P_stride = ((size_t)d.nRp * 192 + 384) * ceil_div((int)N, 64);     // (+ 3 padding rows of the pair form)
     L.off_g1P = take((size_t)L.nk_slots * L.g1P_stride * 8);
     // +R / -R pair map of the Rp list for k_contract_pair: 3 int + 4 double per real row, at most 2 nRp rows
-    L.off_pair = take((size_t)2 * d.nRp * (3 * 4 + 4 * 8));
+    L.off_pair = take((size_t)(2 * d.nRp + 4) * (3 * 4 + 4 * 8));
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_PtP = take((size_t)L.Kpad * L.ldq * 24);
     L.off_C = take((size_t)L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16);
@@ -185,7 +185,9 @@ struct phoebe_elph_ctx {
     double *g1P = nullptr, *PtP = nullptr;   // planar blocked operands of k_contract_planar
     bool planar = true;       // tuning "planar": a4 through k_contract_planar (default) or k_contract
     // k_contract_pair: the Rp list folded into Kr real rows (pair_Kr == 0: not usable); g1P then holds the pair form
-    int pair_Kr = 0, pair_KrPad = 0, pair_K2 = 0;   // K2 = (cos, sin) row pairs; single cos rows (R = 0) follow them
+    int pair_Kr = 0, pair_KrPad = 0, pair_K2 = 0;   // K2 = (cos, sin) row pairs
+    int pair_Kc = 0, pair_Kc4 = 0;                  // cosine rows (pairs + self-inverse vectors), padded to a multiple of 4
+    bool rp_integer = false;
     int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
     int pair_ctas = 1;        // tuning "pair_ctas": persistent CTAs of k_contract_pair per SM (its ring is 100 KB: two fit)
     int last_pair = -1;       // did the last contraction launch use the pair form (-1: no launch yet)
@@ -602,9 +604,10 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
             if (use_pair) {
-                dim3 grid(ceil_div(ncols, 256), std::min(c->pair_KrPad - c->pair_K2, 64));
-                pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, nqs,
-                                                               c->pair_Kr, c->pair_KrPad, c->L.ldq, c->phase_sign, c->PtP);
+                dim3 grid(ceil_div(ncols, 256), std::min(c->pair_Kc4, 64));
+                pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc,
+                                                               c->pair_Kc4, nqs, c->pair_Kr, c->pair_KrPad, c->L.ldq,
+                                                               c->phase_sign, c->PtP, nullptr, nullptr, nullptr, 0);
             } else {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
                 pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
@@ -803,8 +806,9 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
     up(c->Rp, Rp_host, (size_t)dims->nRp * 24);
     up(c->deg_e, deg_e_host ? deg_e_host : ones.data(), (size_t)dims->nRe * 8);
     up(c->deg_p, deg_p_host ? deg_p_host : ones.data(), (size_t)dims->nRp * 8);
-    // ---- +R / -R pair map of the Rp list (contract_pair.cuh): groups of two real rows (cos | sin) for a pair or a
-    // vector without partner, then one row (cos) per self-inverse vector (R = 0) ----
+    // ---- +R / -R pair map of the Rp list (contract_pair.cuh): a cosine block (one row per pair or vector without
+    // partner, then one per self-inverse vector R = 0, zero rows up to a multiple of 4) and a sine block (one row per
+    // pair, same order) ----
     std::vector<int> h_pa, h_pb, h_kind;
     std::vector<double> h_R, h_w;
     {
@@ -822,6 +826,7 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
             h_R.push_back(Rp_host[3 * a]); h_R.push_back(Rp_host[3 * a + 1]); h_R.push_back(Rp_host[3 * a + 2]);
             h_w.push_back(1.0 / wt(a));
         };
+        std::vector<std::pair<int, int>> pairs;
         for (int p = 0; p < nRp; ++p) {
             if (used[p]) continue;
             used[p] = 1;
@@ -829,19 +834,25 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
             int partner = -1;
             auto it = first.find(key(p, -1.0));
             if (it != first.end() && !used[it->second] && wt(it->second) == wt(p)) { partner = it->second; used[partner] = 1; }
-            row(p, partner, 0);
-            row(p, partner, 1);
+            pairs.push_back({p, partner});
         }
-        c->pair_K2 = (int)h_pa.size() / 2;
+        for (auto& pr : pairs) row(pr.first, pr.second, 0);
+        c->pair_K2 = (int)pairs.size();
         for (int p : selfs) row(p, -1, 0);
+        c->pair_Kc = (int)h_pa.size();
+        while (h_pa.size() % 4) row(0, -1, 2);                  // zero rows: the sine block starts at a k-step boundary
+        c->pair_Kc4 = (int)h_pa.size();
+        for (auto& pr : pairs) row(pr.first, pr.second, 1);
         c->pair_Kr = (int)h_pa.size();
+        c->rp_integer = true;                                   // q -> q + G leaves the phases alone only for integer Rp
+        for (int i = 0; i < 3 * nRp; ++i) if (Rp_host[i] != std::floor(Rp_host[i])) c->rp_integer = false;
         c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, (size_t)std::max(kKPad, pe::PairCfg::KC));
         // the pair form reuses the planar buffers: rows must fit them (g1P: Kr*128 <= nRp*192 doubles per tile column,
         // PtP: KrPad*8 <= Kpad*24 bytes per q)
-        if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
+        if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 + 384 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
         if (c->pair_Kr > 0) {
             char* base = c->ws + L.off_pair;
-            const size_t cap = (size_t)2 * nRp;
+            const size_t cap = (size_t)2 * nRp + 4;
             c->pair_pa = reinterpret_cast<int*>(base);
             c->pair_pb = c->pair_pa + cap;
             c->pair_kind = c->pair_pb + cap;

@@ -32,11 +32,11 @@ def _inputs(wl, w, ik=0):
                 q=wl.q_points(w, ik), Ukq=wl.U_kq(w, ik), ev=wl.ph_eigvecs(w, ik), om=wl.omega(w, ik))
 
 
-#        grid_p      deg_p      pair  expected real rows (None = only check > nRp)
-CASES = [((3, 3, 3), None, 1, 27),            # symmetric: 13 pairs x 2 + R = 0
-         ((5, 3, 1), None, 1, 15),
-         ((3, 3, 3), "broken", 1, 31),         # unequal weights inside two pairs -> those four vectors have no partner
-         ((3, 3, 3), "symmetric", 1, 27),      # non-trivial but inversion-symmetric degeneracies
+#        grid_p      deg_p      pair  expected real rows (None = only check > nRp): cosine block padded to 4 + sine block
+CASES = [((3, 3, 3), None, 1, 29),            # symmetric: 13 pairs + R = 0 -> 14 -> 16 cosine rows, 13 sine rows
+         ((5, 3, 1), None, 1, 15),            # 7 pairs + R = 0 -> 8, + 7
+         ((3, 3, 3), "broken", 1, 31),         # unequal weights inside two pairs -> those four vectors have no partner: 15 + 1, + 15
+         ((3, 3, 3), "symmetric", 1, 29),      # non-trivial but inversion-symmetric degeneracies
          ((2, 3, 1), None, 2, None),           # x in {-1, 0}: the x = -1 vectors have no partner
          ((4, 1, 1), None, 2, None)]
 
@@ -141,7 +141,7 @@ def test_non_integer_lattice_vectors(env, kind, pair):
     ref = oracle.elph(gW, Re, Rp, None, None, k, Uk, q, Ukq, ev, om)
     out, rows = _run_custom_lists(env, gW, Re, Rp, None, k, Uk, q, Ukq, ev, om, pair)
     if kind == "symmetric" and pair:
-        assert rows == nRp
+        assert rows == 8 + 5          # 5 pairs + the origin -> 6 -> 8 cosine rows, 5 sine rows
     assert _relerr(out, ref) <= TOL
 
 
