@@ -70,7 +70,8 @@ enum {
     PHOEBE_ELPH_K_RATE_REDUCE = 6,  /* f2: fixed-order sum of the per-CTA linewidth partials    */
     PHOEBE_ELPH_K_POLAR       = 7,  /* f4: (q, nu) amplitudes of the polar long-range term        */
     PHOEBE_ELPH_K_PACK        = 8,  /* g1' -> planar blocked operand of the planar contraction    */
-    PHOEBE_ELPH_K_COUNT       = 9
+    PHOEBE_ELPH_K_QFOLD       = 9,  /* a4 on inversion-symmetric q lists: detection of the (q, -q) pairs  */
+    PHOEBE_ELPH_K_COUNT       = 10
 };
 
 /* Size the workspace (L576: "the size of the set {k'} is optimized at runtime so
@@ -323,6 +324,14 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               pairs (4 Kr < 6 nRp, Kr = real rows: 2 per pair or partner-less vector, 1 for R = 0); 0 = never; 2 = whenever
  *               the rows fit the operand buffers (Kr <= 1.5 nRp).  get_tuning("pair_rows") = Kr if the last contraction
  *               launch used the form, else 0.   "pair_ctas" 1 | 2 = persistent CTAs per SM of that kernel
+ *   "qfold"     1 = q lists that contain -q with q (uniform meshes; modulo a reciprocal lattice vector when all Rp are
+ *               integer vectors) are contracted once per (q, -q) pair: the cosine rows of the pair form are even in q, the
+ *               sine rows odd, C(+-q) = Ce +- Co.  The pairs are found on the device in every q_batch call (no host round
+ *               trip; coordinates must match EXACTLY in binary, e.g. i/2^m meshes); lists with < 25 % of their q-points
+ *               paired, the stacked forms and lists of < 256 q-points take the plain path.  0 (default) = off: the
+ *               single-CTA pair search (24 us for 4096 q, 0.35 ms for 32768 q) costs more than the halved contraction
+ *               saves at the sizes measured.  get_tuning("qfold_reps") = representatives of the
+ *               LAST q_batch call if it took the fold, else 0 (synchronises the stream)
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
  *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the geometry of the tensor-core rotation kernel (rotate_v3.cuh):
  *               q-points per ring stage, b1 per C stage (forces the two-ring form), 8-row tiles of b2 per warp item

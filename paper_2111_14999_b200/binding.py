@@ -14,7 +14,7 @@ from ctypes import POINTER, byref, c_char_p, c_double, c_int32, c_int64, c_size_
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libphoebe_elph.so")
 
-KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm", "rate_reduce", "polar", "pack"]
+KERNEL_KINDS = ["setk_stream", "setk_rotate", "qphase", "contract", "rotate_epilogue", "setk_gemm", "rate_reduce", "polar", "pack", "qfold"]
 
 #: every symbol declared in include/phoebe_elph.h
 EXPORTS = [

@@ -40,6 +40,12 @@ struct PairCfg {
     static constexpr int LDA = ROWA + 4, LDB = ROWB + 4;
     static constexpr size_t kRingBytes = (size_t)STAGES * KC * (LDA + LDB) * sizeof(double);
     static constexpr size_t kSmemBytes = kRingBytes + 2 * STAGES * sizeof(uint64_t);
+    // q <-> -q fold (qfold.cuh): three ring stages + a lane-private copy of the accumulators (the even part Ce of a tile
+    // while the odd part Co is summed): 8 warps x 32 lanes x 32 doubles
+    static constexpr int FOLD_STAGES = 3;
+    static constexpr size_t kFoldRingBytes = (size_t)FOLD_STAGES * KC * (LDA + LDB) * sizeof(double);
+    static constexpr size_t kFoldSaveBytes = (size_t)kConsumerWarps * 32 * TM * TN * 2 * 2 * sizeof(double);
+    static constexpr size_t kFoldSmemBytes = kFoldRingBytes + kFoldSaveBytes + 2 * FOLD_STAGES * sizeof(uint64_t);
 };
 
 // B rows from the canonical g1' [nRp][ld] (+ slot stride): row r = a + b (kind 0) or i (a - b) (kind 1),
@@ -105,22 +111,38 @@ k_qphase_pair(const double* __restrict__ q /* [nq][3] */, const double* __restri
 
 // AtR, BP2 as above (BP2 of k slot 0; slot j at + j*strideBslot doubles); C [M][ldc] complex; K = Kr, Kpad = KrPad.
 // rowsPerB > 0: rows [j*rowsPerB, (j+1)*rowsPerB) of the stacked q lists use slot j (multi-k form, see k_contract).
+//
+// fold.meta != nullptr (qfold.cuh): meta[0] = representatives, meta[1] = whether the q <-> -q fold is taken.
+//   FOLD = false: the plain launch returns at once when the fold is taken.
+//   FOLD = true : returns at once when it is not; else M = meta[0] rows (the columns of AtR are the representatives), the
+//   accumulators are saved at the cosine | sine boundary (row Kc4) and the tile is finished as
+//   C[rep] = Ce + Co, C[mate] = Ce - Co.
+struct FoldArgs { const int* meta; const int* rep_idx; const int* mate; int Kc4; };
+
+template <bool FOLD>
 __global__ void __launch_bounds__(PairCfg::kThreads, 1)
 k_contract_pair(const double* __restrict__ AtR, int lda, const double* __restrict__ BP2, int ntnB, long long strideBslot,
                 double2* __restrict__ C, long long ldc, int M, int N, int K, int Kpad, int rowsPerB, int rowOffset,
-                int panelW, CMap cm)
+                int panelW, CMap cm, FoldArgs fold)
 {
     using Cfg = PairCfg;
-    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = Cfg::STAGES, LDA = Cfg::LDA, LDB = Cfg::LDB;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, STAGES = FOLD ? Cfg::FOLD_STAGES : Cfg::STAGES;
+    constexpr int LDA = Cfg::LDA, LDB = Cfg::LDB;
     constexpr int ROWA = Cfg::ROWA, ROWB = Cfg::ROWB, TM = Cfg::TM, TN = Cfg::TN, KS = KC / 4;
+    constexpr size_t kRingBytes = FOLD ? Cfg::kFoldRingBytes : Cfg::kRingBytes;
+    if (fold.meta != nullptr) {
+        if ((fold.meta[1] != 0) != FOLD) return;
+        if (FOLD) M = fold.meta[0];
+    }
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* As = reinterpret_cast<double*>(smem_raw);                    // [STAGES][KC][LDA]
     double* Bs = As + (size_t)STAGES * KC * LDA;                         // [STAGES][KC][LDB]
-    uint64_t* full = reinterpret_cast<uint64_t*>(Bs + (size_t)STAGES * KC * LDB);
+    double* save = Bs + (size_t)STAGES * KC * LDB;                       // FOLD: [32 accumulator values][256 consumer lanes]
+    uint64_t* full = reinterpret_cast<uint64_t*>(save + (FOLD ? Cfg::kFoldSaveBytes / sizeof(double) : 0));
     uint64_t* empty = full + STAGES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int i = threadIdx.x; i < (int)(Cfg::kRingBytes / sizeof(double2)); i += Cfg::kThreads)
+    for (int i = threadIdx.x; i < (int)(kRingBytes / sizeof(double2)); i += Cfg::kThreads)
         reinterpret_cast<double2*>(As)[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, Cfg::kConsumerWarps); }
@@ -202,6 +224,20 @@ k_contract_pair(const double* __restrict__ AtR, int lda, const double* __restric
             for (int k4 = 0; k4 < KS; ++k4) {
                 const int cur = k4 & 1, nxt = cur ^ 1;
                 if (k4 >= ks_n) break;
+                if (FOLD && c * KC + 4 * k4 == fold.Kc4) {
+                    // cosine | sine boundary: keep the even part Ce of the tile (lane-private slots), start the odd part
+#pragma unroll
+                    for (int i = 0; i < TM; ++i)
+#pragma unroll
+                        for (int j = 0; j < TN; ++j)
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+                                const int e = ((i * TN + j) * 2 + h) * 2;
+                                save[(size_t)e * 256 + threadIdx.x] = cr[i][j][h];
+                                save[(size_t)(e + 1) * 256 + threadIdx.x] = ci[i][j][h];
+                                cr[i][j][h] = 0.0; ci[i][j][h] = 0.0;
+                            }
+                }
                 if (k4 + 1 < KS) {
                     a[nxt][0] = lda2(k4 + 1, 0); a[nxt][1] = lda2(k4 + 1, 1);
                     b[nxt][0] = ldb2(k4 + 1, 0); b[nxt][1] = ldb2(k4 + 1, 1);
@@ -234,6 +270,22 @@ k_contract_pair(const double* __restrict__ AtR, int lda, const double* __restric
         for (int i = 0; i < TM; ++i) {
             const int m = m0 + wm * 32 + 16 * (i >> 1) + 2 * g + (i & 1);
             if (m >= M) continue;
+            if (FOLD) {
+                double2* dst = C + (size_t)fold.rep_idx[m] * ldc;
+                const int im = fold.mate[m];
+                double2* dstm = C + (size_t)max(im, 0) * ldc;
+#pragma unroll
+                for (int cc = 0; cc < 4; ++cc) {
+                    const int j = cc & 1, h = cc >> 1;
+                    const int e = ((i * TN + j) * 2 + h) * 2;
+                    const double er = save[(size_t)e * 256 + threadIdx.x], ei = save[(size_t)(e + 1) * 256 + threadIdx.x];
+                    if (cc < nleft) {
+                        dst[coff[cc]] = make_double2(er + cr[i][j][h], ei + ci[i][j][h]);
+                        if (im >= 0) dstm[coff[cc]] = make_double2(er - cr[i][j][h], ei - ci[i][j][h]);
+                    }
+                }
+                continue;
+            }
             double2* dst = C + (size_t)m * ldc;
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {

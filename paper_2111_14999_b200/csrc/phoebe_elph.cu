@@ -17,6 +17,7 @@
 
 #include "contract_planar.cuh"
 #include "contract_pair.cuh"
+#include "qfold.cuh"
 #include "qbatch_kernels.cuh"
 #include "rotate_v3.cuh"
 #include "setk_kernels.cuh"
@@ -58,7 +59,7 @@ struct Layout {
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t g1P_stride = 0;  // doubles between the planar blocked copies of g1' (k_contract_planar) of consecutive k slots
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
-           off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_fold = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
@@ -113,6 +114,8 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_C = take((size_t)L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16);
     // f2: linewidth partials [nq][groups of b2 tiles][nb1], staging of rate / eps_k / eps_kq for the host entry point
     L.off_part = take((size_t)nq_max * ceil_div(d.nb2_max, 8) * d.nb1_max * 8);
+    // q <-> -q fold: hash table (power of two >= 2 nq, so < 4 nq ints), partner / representative / mate lists, meta
+    L.off_fold = take((size_t)nq_max * (7 * 4 + 8) + 512);
     L.off_rate = take((size_t)2 * 2 * L.nk_slots * d.nb1_max * 8);    // two slots of (rate, eps_k), each [k slots][nb1]
     L.off_seps = take((size_t)2 * nq_max * d.nb2_max * 8);            // two slots of eps_kq
     // f4: G list and Born charges of the polar term, its (q, nu) amplitudes
@@ -170,7 +173,9 @@ struct phoebe_elph_ctx {
     bool rot_plain = false;   // tuning "rot_plain": force the DFMA rotation kernel
     int rot_blk = 0;          // tuning "rot_blk": U_kq / ev staging of the rotation kernel: 0 automatic, 1 row copies, 2 one block per q
     int rot_qg = 0, rot_gb1 = 0, rot_mtw = 0;   // tuning "rot_qg" / "rot_gb1" / "rot_mtw": override the v2 rotation geometry (0 = automatic)
-    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    bool qfold = false;       // tuning "qfold" (opt-in): contract (q, -q) pairs of a q list once (qfold.cuh)
+    bool last_fold = false;   // the last contraction went through the fold-capable launch sequence
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
@@ -601,13 +606,44 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             c->g1P_stale = false;
             c->g1P_form = use_pair ? 2 : 1;
         }
+        // q <-> -q fold (qfold.cuh): the pairs are found on the device; both launch sequences are enqueued and the
+        // kernels of the path not taken return at once
+        const bool try_fold = use_pair && c->qfold && rows_per_k == 0 && nqs >= 256 && c->pair_K2 > 0;
+        int* fold_base = reinterpret_cast<int*>(c->ws + c->L.off_fold);
+        int tsize = 1;
+        while (tsize < 2 * nqs) tsize <<= 1;
+        int* f_meta = fold_base;                 // [2] (+ padding)
+        int* f_partner = fold_base + 64;
+        int* f_rep = f_partner + nqs;
+        int* f_mate = f_rep + nqs;
+        int* f_table = f_mate + nqs;             // [tsize] < 4 nqs
+        unsigned long long* f_fp = reinterpret_cast<unsigned long long*>(
+            c->ws + c->L.off_fold + align_up((size_t)(64 + 3 * (size_t)nqs + tsize) * 4, 8));
+        pe::FoldArgs fa{nullptr, nullptr, nullptr, 0};
+        c->last_fold = try_fold;
+        if (try_fold) {
+            LaunchScope ls(c, PHOEBE_ELPH_K_QFOLD);
+            const bool in_smem = nqs <= 8192;                  // fingerprints + table + partners: nq (8 + 4) + 4 tsize bytes
+            const size_t dsm = in_smem ? (size_t)nqs * 12 + (size_t)tsize * 4 : 0;
+            PE_CUDA(c, ensure_smem_optin((const void*)pe::k_qfold_detect, dsm));
+            pe::k_qfold_detect<<<1, 1024, dsm, c->stream>>>(q + 3 * (size_t)qs, nqs, c->rp_integer ? 1 : 0, in_smem ? 1 : 0, f_table,
+                                                            tsize, f_partner, f_fp, f_rep, f_mate, f_meta);
+            PE_CUDA(c, cudaGetLastError());
+            fa = pe::FoldArgs{f_meta, f_rep, f_mate, c->pair_Kc4};
+        }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
             if (use_pair) {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->pair_Kc4, 64));
                 pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc,
                                                                c->pair_Kc4, nqs, c->pair_Kr, c->pair_KrPad, c->L.ldq,
-                                                               c->phase_sign, c->PtP, nullptr, nullptr, nullptr, 0);
+                                                               c->phase_sign, c->PtP, nullptr, nullptr, fa.meta ? fa.meta + 1 : nullptr, 0);
+                if (try_fold) {      // the same over the representatives only
+                    PE_CUDA(c, cudaGetLastError());
+                    pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc,
+                                                                   c->pair_Kc4, nqs, c->pair_Kr, c->pair_KrPad, c->L.ldq,
+                                                                   c->phase_sign, c->PtP, f_rep, f_meta, f_meta + 1, 1);
+                }
             } else {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->L.Kpad, 64));
                 pe::k_qphase<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->Rp, c->deg_p, nqs, d.nRp, c->L.Kpad,
@@ -624,16 +660,23 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 g.strideBrow = (long long)c->L.g1_stride;
             }
             if (use_pair) {
-                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair, pe::PairCfg::kSmemBytes));
+                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair<false>, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs * c->pair_ctas);
                 const int slot = rows_per_k > 0 ? slot0 : c->k_sel;
                 int panelW = grid;      // as for the planar form: the panel of pair rows (width x Kr x 1024 B) stays in L2
                 while (panelW % 2 == 0 && (size_t)panelW * c->pair_Kr * pe::PairCfg::ROWB * 8 > (48u << 20)) panelW /= 2;
-                pe::k_contract_pair<<<grid, pe::PairCfg::kThreads, pe::PairCfg::kSmemBytes, c->stream>>>(
+                pe::k_contract_pair<false><<<grid, pe::PairCfg::kThreads, pe::PairCfg::kSmemBytes, c->stream>>>(
                     c->PtP, c->L.ldq, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64), (long long)c->L.g1P_stride,
-                    c->C, ldcq, nqs, N, c->pair_Kr, c->pair_KrPad, rows_per_k, qs, panelW, cm);
+                    c->C, ldcq, nqs, N, c->pair_Kr, c->pair_KrPad, rows_per_k, qs, panelW, cm, fa);
                 PE_CUDA(c, cudaGetLastError());
+                if (try_fold) {
+                    PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair<true>, pe::PairCfg::kFoldSmemBytes));
+                    pe::k_contract_pair<true><<<grid, pe::PairCfg::kThreads, pe::PairCfg::kFoldSmemBytes, c->stream>>>(
+                        c->PtP, c->L.ldq, c->g1P + (size_t)slot * c->L.g1P_stride, ceil_div(N, 64), (long long)c->L.g1P_stride,
+                        c->C, ldcq, nqs, N, c->pair_Kr, c->pair_KrPad, 0, 0, panelW, cm, fa);
+                    PE_CUDA(c, cudaGetLastError());
+                }
             } else if (use_planar) {
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_planar, pe::PlanarCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
@@ -1379,6 +1422,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "qfold")) { c->qfold = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_blk")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
         c->rot_blk = (int)value;
@@ -1416,6 +1460,16 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "qfold_reps")) {       // representatives of the last q_batch call if it took the fold, else 0
+        *value = 0;
+        if (c->last_fold) {
+            int meta[2] = {0, 0};
+            if (cudaMemcpyAsync(meta, c->ws + c->L.off_fold, 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                cudaStreamSynchronize(c->stream) != cudaSuccess) return PHOEBE_ELPH_E_CUDA;
+            *value = meta[1] ? meta[0] : 0;
+        }
+        return PHOEBE_ELPH_OK;
+    }
     if (!strcmp(key, "nq_sub_max")) { *value = c->L.nq_sub; return PHOEBE_ELPH_OK; }
     // byte offsets of the C and Pt scratch areas inside the workspace (debugging aids for the tests)
     if (!strcmp(key, "off_C")) { *value = (int64_t)c->L.off_C; return PHOEBE_ELPH_OK; }
