@@ -83,10 +83,24 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def single(self, out):
+        """One query right now (timed regions shorter than the sampling period leave no sample)."""
+        try:
+            r = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                               capture_output=True, text=True, timeout=10).stdout.strip().split(",")
+            if len(r) >= 7:
+                names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+                out.update(sm_mhz=float(r[0]), sm_max_mhz=float(r[1]), power_w_max=float(r[2]), samples=1,
+                           reasons=sorted(n for n, v in zip(names, r[3:7]) if v.strip().lower() == "active"),
+                           note="timed region shorter than the 100 ms sampling period: one query right after it")
+        except Exception:
+            pass
+        return out
+
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.proc is None:
-            return out
+            return self.single(out)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
@@ -108,6 +122,8 @@ class ClockSampler:
                            samples=len(sm), power_w_max=max(float(r[2]) for r in rows if len(r) >= 7))
         except Exception:
             pass
+        if not out["samples"]:
+            return self.single(out)
         return out
 
 

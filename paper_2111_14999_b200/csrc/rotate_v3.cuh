@@ -33,7 +33,10 @@ namespace pe {
 // ~230 registers: 8 consumer warps (8 x 232 + 4 x 40 = 12 x 168); items with one tile fit 160: 12 consumer warps
 // (12 x 160 + 4 x 32 = 16 x 128), three per scheduler -- more warps to overlap one item's DMMA phases with another's
 // operand sums / epilogue.
-__host__ __device__ constexpr int rot3_consumers(int MTW) { return MTW == 2 ? 8 : 12; }
+#ifndef PHOEBE_ROT3_NCW1
+#define PHOEBE_ROT3_NCW1 12
+#endif
+__host__ __device__ constexpr int rot3_consumers(int MTW) { return MTW == 2 ? 8 : PHOEBE_ROT3_NCW1; }
 __host__ __device__ constexpr int rot3_threads(int MTW) { return (rot3_consumers(MTW) + 4) * 32; }
 constexpr int kRot3Stages = 3;
 
@@ -99,7 +102,7 @@ __global__ void __launch_bounds__(rot3_threads(MTW), 1)
 k_rotate_v3(const Rot3Args a)
 {
     constexpr int NCW = rot3_consumers(MTW), NTHREADS = rot3_threads(MTW);
-    constexpr int REGS_C = MTW == 2 ? 232 : 160, REGS_P = MTW == 2 ? 40 : 32;
+    constexpr int REGS_C = MTW == 2 ? 232 : (NCW == 16 ? 112 : 160), REGS_P = MTW == 2 ? 40 : 32;
     constexpr bool RSM = (MODE & 1) != 0;                 // the Eq. 29 arrays exist in the Q stages
     constexpr bool POLAR = (MODE & 2) != 0;
     const bool rates = RSM && (MODE != 3 || a.ra.eps_k != nullptr);
