@@ -255,12 +255,12 @@ k_rotate_v3(const Rot3Args a)
     const int uof = t * ldu + g;                         // A fragment of a5: row t of a k-step, column g of a tile of b2
     // two consecutive outputs of a lane are one aligned 16-byte store
     const bool st2 = (nm & 1) == 0 && (reinterpret_cast<uintptr_t>(a.out) & 15u) == 0;
-    int Sq = 0, Sc = 0;              // stages of the two rings consumed so far (slot = S % NS, phase = (S / NS) & 1)
+    int sq = 0, sc = 0; uint32_t phq = 0, phc = 0;       // slot and phase parity of the two rings
     int rem = 0;                     // (items of all earlier stages) % NCW
-    for (int qg = blockIdx.x; qg < nqg; qg += gridDim.x, ++Sq) {
+    const int nbg_full = (min(gb1, nb1) + GB - 1) / GB;
+    for (int qg = blockIdx.x; qg < nqg; qg += gridDim.x) {
         const int q0 = qg * QS, nql = min(QS, a.nq - q0);
-        const int sq = Sq % NS;
-        mbar_wait(qfull + sq, (uint32_t)(Sq / NS) & 1u);
+        mbar_wait(qfull + sq, phq);
         const unsigned char* Q = smem_raw + L.off_Q + (size_t)sq * L.szQ;
         const double2* Us = reinterpret_cast<const double2*>(Q);
         const double2* Zs = reinterpret_cast<const double2*>(Q + L.szU);
@@ -269,17 +269,16 @@ k_rotate_v3(const Rot3Args a)
         const double* bose_s = om_s + QS * 8 * NT;
         const double* e2_s = bose_s + QS * 8 * NT;
         const double* f2_s = e2_s + QS * 8 * MT;
-        for (int grp = 0; grp < ngroups; ++grp, ++Sc) {
-            const int sc = Sc % NS;
+        for (int grp = 0; grp < ngroups; ++grp) {
             const double2* Cs = reinterpret_cast<const double2*>(smem_raw + L.off_C + (size_t)sc * L.szC);
             const int b10 = grp * gb1;
             const int nb1l = min(gb1, nb1 - b10);
-            const int nbg = (nb1l + GB - 1) / GB;
+            const int nbg = nb1l == gb1 ? nbg_full : (nb1l + GB - 1) / GB;
             const int per_q = nbg * nmg;
             const int ni = nql * per_q;
             int item = warp - rem; if (item < 0) item += NCW;           // this warp's first item of the stage
             rem = (rem + ni) % NCW;
-            mbar_wait(cfull + sc, (uint32_t)(Sc / NS) & 1u);
+            mbar_wait(cfull + sc, phc);
             for (; item < ni; item += NCW) {
                 int ql = 0, r = item;
                 if (nql > 1) { ql = (int)((unsigned)item / (unsigned)per_q); r = item - ql * per_q; }
@@ -499,10 +498,12 @@ k_rotate_v3(const Rot3Args a)
             __threadfence_block();
             __syncwarp();
             if (lane == 0) mbar_arrive(cempty + sc);
+            if (++sc == NS) { sc = 0; phc ^= 1u; }
         }
         __threadfence_block();
         __syncwarp();
         if (lane == 0) mbar_arrive(qempty + sq);
+        if (++sq == NS) { sq = 0; phq ^= 1u; }
     }
 }
 
