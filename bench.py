@@ -492,6 +492,9 @@ def run_ours(args):
     n_k = len(dev_inputs)
     # algorithmic work per LAUNCH of each kernel
     gemm_launches = max(1, kernels.get("setk_gemm", {}).get("launches_per_step", 1))
+    setk_rows = ctx.get_tuning("setk_pair_rows")     # > 0: a1 GEMM in the +R / -R pair form: 4 real flop per (k, ring row, x)
+    if setk_rows:
+        counts["setk_gemm_flop"] = 4 * setk_rows * w.nRp * w.X        # (rows of THIS context: a Re shard when pooled)
     gemm_flop = counts["setk_gemm_flop"] * n_k / gemm_launches
     gemm_alu = gemm_flop / (FP64_PEAK_TFLOPS * 1e12) > counts["setk_stream_bytes"] / (hbm_peak * 1e9)
     per_launch = {

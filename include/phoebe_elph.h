@@ -332,6 +332,10 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               single-CTA pair search (24 us for 4096 q, 0.35 ms for 32768 q) costs more than the halved contraction
  *               saves at the sizes measured.  get_tuning("qfold_reps") = representatives of the
  *               LAST q_batch call if it took the fold, else 0 (synchronises the stream)
+ *   "setk_pair" 1 (default) = the a1 GEMM of set_k_batch folds the +R / -R pairs of the Re list (real phases x complex sums
+ *               g_W[e] +- g_W[ebar] formed on the fly: 2 instead of 3 tensor instructions per tile and k-step) whenever
+ *               that saves time (batches of >= 12 k-points, where the three-multiply form is FP64-bound); 0 = always the
+ *               three-multiply form.  get_tuning("setk_pair_rows") = ring rows (2 per pair) if the last set_k_batch used it
  *   "rot_plain" 1 = force the plain DFMA rotation kernel (the fallback for nmodes > 48)
  *   "rot_qg" / "rot_gb1" / "rot_mtw"   override the geometry of the tensor-core rotation kernel (rotate_v3.cuh):
  *               q-points per ring stage, b1 per C stage (forces the two-ring form), 8-row tiles of b2 per warp item

@@ -21,6 +21,7 @@
 #include "qbatch_kernels.cuh"
 #include "rotate_v3.cuh"
 #include "setk_kernels.cuh"
+#include "setk_pair.cuh"
 
 namespace {
 
@@ -58,7 +59,7 @@ struct Layout {
     int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t g1P_stride = 0;  // doubles between the planar blocked copies of g1' (k_contract_planar) of consecutive k slots
-    size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_Tpart = 0,
+    size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_pairE = 0, off_zero = 0, off_Tpart = 0,
            off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_fold = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
@@ -101,7 +102,10 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_degp = take((size_t)d.nRp * 8);
     L.off_Uk = take((size_t)L.nk_slots * d.nw * d.nb1_max * 16);
     L.off_kdev = take((size_t)kKBatchMax * 3 * 8);
-    L.off_Ptk = take((size_t)L.KpadE * kKBatchMax * 16);
+    L.off_Ptk = take((size_t)(L.KpadE + 16) * kKBatchMax * 16);
+    // +R / -R pair map of the Re list for the a1 GEMM (setk_pair.cuh): row map (2 ints) + vector + weight per pair
+    L.off_pairE = take((size_t)(d.nRe + 8) * (2 * 4 + 4 * 8));
+    L.off_zero = take(X * 16);                                       // a row of zeros (vectors without partner)
     L.off_Tpart = take((size_t)std::max(L.S_alloc, L.nk_slots) * d.nRp * X * 16);
     L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
     // planar blocked copies ([rows][tiles of 64][3][64] doubles) of g1' and of the phases for k_contract_planar
@@ -193,6 +197,11 @@ struct phoebe_elph_ctx {
     int pair_Kr = 0, pair_KrPad = 0, pair_K2 = 0;   // K2 = (cos, sin) row pairs
     int pair_Kc = 0, pair_Kc4 = 0;                  // cosine rows (pairs + self-inverse vectors), padded to a multiple of 4
     bool rp_integer = false;
+    // a1 pair form (setk_pair.cuh): the Re list folded into npairE (cos, sin) row pairs; 0 = not usable
+    int npairE = 0;
+    int* pairE_rowmap = nullptr; double *pairE_R = nullptr, *pairE_w = nullptr; double2* zero_row = nullptr;
+    bool setk_pair = true;    // tuning "setk_pair": 1 = use it when it saves tensor work (default), 0 = never
+    bool last_setk_pair = false;
     int pair = 1;             // tuning "pair": 1 = use it when 4 Kr < 6 nRp (default), 0 = never, 2 = whenever the map exists
     int pair_ctas = 1;        // tuning "pair_ctas": persistent CTAs of k_contract_pair per SM (its ring is 100 KB: two fit)
     int last_pair = -1;       // did the last contraction launch use the pair form (-1: no launch yet)
@@ -389,6 +398,37 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     const int X = d.nw * d.nw * d.nmodes;
     if (int rc = keep_Uk(c, Uk_dev, nk, nb1)) return rc;
     PE_CUDA(c, cudaMemcpyAsync(c->kdev, k_host, (size_t)nk * 24, cudaMemcpyHostToDevice, c->stream));
+    // the fold pays where the three-multiply GEMM is FP64-bound (6 nk flop per 16 bytes of g_W against 37 TFLOP/s and
+    // 6.5 TB/s: nk >= 12; measured: 32 k band-window 0.306 -> 0.201 ms, 16 k 4-atom 4.93 -> 4.69 ms, 4 k large cell
+    // 8.1 -> 9.4 ms -- HBM-bound, where the plain form streams better)
+    c->last_setk_pair = c->setk_pair && c->m3 && c->npairE > 0 && nk >= 12;
+    if (c->last_setk_pair) {
+        // +R / -R pairs of the Re list folded (setk_pair.cuh): real phases x complex sums formed on the fly
+        const int Kr = 2 * c->npairE, KrPad = (int)align_up((size_t)Kr, 8);
+        double* PtkR = reinterpret_cast<double*>(c->Ptk);
+        {
+            LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
+            pe::k_kphase_pair<<<dim3(1, std::min(KrPad / 2, 256)), 32, 0, c->stream>>>(c->kdev, c->pairE_R, c->pairE_w, nk, c->npairE,
+                                                                                      KrPad, c->phase_sign, PtkR);
+            PE_CUDA(c, cudaGetLastError());
+        }
+        {
+            LaunchScope ls(c, PHOEBE_ELPH_K_SETK_GEMM);
+            const int grid = ceil_div(X, 128) * d.nRp;
+            auto launch = [&](auto kern, size_t smem, int threads) -> cudaError_t {
+                cudaError_t e2 = ensure_smem_optin((const void*)kern, smem);
+                if (e2 != cudaSuccess) return e2;
+                kern<<<grid, threads, smem, c->stream>>>(PtkR, c->gW, (long long)d.nRe * X, X, c->pairE_rowmap, c->zero_row, c->Tpart,
+                                                         (long long)d.nRp * X, nk, Kr, KrPad, d.nRp);
+                return cudaGetLastError();
+            };
+            cudaError_t e;
+            if (nk <= 8) e = launch(pe::k_setk_pair<8, 128, 4, 8, 6>, pe::SetkPairCfg<8, 128, 4, 8, 6>::kSmemBytes, 160);
+            else if (nk <= 16) e = launch(pe::k_setk_pair<16, 128, 4, 8, 6>, pe::SetkPairCfg<16, 128, 4, 8, 6>::kSmemBytes, 160);
+            else e = launch(pe::k_setk_pair<32, 128, 4, 8, 5>, pe::SetkPairCfg<32, 128, 4, 8, 5>::kSmemBytes, 160);
+            PE_CUDA(c, e);
+        }
+    } else {
     {
         LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
         dim3 grid(1, std::min(c->L.KpadE, 256));
@@ -413,6 +453,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
             else e = launch_contract<32, 128, 1, 4, 8, 4, false>(c->stream, g, false);
         }
         PE_CUDA(c, e);
+    }
     }
     {
         int rc = launch_setk_rotate(c, c->Tpart, 1, Uk_dev, nb1, c->g1_base, nk, (long long)d.nRp * X,
@@ -907,6 +948,46 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
             up(c->pair_R, h_R.data(), h_R.size() * 8);
             up(c->pair_w, h_w.data(), h_w.size() * 8);
         }
+    }
+    // ---- +R / -R pair map of the Re list (setk_pair.cuh): every vector is in exactly one "pair" (e, ebar | none) ----
+    std::vector<int> hE_map;
+    std::vector<double> hE_R, hE_w;
+    {
+        const int nRe = dims->nRe;
+        auto key = [&](int p, double sg) {
+            return std::array<double, 3>{sg * Re_host[3 * p] + 0.0, sg * Re_host[3 * p + 1] + 0.0, sg * Re_host[3 * p + 2] + 0.0};
+        };
+        auto wt = [&](int p) { return deg_e_host ? deg_e_host[p] : 1.0; };
+        std::map<std::array<double, 3>, int> first;
+        for (int p = nRe - 1; p >= 0; --p) first[key(p, 1.0)] = p;
+        std::vector<char> used((size_t)nRe, 0);
+        for (int p = 0; p < nRe; ++p) {
+            if (used[p]) continue;
+            used[p] = 1;
+            int partner = -1;
+            if (!(key(p, 1.0) == key(p, -1.0))) {
+                auto it = first.find(key(p, -1.0));
+                if (it != first.end() && !used[it->second] && wt(it->second) == wt(p)) { partner = it->second; used[partner] = 1; }
+            }
+            hE_map.push_back(p); hE_map.push_back(partner);
+            hE_R.push_back(Re_host[3 * p]); hE_R.push_back(Re_host[3 * p + 1]); hE_R.push_back(Re_host[3 * p + 2]);
+            hE_w.push_back(1.0 / wt(p));
+        }
+        const int P = (int)hE_w.size();
+        // 2 DMMA per ring row x 2 P rows against 3 per row x nRe rows of the three-multiply form
+        c->npairE = ((size_t)4 * P < (size_t)3 * nRe && 2 * P <= nRe + 8) ? P : 0;
+        char* base = c->ws + L.off_pairE;
+        c->pairE_rowmap = reinterpret_cast<int*>(base);
+        c->pairE_R = reinterpret_cast<double*>(base + align_up((size_t)(nRe + 8) * 2 * 4, 8));
+        c->pairE_w = c->pairE_R + 3 * (size_t)(nRe + 8);
+        c->zero_row = reinterpret_cast<double2*>(c->ws + L.off_zero);
+        if (c->npairE > 0) {
+            up(c->pairE_rowmap, hE_map.data(), hE_map.size() * 4);
+            up(c->pairE_R, hE_R.data(), hE_R.size() * 8);
+            up(c->pairE_w, hE_w.data(), hE_w.size() * 8);
+        }
+        if (e == cudaSuccess)
+            e = cudaMemsetAsync(c->zero_row, 0, (size_t)dims->nw * dims->nw * dims->nmodes * 16, c->stream);
     }
     // the padding elements of the C layout (rotate_v3.cuh) are read, never written: they must hold finite values
     if (e == cudaSuccess)
@@ -1423,6 +1504,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold")) { c->qfold = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "setk_pair")) { c->setk_pair = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_blk")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
         c->rot_blk = (int)value;
@@ -1460,6 +1542,8 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
+    // ring rows of the a1 pair form (2 per +R / -R pair of the Re list) if the LAST set_k_batch used it, else 0
+    if (!strcmp(key, "setk_pair_rows")) { *value = c->last_setk_pair ? 2 * c->npairE : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold_reps")) {       // representatives of the last q_batch call if it took the fold, else 0
         *value = 0;
         if (c->last_fold) {
