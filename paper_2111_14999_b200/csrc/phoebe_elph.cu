@@ -423,9 +423,15 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
                 return cudaGetLastError();
             };
             cudaError_t e;
-            if (nk <= 8) e = launch(pe::k_setk_pair<8, 128, 4, 8, 6>, pe::SetkPairCfg<8, 128, 4, 8, 6>::kSmemBytes, 160);
-            else if (nk <= 16) e = launch(pe::k_setk_pair<16, 128, 4, 8, 6>, pe::SetkPairCfg<16, 128, 4, 8, 6>::kSmemBytes, 160);
-            else e = launch(pe::k_setk_pair<32, 128, 4, 8, 5>, pe::SetkPairCfg<32, 128, 4, 8, 5>::kSmemBytes, 160);
+            // ring depth 4 (72 KB per CTA: three CTAs per SM); measured on the 4-atom cell (16 k): 4 / 6 / 8 stages of 8 rows ->
+            // 3.92 / 4.70 / 7.50 ms, 3 / 4 stages of 16 rows -> 4.42 / 6.44 ms: resident CTAs matter more than ring depth
+#ifndef PHOEBE_SETKP_ST
+#define PHOEBE_SETKP_ST 4
+#endif
+            constexpr int ST = PHOEBE_SETKP_ST;
+            if (nk <= 8) e = launch(pe::k_setk_pair<8, 128, 4, 8, ST>, pe::SetkPairCfg<8, 128, 4, 8, ST>::kSmemBytes, 160);
+            else if (nk <= 16) e = launch(pe::k_setk_pair<16, 128, 4, 8, ST>, pe::SetkPairCfg<16, 128, 4, 8, ST>::kSmemBytes, 160);
+            else e = launch(pe::k_setk_pair<32, 128, 4, 8, ST + 1>, pe::SetkPairCfg<32, 128, 4, 8, ST + 1>::kSmemBytes, 160);   // band-window, 32 k: 3 / 4 / 5 stages -> 0.223 / 0.205 / 0.201 ms
             PE_CUDA(c, e);
         }
     } else {
