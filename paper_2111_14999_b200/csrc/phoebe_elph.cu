@@ -568,17 +568,18 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
     const int nb1 = c->nb1, Y = d.nw * d.nmodes, N = nb1 * Y;
     const int nq_sub = std::min(c->nq_sub, c->L.nq_sub);
     // rotation kernel geometry: rotate_v3 (FP64 tensor cores) for nm <= 48, else the plain DFMA kernel
-    const bool use_mma = d.nmodes <= 48 && !c->rot_plain;
-    const bool fused_rates = rr != nullptr && use_mma;
     const bool polar = c->nG > 0;
     Rot3Geom G{};
+    // (a cell whose U_kq / ev stages do not fit three-deep in shared memory -- nw beyond ~56 -- takes the plain kernel too)
+    const bool use_mma = d.nmodes <= 48 && !c->rot_plain &&
+                         rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), rr != nullptr || polar, c->rot_qg, c->rot_gb1,
+                                       c->rot_mtw, c->rot_blk, &G);
+    const bool fused_rates = rr != nullptr && use_mma;
     int gb1 = nb1, rot_threads = 0;
     size_t rot_smem = 0;
     int P = d.nmodes, PB = d.nw * d.nmodes;                 // C layout (plain for the DFMA kernel)
     if (use_mma) {
-        // the polar kernels (mode 3) always carry the Eq. 29 arrays in their stages
-        if (!rot3_geometry(d.nw, d.nmodes, nb1, nb2, std::min(nq, nq_sub), fused_rates || polar, c->rot_qg, c->rot_gb1, c->rot_mtw, c->rot_blk, &G))
-            return fail(c, PHOEBE_ELPH_E_DIMS, "rotation tile does not fit shared memory");
+        // (the polar kernels, mode 3, always carry the Eq. 29 arrays in their stages)
         P = G.P; PB = G.PB; gb1 = G.gb1; rot_smem = G.smem; rot_threads = pe::rot3_threads(G.MTW);
     } else {
         const size_t fixed = ((size_t)d.nw * nb2 + (size_t)d.nmodes * d.nmodes) * 16;

@@ -49,6 +49,7 @@ CASES = [(5, 3, 4, nm, 37) for nm in (4, 5, 17, 21, 22, 25, 33, 37, 41, 48)] + \
     (9, 2, 9, 8, 200),        # KS = 2, two m-tiles, 2 b1 per item, nm = 0 mod 8
     (7, 6, 7, 16, 100),       # KS = 4, 2 b1 per item
     (32, 32, 32, 30, 5),      # the large cell's shape: b1 groups, two rings
+    (64, 3, 64, 6, 10),       # U_kq stages of 68 KB: three do not fit shared memory -> the plain kernel takes over
 ]
 
 
