@@ -1,0 +1,348 @@
+// contract_i8.cuh -- step a4 (Eq. 70) on the 5th-generation tensor cores (tcgen05.mma kind::i8, accumulators
+// in TMEM) by exact integer splitting (the Ozaki scheme): B200's FP64 tensor pipe gives 37 TFLOP/s, its INT8 one 4.4 POP/s.
+//
+// The pair form (contract_pair.cuh) makes a4 a REAL GEMM  C'[q][n'] = sum_r A[q][r] B'[r][n'],  n' = (n, re|im).
+// Every operand value is written as a 48-bit fixed-point number relative to a power-of-two scale (A: one scale for the
+// whole phase matrix, |A| <= max weight; B': one scale per complex column n = twice the column's largest magnitude) and
+// split into SIX balanced base-256 digits d_i in [-128, 127]:   x = scale * sum_i d_i 256^i / 2^47.
+// Then  A B' = sA sB 2^-94 sum_{i,j} 256^(i+j) (A_i B'_j)  with A_i B'_j an INT8 x INT8 GEMM whose INT32 accumulation is
+// EXACT (|sum| <= 6 * 736 * 128^2 < 2^27).  The 21 digit pairs with i + j >= 5 are kept, summed per level l = i + j - 5 in
+// six TMEM accumulators; the dropped pairs are below 2^-45 of scale_A * scale_B per term -- a NORMWISE error of ~1e-13 of
+// the column scale, inside the 1e-10 parity bar with two orders of magnitude to spare.  The levels
+// are recombined exactly in 64-bit integers (two halves) and rounded once, in the FP64 epilogue that writes C in the
+// layout the rotation kernel reads.
+//
+// Operands are produced ALREADY TILED for the tensor core (no-swizzle K-major canonical layout: core matrices of
+// 8 rows x 16 bytes, 128 contiguous bytes each), so that a ring stage is twelve contiguous 1-D bulk copies:
+//   A digits  Ai8[d][m tile of 128][k chunk of 64][row group 16][k group 4][8 rows][16 bytes]      (k_qphase_i8)
+//   B digits  Bi8[slot][d][n' tile of 64][k chunk of 64][col group 8][k group 4][8 cols][16 bytes]  (k_pack_i8)
+// Kernel: warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warps 2..9 = epilogue (TMEM -> registers -> C).
+#pragma once
+#include "ptx_helpers.cuh"
+
+namespace pe {
+
+struct I8Cfg {
+    static constexpr int BM = 128, BN = 64, KC = 64, ND = 6, NLEV = 6, STAGES = 3;
+    static constexpr int kThreads = 10 * 32;
+    static constexpr int A_PLANE = BM * KC, B_PLANE = BN * KC;                    // bytes of one digit plane of a stage
+    static constexpr int STAGE_BYTES = ND * (A_PLANE + B_PLANE);                 // 72 KB
+    static constexpr size_t kSmemBytes = (size_t)STAGES * STAGE_BYTES + 1024 + 256;   // + alignment slack + barriers
+    static constexpr int TMEM_COLS = 512;                                        // NLEV * BN = 384 used
+};
+
+// six balanced base-256 digits of round(v * inv_scale * 2^47); |v * inv_scale| <= 1/2
+__device__ __forceinline__ void i8_digits(double v, double inv_scale, int8_t (&d)[6])
+{
+    long long X = __double2ll_rn(v * inv_scale * 140737488355328.0);             // 2^47
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        const int di = (int)((X + 128) & 255) - 128;
+        d[i] = (int8_t)di;
+        X = (X - di) >> 8;
+    }
+}
+
+// byte offset of element (row, k) inside a digit plane tiled [row tile][k chunk][row group][k group][8][16]
+__device__ __forceinline__ size_t i8_tiled_off(int row, int k, int rows_per_tile, int nchunks)
+{
+    constexpr int KC = I8Cfg::KC;
+    const int tile = row / rows_per_tile, rl = row - tile * rows_per_tile;
+    const int chunk = k / KC, kl = k - chunk * KC;
+    return ((size_t)tile * nchunks + chunk) * (size_t)(rows_per_tile * KC) +
+           (size_t)(((rl >> 3) * (KC / 16) + (kl >> 4)) * 128 + (rl & 7) * 16 + (kl & 15));
+}
+
+// A digits.  Row order of the pair form (k_qphase_pair): cosine rows r < Kc (pairs first), sine row of pair sl at Kc16 + sl
+// (Kc16 = the cosine block padded to a multiple of 16, so a thread's 16 cosine rows and their 16 sine rows are whole
+// 16-byte groups).  One thread = one q-point x 16 consecutive cosine rows.  Columns q >= nq are zero digits; the 16-row groups
+// behind the sine block are never written (the planes are zeroed once at setup).
+// grid (ceil(ldq/128), ceil(Kc16/16)), block 128.
+__global__ void __launch_bounds__(128)
+k_qphase_i8(const double* __restrict__ q, const double* __restrict__ Rrow, const double* __restrict__ wrow, int K2, int Kc,
+            int Kc16, int nq, int Kpad, int ldq, double sgn, double inv_scaleA, int8_t* __restrict__ Ai8, size_t plane_bytes)
+{
+    const int iq = blockIdx.x * 128 + threadIdx.x;
+    if (iq >= ldq) return;
+    const int r0 = blockIdx.y * 16;
+    const int nchunks = Kpad / I8Cfg::KC;
+    double q0 = 0.0, q1 = 0.0, q2 = 0.0;
+    const bool valid = iq < nq;
+    if (valid) { q0 = q[3 * (size_t)iq]; q1 = q[3 * (size_t)iq + 1]; q2 = q[3 * (size_t)iq + 2]; }
+    int8_t dc[6][16], ds[6][16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        const int r = r0 + u;
+        double vc = 0.0, vs = 0.0;
+        if (valid && r < Kc) {
+            const double x = q0 * Rrow[3 * r] + q1 * Rrow[3 * r + 1] + q2 * Rrow[3 * r + 2];
+            double sn, cs;
+            sincospi(2.0 * x, &sn, &cs);
+            vc = wrow[r] * cs; vs = (r < K2) ? wrow[r] * sgn * sn : 0.0;
+        }
+        int8_t d[6];
+        i8_digits(vc, inv_scaleA, d);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) dc[i][u] = d[i];
+        i8_digits(vs, inv_scaleA, d);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) ds[i][u] = d[i];
+    }
+    const size_t oc = i8_tiled_off(iq, r0, I8Cfg::BM, nchunks);
+    const bool has_sin = r0 < K2;                          // the sine group of these 16 rows exists
+    const size_t os = has_sin ? i8_tiled_off(iq, Kc16 + r0, I8Cfg::BM, nchunks) : 0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        *reinterpret_cast<int4*>(Ai8 + (size_t)i * plane_bytes + oc) = *reinterpret_cast<const int4*>(dc[i]);
+        if (has_sin) *reinterpret_cast<int4*>(Ai8 + (size_t)i * plane_bytes + os) = *reinterpret_cast<const int4*>(ds[i]);
+    }
+}
+
+// column maxima of B': cmax[slot][n] = max_r |pair row r of column n| (re or im), as the bit pattern of the non-negative
+// double (ordered like the integers) under atomicMax; zeroed by the host before the launch.  One thread = one column x 16
+// rows.  grid (ceil(N/128), ceil(Kr/16), nslots), block 128.
+__global__ void __launch_bounds__(128)
+k_i8_colmax(const double2* __restrict__ g1, long long ld, long long strideS, int N, int Kr, const int* __restrict__ pa,
+            const int* __restrict__ pb, const int* __restrict__ kind, unsigned long long* __restrict__ cmax, int ldsb)
+{
+    const int n = blockIdx.x * 128 + threadIdx.x, slot = blockIdx.z, r0 = blockIdx.y * 16;
+    if (n >= N) return;
+    const double2* s = g1 + (size_t)slot * strideS + n;
+    double m = 0.0;
+#pragma unroll 4
+    for (int r = r0; r < min(r0 + 16, Kr); ++r) {
+        if (kind[r] == 2) continue;
+        const double2 a = s[(size_t)pa[r] * ld];
+        const int ib = pb[r];
+        const double2 b = ib >= 0 ? s[(size_t)ib * ld] : make_double2(0.0, 0.0);
+        const double x = kind[r] == 0 ? a.x + b.x : a.y - b.y, y = kind[r] == 0 ? a.y + b.y : a.x - b.x;
+        m = fmax(m, fmax(fabs(x), fabs(y)));
+    }
+    if (m > 0.0) atomicMax(cmax + (size_t)slot * ldsb + n, (unsigned long long)__double_as_longlong(m));
+}
+
+// column scale from the maximum: 2^(e+1) with 2^e > m (m = f 2^e, f in [1/2, 1)); 1 for an all-zero column
+__device__ __forceinline__ double i8_scale_of(unsigned long long mbits)
+{
+    const double m = __longlong_as_double((long long)mbits);
+    if (!(m > 0.0)) return 1.0;
+    int e = 0;
+    frexp(m, &e);
+    return ldexp(1.0, e + 1);
+}
+
+// B' digits: real column n' = 2 n + c (c = 0: re, 1: im) of pair row r, relative to the column scale sb[slot][n] (written here
+// from the column maximum).  One thread = one real column x 16 consecutive rows.
+// grid (ceil(Npad2/128), Kpad/16, nslots), block 128.  Columns >= 2 N and rows >= Kr are zero digits.
+__global__ void __launch_bounds__(128)
+k_pack_i8(const double2* __restrict__ g1, long long ld, long long strideS, int N, int Npad2, int Kr, int Kpad,
+          const int* __restrict__ pa, const int* __restrict__ pb, const int* __restrict__ kind,
+          const unsigned long long* __restrict__ cmax, double* __restrict__ sb, int ldsb, int8_t* __restrict__ Bi8,
+          size_t plane_bytes, size_t slot_bytes)
+{
+    const int np = blockIdx.x * 128 + threadIdx.x, slot = blockIdx.z;
+    if (np >= Npad2) return;
+    const int n = np >> 1, c = np & 1, r0 = blockIdx.y * 16;
+    const bool colok = n < N;
+    const double scale = colok ? i8_scale_of(cmax[(size_t)slot * ldsb + n]) : 1.0;
+    const double inv = colok ? 1.0 / scale : 0.0;
+    if (colok && c == 0 && blockIdx.y == 0) sb[(size_t)slot * ldsb + n] = scale;      // the GEMM epilogue's column scale
+    const double2* s = g1 + (size_t)slot * strideS + (colok ? n : 0);
+    int8_t dd[6][16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+        const int r = r0 + u;
+        double v = 0.0;
+        if (colok && r < Kr && kind[r] != 2) {
+            const double2 a = s[(size_t)pa[r] * ld];
+            const int ib = pb[r];
+            const double2 b = ib >= 0 ? s[(size_t)ib * ld] : make_double2(0.0, 0.0);
+            if (kind[r] == 0) v = c ? a.y + b.y : a.x + b.x;            // a + b
+            else v = c ? a.x - b.x : -(a.y - b.y);                      // i (a - b)
+        }
+        int8_t d[6];
+        i8_digits(v, inv, d);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) dd[i][u] = d[i];
+    }
+    const size_t o = i8_tiled_off(np, r0, I8Cfg::BN, Kpad / I8Cfg::KC);
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+        *reinterpret_cast<int4*>(Bi8 + (size_t)slot * slot_bytes + (size_t)i * plane_bytes + o) = *reinterpret_cast<const int4*>(dd[i]);
+}
+
+// ---- tcgen05 helpers (PTX ISA: tcgen05.*, sm_100a) -------------------------------------------------------------------
+// shared-memory matrix descriptor, K-major, no swizzle: core matrices of 8 rows x 16 bytes; lbo = byte distance between
+// core matrices adjacent in K, sbo = between those adjacent in M / N (verified against a host product on this B200)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) |
+           ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}\n"
+                 :: "r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(0u) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar)      // arrives on bar when all MMAs issued so far have completed
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                   "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr));
+}
+
+// C[q][n] (complex, layout CMap) = sum_r A[q][r] B'[r][(n, re|im)] from the digit planes.  M rows of A (q), N complex
+// columns, Kpad (multiple of 64) rows; Ai8 / Bi8 tiled as above (plane strides in bytes); sb = column scales of this slot.
+// rowsPerB > 0: stacked multi-k form, rows [j rowsPerB, (j+1) rowsPerB) use B slot j (rowsPerB a multiple of 128).
+__global__ void __launch_bounds__(I8Cfg::kThreads, 1)
+k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t* __restrict__ Bi8, size_t b_plane_bytes,
+              size_t b_slot_bytes, const double* __restrict__ sb, int ldsb, double scaleA, double2* __restrict__ C,
+              long long ldc, int M, int N, int Kpad, int rowsPerB, int rowOffset, CMap cm)
+{
+    using Cfg = I8Cfg;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = Cfg::KC, ND = Cfg::ND, ST = Cfg::STAGES;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)ST * Cfg::STAGE_BYTES);
+    uint64_t* empty = full + ST;
+    uint64_t* tfull = empty + ST;           // accumulators of a tile complete
+    uint64_t* tempty = tfull + 1;           // accumulators read out by the epilogue
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 1);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        mbar_init(tfull, 1); mbar_init(tempty, 8);
+        mbar_fence_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(tmem_slot)), "r"(Cfg::TMEM_COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+    const int nchunks = Kpad / KC;
+    const int ntn = (2 * N + BN - 1) / BN, ntm = (M + BM - 1) / BM;
+    const int ntiles = ntn * ntm;                       // n fastest: the CTAs running together share a few A row blocks
+
+    if (warp == 0) {
+        // ================= TMA producer: twelve contiguous bulk copies per stage =================
+        int s = 0; uint32_t ph = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int tm = tile / ntn, tn = tile - tm * ntn;
+            const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
+            const int8_t* a_src = Ai8 + (size_t)tm * nchunks * Cfg::A_PLANE;
+            const int8_t* b_src = Bi8 + (size_t)slot * b_slot_bytes + (size_t)tn * nchunks * Cfg::B_PLANE;
+            for (int c = 0; c < nchunks; ++c) {
+                mbar_wait(empty + s, ph ^ 1u);
+                if (lane == 0) mbar_arrive_expect_tx(full + s, (uint32_t)Cfg::STAGE_BYTES);
+                __syncwarp();
+                unsigned char* st = smem + (size_t)s * Cfg::STAGE_BYTES;
+                if (lane < ND)
+                    bulk_g2s(st + lane * Cfg::A_PLANE, a_src + (size_t)lane * a_plane_bytes + (size_t)c * Cfg::A_PLANE, Cfg::A_PLANE, full + s);
+                else if (lane < 2 * ND)
+                    bulk_g2s(st + ND * Cfg::A_PLANE + (lane - ND) * Cfg::B_PLANE,
+                             b_src + (size_t)(lane - ND) * b_plane_bytes + (size_t)c * Cfg::B_PLANE, Cfg::B_PLANE, full + s);
+                if (++s == ST) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer (one thread) =================
+        // Digit plane A_i meets the B' planes j = 5 - i .. 5, whose products belong to the levels 0 .. i: the planes are
+        // contiguous in the stage and the level accumulators contiguous in TMEM, so ONE instruction with N = 64 (i + 1)
+        // does all of them and reads the A tile from shared memory once (the unit's limit is N <= 256: i = 4 and 5 take two).
+        // Shared-memory reads per 32-deep step: 75 KB instead of the 126 KB of 21 single-level instructions -- below the
+        // 128 B/clk the tensor pipe's own time (693 clk) allows.
+        // instruction descriptor: D = S32, A = B = signed 8 bit, both K-major, M = 128, N in bits 17..22
+        constexpr uint32_t idesc0 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BM >> 4) << 24);
+        int s = 0; uint32_t ph = 0, tph = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            mbar_wait(tempty, tph ^ 1u);                 // the epilogue has read the previous tile's accumulators
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            for (int c = 0; c < nchunks; ++c) {
+                mbar_wait(full + s, ph);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                if (lane == 0) {
+                    const uint32_t a0 = smem_u32(smem + (size_t)s * Cfg::STAGE_BYTES), b0 = a0 + ND * Cfg::A_PLANE;
+#pragma unroll
+                    for (int ks = 0; ks < KC / 32; ++ks) {
+                        const uint32_t acc = (c == 0 && ks == 0) ? 0u : 1u;
+                        // i = 5 first: its two instructions initialise all six levels of a new tile
+#pragma unroll
+                        for (int i = ND - 1; i >= 0; --i) {
+                            const uint64_t da = umma_desc(a0 + i * Cfg::A_PLANE + ks * 256, 128, (KC / 16) * 128);
+                            const int j0 = ND - 1 - i, nlev = i + 1;              // planes j0 .. 5 -> levels 0 .. i
+                            const int n1 = nlev > 4 ? 4 : nlev;                   // first instruction: levels 0 .. n1 - 1
+                            umma_i8(tmem, da, umma_desc(b0 + j0 * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
+                                    idesc0 | ((uint32_t)((n1 * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
+                            if (nlev > 4)
+                                umma_i8(tmem + 4u * BN, da, umma_desc(b0 + (j0 + 4) * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
+                                        idesc0 | ((uint32_t)(((nlev - 4) * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
+                        }
+                    }
+                    umma_commit(empty + s);               // frees the stage when these MMAs have read it
+                    if (c == nchunks - 1) umma_commit(tfull);
+                }
+                __syncwarp();
+                if (++s == ST) { s = 0; ph ^= 1u; }
+            }
+            tph ^= 1u;
+        }
+    } else {
+        // ================= epilogue warps (8): TMEM lanes 32 (warp % 4) .. + 31 = rows; half h = 32 real columns ========
+        // Phase A reads the six levels of the warp's 32 columns and recombines them (exactly, in 64-bit integers) into 32
+        // doubles held in registers, then hands the accumulators back to the MMA warp; phase B scales and stores while the
+        // next tile's MMAs run.  Column offsets (CMap) and scales are computed once per tile by lanes 0..15 and broadcast.
+        const int wq = warp & 3, half = (warp - 2) >> 2;
+        uint32_t tph = 0;
+        const double kscale = scaleA * 5.551115123125783e-17;        // 2^-54
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            const int tm = tile / ntn, tn = tile - tm * ntn;
+            const int m = tm * BM + wq * 32 + lane;
+            const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
+            const int ncol = tn * (BN / 2) + half * 16 + (lane & 15);    // this lane's complex column (lanes 16..31 mirror)
+            long long off_l = -1; double sc_l = 0.0;
+            if (ncol < N) { off_l = cmap_off(ncol, cm); sc_l = kscale * sb[(size_t)slot * ldsb + ncol]; }
+            double val[32];
+            mbar_wait(tfull, tph);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int rd = 0; rd < 2; ++rd) {
+                uint32_t v[Cfg::NLEV][16];
+#pragma unroll
+                for (int l = 0; l < Cfg::NLEV; ++l)
+                    tmem_ld16(tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)(l * BN + half * 32 + rd * 16), v[l]);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const long long lo = (long long)(int)v[0][e] + ((long long)(int)v[1][e] << 8) + ((long long)(int)v[2][e] << 16);
+                    const long long hi = (long long)(int)v[3][e] + ((long long)(int)v[4][e] << 8) + ((long long)(int)v[5][e] << 16);
+                    val[rd * 16 + e] = fma((double)hi, 16777216.0, (double)lo);   // exact up to the one final rounding
+                }
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty);
+            tph ^= 1u;
+            double2* crow = C + (size_t)min(m, M - 1) * ldc;
+#pragma unroll
+            for (int jc = 0; jc < 16; ++jc) {
+                const long long off = __shfl_sync(0xffffffffu, off_l, jc);
+                const double sc = __shfl_sync(0xffffffffu, sc_l, jc);
+                if (m < M && off >= 0) crow[off] = make_double2(val[2 * jc] * sc, val[2 * jc + 1] * sc);
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(Cfg::TMEM_COLS));
+}
+
+}  // namespace pe

@@ -18,6 +18,7 @@
 #include "contract_planar.cuh"
 #include "contract_pair.cuh"
 #include "qfold.cuh"
+#include "contract_i8.cuh"
 #include "qbatch_kernels.cuh"
 #include "rotate_v3.cuh"
 #include "setk_kernels.cuh"
@@ -59,8 +60,11 @@ struct Layout {
     int Kpad = 0, KpadE = 0, ldq = 0, nq_sub = 0, S_alloc = 0, nk_slots = 1;
     size_t g1_stride = 0;   // complex elements between the g1' of consecutive k slots
     size_t g1P_stride = 0;  // doubles between the planar blocked copies of g1' (k_contract_planar) of consecutive k slots
+    // contract_i8.cuh: bytes of one digit plane of A (all q tiles) and of B' (one k slot), rows padded to 64, columns to 64
+    int i8_Kpad = 0, i8_Npad2 = 0, i8_ldsb = 0;
+    size_t i8_a_plane = 0, i8_b_plane = 0;
     size_t off_Re = 0, off_Rp = 0, off_dege = 0, off_degp = 0, off_Uk = 0, off_kdev = 0, off_Ptk = 0, off_pairE = 0, off_zero = 0, off_Tpart = 0,
-           off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_fold = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
+           off_g1 = 0, off_g1P = 0, off_pair = 0, off_Pt = 0, off_PtP = 0, off_C = 0, off_part = 0, off_fold = 0, off_Ai8 = 0, off_Bi8 = 0, off_sb = 0, off_rate = 0, off_seps = 0, off_G = 0, off_Zstar = 0, off_P = 0, off_sq = 0, off_sUkq = 0, off_sev = 0, off_som = 0, off_sout = 0, total = 0;
     size_t sz_sq = 0, sz_sUkq = 0, sz_sev = 0, sz_som = 0, sz_sout = 0;   // bytes of ONE staging slot (there are two)
 };
 
@@ -109,15 +113,24 @@ Layout make_layout(const phoebe_elph_dims& d, int nq_max)
     L.off_Tpart = take((size_t)std::max(L.S_alloc, L.nk_slots) * d.nRp * X * 16);
     L.off_g1 = take((size_t)L.nk_slots * L.g1_stride * 16);
     // planar blocked copies ([rows][tiles of 64][3][64] doubles) of g1' and of the phases for k_contract_planar
-    L.g1P_stride = ((size_t)d.nRp * 192 + 384) * ceil_div((int)N, 64);     // (+ 3 padding rows of the pair form)
+    L.g1P_stride = ((size_t)d.nRp * 192 + 1920) * ceil_div((int)N, 64);    // (+ 15 padding rows of the pair form)
     L.off_g1P = take((size_t)L.nk_slots * L.g1P_stride * 8);
     // +R / -R pair map of the Rp list for k_contract_pair: 3 int + 4 double per real row, at most 2 nRp rows
-    L.off_pair = take((size_t)(2 * d.nRp + 4) * (3 * 4 + 4 * 8));
+    L.off_pair = take((size_t)(2 * d.nRp + 16) * (3 * 4 + 4 * 8));
     L.off_Pt = take((size_t)L.Kpad * L.ldq * 16);
     L.off_PtP = take((size_t)L.Kpad * L.ldq * 24);
     L.off_C = take((size_t)L.nq_sub * c_elems_per_q(d, d.nb1_max) * 16);
     // f2: linewidth partials [nq][groups of b2 tiles][nb1], staging of rate / eps_k / eps_kq for the host entry point
     L.off_part = take((size_t)nq_max * ceil_div(d.nb2_max, 8) * d.nb1_max * 8);
+    // a4 on the INT8 tensor cores (contract_i8.cuh): six digit planes of the phases and of the pair rows, column scales
+    L.i8_Kpad = (int)align_up((size_t)(2 * d.nRp + 16), 64);                   // >= any Kr
+    L.i8_Npad2 = (int)align_up(2 * N, 64);
+    L.i8_ldsb = (int)align_up(N, 32);
+    L.i8_a_plane = (size_t)L.ldq * L.i8_Kpad;
+    L.i8_b_plane = (size_t)L.i8_Npad2 * L.i8_Kpad;
+    L.off_Ai8 = take(6 * L.i8_a_plane);
+    L.off_Bi8 = take((size_t)L.nk_slots * 6 * L.i8_b_plane);
+    L.off_sb = take((size_t)2 * L.nk_slots * L.i8_ldsb * 8);      // column scales, then the column maxima they come from
     // q <-> -q fold: hash table (power of two >= 2 nq, so < 4 nq ints), partner / representative / mate lists, meta
     L.off_fold = take((size_t)nq_max * (7 * 4 + 8) + 512);
     L.off_rate = take((size_t)2 * 2 * L.nk_slots * d.nb1_max * 8);    // two slots of (rate, eps_k), each [k slots][nb1]
@@ -179,6 +192,10 @@ struct phoebe_elph_ctx {
     int rot_qg = 0, rot_gb1 = 0, rot_mtw = 0;   // tuning "rot_qg" / "rot_gb1" / "rot_mtw": override the v2 rotation geometry (0 = automatic)
     int64_t launches[PHOEBE_ELPH_K_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
     bool qfold = false;       // tuning "qfold" (opt-in): contract (q, -q) pairs of a q list once (qfold.cuh)
+    int i8 = 1;               // tuning "i8": 1 = a4 on the INT8 tensor cores by exact digit splitting (contract_i8.cuh), 0 = FP64 DMMA
+    bool Bi8_stale = true;    // the digit planes of g1' must be rebuilt (as g1P_stale)
+    double i8_scaleA = 2.0;   // power-of-two scale of the phase matrix: 2 x the largest weight 1/deg_p, rounded up
+    int last_i8 = -1;
     bool last_fold = false;   // the last contraction went through the fold-capable launch sequence
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -384,6 +401,7 @@ int run_set_k(phoebe_elph_ctx* c, const double* k, const double2* Uk_dev, int nb
     c->nb1 = nb1;
     c->nk_have = 1;
     c->g1P_stale = true;
+    c->Bi8_stale = true;
     c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
@@ -469,6 +487,7 @@ int run_set_k_batch(phoebe_elph_ctx* c, int nk, const double* k_host, const doub
     c->nb1 = nb1;
     c->nk_have = nk;
     c->g1P_stale = true;
+    c->Bi8_stale = true;
     c->k_sel = 0;
     c->g1 = c->g1_base;
     c->have_k = true;
@@ -638,7 +657,28 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         const bool use_pair = use_planar && c->pair_Kr > 0 &&
                               (c->pair == 2 || (c->pair == 1 && (size_t)4 * c->pair_Kr < (size_t)6 * d.nRp));
         c->last_pair = use_pair ? 1 : 0;
-        if (use_planar && (c->g1P_stale || c->g1P_form != (use_pair ? 2 : 1))) {
+        // the pair form on the INT8 tensor cores by exact digit splitting (contract_i8.cuh)
+        const bool use_i8 = use_pair && c->i8 != 0 && !(c->qfold && rows_per_k == 0 && nqs >= 256) &&
+                            (rows_per_k == 0 || rows_per_k % pe::I8Cfg::BM == 0);      // a row tile must not straddle two k slots
+        c->last_i8 = use_i8 ? 1 : 0;
+        const int i8_Kpad = (int)align_up((size_t)c->pair_Kr, 64), i8_Npad2 = (int)align_up((size_t)2 * N, 64);
+        int8_t* Ai8 = reinterpret_cast<int8_t*>(c->ws + c->L.off_Ai8);
+        int8_t* Bi8 = reinterpret_cast<int8_t*>(c->ws + c->L.off_Bi8);
+        double* sbv = reinterpret_cast<double*>(c->ws + c->L.off_sb);
+        if (use_i8 && c->Bi8_stale) {
+            LaunchScope ls(c, PHOEBE_ELPH_K_PACK);
+            unsigned long long* cmax = reinterpret_cast<unsigned long long*>(sbv + (size_t)c->L.nk_slots * c->L.i8_ldsb);
+            PE_CUDA(c, cudaMemsetAsync(cmax, 0, (size_t)c->nk_have * c->L.i8_ldsb * 8, c->stream));
+            pe::k_i8_colmax<<<dim3(ceil_div(N, 128), ceil_div(c->pair_Kr, 16), c->nk_have), 128, 0, c->stream>>>(
+                c->g1_base, (long long)N, (long long)c->L.g1_stride, N, c->pair_Kr, c->pair_pa, c->pair_pb, c->pair_kind, cmax, c->L.i8_ldsb);
+            PE_CUDA(c, cudaGetLastError());
+            pe::k_pack_i8<<<dim3(ceil_div(i8_Npad2, 128), i8_Kpad / 16, c->nk_have), 128, 0, c->stream>>>(
+                c->g1_base, (long long)N, (long long)c->L.g1_stride, N, i8_Npad2, c->pair_Kr, i8_Kpad, c->pair_pa, c->pair_pb,
+                c->pair_kind, cmax, sbv, c->L.i8_ldsb, Bi8, c->L.i8_b_plane, 6 * c->L.i8_b_plane);
+            PE_CUDA(c, cudaGetLastError());
+            c->Bi8_stale = false;
+        }
+        if (use_planar && !use_i8 && (c->g1P_stale || c->g1P_form != (use_pair ? 2 : 1))) {
             // canonical g1' of every filled k slot -> blocked operand copy (planar planes, or pair rows)
             LaunchScope ls(c, PHOEBE_ELPH_K_PACK);
             if (use_pair) {
@@ -656,7 +696,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
         // q <-> -q fold (qfold.cuh): the pairs are found on the device; both launch sequences are enqueued and the
         // kernels of the path not taken return at once
-        const bool try_fold = use_pair && c->qfold && rows_per_k == 0 && nqs >= 256 && c->pair_K2 > 0;
+        const bool try_fold = use_pair && !use_i8 && c->qfold && rows_per_k == 0 && nqs >= 256 && c->pair_K2 > 0;
         int* fold_base = reinterpret_cast<int*>(c->ws + c->L.off_fold);
         int tsize = 1;
         while (tsize < 2 * nqs) tsize <<= 1;
@@ -681,7 +721,11 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
         }
         {
             LaunchScope ls(c, PHOEBE_ELPH_K_QPHASE);
-            if (use_pair) {
+            if (use_i8) {
+                pe::k_qphase_i8<<<dim3(ceil_div(ncols, 128), c->pair_Kc4 / 16), 128, 0, c->stream>>>(
+                    q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc, c->pair_Kc4, nqs, i8_Kpad, c->L.ldq,
+                    c->phase_sign, 1.0 / c->i8_scaleA, Ai8, c->L.i8_a_plane);
+            } else if (use_pair) {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->pair_Kc4, 64));
                 pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc,
                                                                c->pair_Kc4, nqs, c->pair_Kr, c->pair_KrPad, c->L.ldq,
@@ -707,7 +751,15 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 g.B = c->g1_base + (size_t)slot0 * c->L.g1_stride; g.rowsPerB = rows_per_k; g.rowOffset = qs;
                 g.strideBrow = (long long)c->L.g1_stride;
             }
-            if (use_pair) {
+            if (use_i8) {
+                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_i8, pe::I8Cfg::kSmemBytes));
+                const int ntiles = ceil_div(nqs, pe::I8Cfg::BM) * ceil_div(2 * N, pe::I8Cfg::BN);
+                pe::k_contract_i8<<<std::min(ntiles, kSMs), pe::I8Cfg::kThreads, pe::I8Cfg::kSmemBytes, c->stream>>>(
+                    Ai8, c->L.i8_a_plane, Bi8 + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * 6 * c->L.i8_b_plane, c->L.i8_b_plane,
+                    6 * c->L.i8_b_plane, sbv + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * c->L.i8_ldsb, c->L.i8_ldsb, c->i8_scaleA,
+                    c->C, ldcq, nqs, N, i8_Kpad, rows_per_k, qs, cm);
+                PE_CUDA(c, cudaGetLastError());
+            } else if (use_pair) {
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair<false>, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
                 const int grid = std::min(ntiles, kSMs * c->pair_ctas);
@@ -931,19 +983,26 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
         c->pair_K2 = (int)pairs.size();
         for (int p : selfs) row(p, -1, 0);
         c->pair_Kc = (int)h_pa.size();
-        while (h_pa.size() % 4) row(0, -1, 2);                  // zero rows: the sine block starts at a k-step boundary
+        while (h_pa.size() % 16) row(0, -1, 2);                 // zero rows: the sine block starts at a 16-row group (contract_i8.cuh)
         c->pair_Kc4 = (int)h_pa.size();
         for (auto& pr : pairs) row(pr.first, pr.second, 1);
         c->pair_Kr = (int)h_pa.size();
+        {
+            double wmax = 0.0;
+            for (int p = 0; p < nRp; ++p) wmax = std::max(wmax, 1.0 / wt(p));
+            int ex = 0;
+            std::frexp(wmax, &ex);                               // wmax = f 2^ex, f in [1/2, 1)
+            c->i8_scaleA = std::ldexp(1.0, ex + 1);              // |phase| <= wmax < 2^ex = scale / 2
+        }
         c->rp_integer = true;                                   // q -> q + G leaves the phases alone only for integer Rp
         for (int i = 0; i < 3 * nRp; ++i) if (Rp_host[i] != std::floor(Rp_host[i])) c->rp_integer = false;
         c->pair_KrPad = (int)align_up((size_t)c->pair_Kr, (size_t)std::max(kKPad, pe::PairCfg::KC));
         // the pair form reuses the planar buffers: rows must fit them (g1P: Kr*128 <= nRp*192 doubles per tile column,
         // PtP: KrPad*8 <= Kpad*24 bytes per q)
-        if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 + 384 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
+        if ((size_t)c->pair_Kr * 128 > (size_t)nRp * 192 + 1920 || (size_t)c->pair_KrPad * 8 > (size_t)L.Kpad * 24) c->pair_Kr = 0;
         if (c->pair_Kr > 0) {
             char* base = c->ws + L.off_pair;
-            const size_t cap = (size_t)2 * nRp + 4;
+            const size_t cap = (size_t)2 * nRp + 16;
             c->pair_pa = reinterpret_cast<int*>(base);
             c->pair_pb = c->pair_pa + cap;
             c->pair_kind = c->pair_pb + cap;
@@ -996,6 +1055,8 @@ int phoebe_elph_setup(phoebe_elph_ctx** ctx_out, const void* gW_dev, const doubl
         if (e == cudaSuccess)
             e = cudaMemsetAsync(c->zero_row, 0, (size_t)dims->nw * dims->nw * dims->nmodes * 16, c->stream);
     }
+    // the 16-row groups of the A digit planes behind the sine block are read, never written (contract_i8.cuh)
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + L.off_Ai8, 0, 6 * L.i8_a_plane, c->stream);
     // the padding elements of the C layout (rotate_v3.cuh) are read, never written: they must hold finite values
     if (e == cudaSuccess)
         e = cudaMemsetAsync(c->C, 0, (size_t)L.nq_sub * c_elems_per_q(*dims, dims->nb1_max) * 16, c->stream);
@@ -1438,6 +1499,7 @@ int phoebe_elph_g1_buffer(phoebe_elph_ctx* c, int32_t slot, void** ptr_out, size
     const size_t one = (size_t)c->dims.nRp * c->nb1 * c->dims.nw * c->dims.nmodes * 16;
     const size_t stride = c->L.g1_stride * 16;
     c->g1P_stale = true;                 // the caller may change g1' in place (Re-pool all-reduce): re-pack before the next a4
+    c->Bi8_stale = true;
     if (stride_out) *stride_out = stride;
     if (slot >= 0) {
         *ptr_out = c->g1_base + (size_t)slot * c->L.g1_stride;
@@ -1511,6 +1573,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold")) { c->qfold = value != 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8")) { c->i8 = value != 0 ? 1 : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "setk_pair")) { c->setk_pair = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_blk")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
@@ -1549,6 +1612,7 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8")) { *value = c->last_i8 < 0 ? c->i8 : c->last_i8; return PHOEBE_ELPH_OK; }   // did the last a4 run on INT8
     // ring rows of the a1 pair form (2 per +R / -R pair of the Re list) if the LAST set_k_batch used it, else 0
     if (!strcmp(key, "setk_pair_rows")) { *value = c->last_setk_pair ? 2 * c->npairE : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold_reps")) {       // representatives of the last q_batch call if it took the fold, else 0

@@ -423,10 +423,10 @@ def test_q_batch_multi_equals_per_k_calls(env, knob):
         ctx.select_k(ik)
         one = ctx.q_batch(*harness.to_device(list(ins[ik]))).cpu().numpy()
         if "nq_sub" not in knob:
-            assert np.array_equal(one, got[ik])
+            assert _relerr(one, got[ik]) <= 1e-12        # equal up to the rounding order (the two may take different a4 kernels)
     # fewer slots than the batch holds; errors
     part = ctx.q_batch_multi(*[t[:2].contiguous() for t in stacked]).cpu().numpy()
-    assert np.array_equal(part, got[:2])
+    assert _relerr(part, got[:2]) <= 1e-12
     for bad in ([t[:, :100].contiguous() for t in stacked],):            # nq not a multiple of 64
         with pytest.raises(binding.PhoebeElphError) as e:
             ctx.q_batch_multi(*bad)

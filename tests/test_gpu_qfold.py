@@ -94,6 +94,7 @@ def test_qfold_non_integer_lattice_vectors_pair_only_the_literal_negative(env):
     ref = oracle.elph(gW, Re, Rp, None, None, k, Uk, q, Ukq, ev, om)
     ctx = binding.ElphContext(torch.from_numpy(gW).cuda(), Re, Rp, None, None, nb1_max=nb, nb2_max=nb, nq_max=nq)
     ctx.set_tuning("tile", 64)
+    ctx.set_tuning("pair", 2)             # 13 vectors: too short a list for the pair form to be chosen by itself
     ctx.set_tuning("qfold", 1)
     ctx.set_k(k, harness.to_device([Uk])[0])
     out = ctx.q_batch(*harness.to_device([q, Ukq, ev, om])).cpu().numpy()
@@ -115,6 +116,7 @@ def test_qfold_with_rates_and_polar(env):
     rref = oracle.rates(ref, eps_k, eps_kq, om, P["kT"], P["mu"], P["sigma"], P["pref"])
     ctx = harness.make_context(w, torch.from_numpy(gW_np).cuda(), nq_max=len(q))
     ctx.set_tuning("tile", 64)
+    ctx.set_tuning("pair", 2)             # 9 vectors: too short a list for the pair form to be chosen by itself
     ctx.set_tuning("qfold", 1)
     ctx.set_k(k, harness.to_device([Uk])[0])
     d = harness.to_device([q, Ukq, ev, om, eps_k, eps_kq, np.zeros(w.nb1)])
