@@ -34,6 +34,7 @@ DEFAULT_WORKLOAD = "4-atom"
 # 64 FP64 FMA / clk / SM  x 2 flop x 148 SMs x 1.965 GHz (clocks.max.sm)
 FP64_PEAK_TFLOPS = 64 * 2 * 148 * 1.965e9 / 1e12
 HBM_FALLBACK_GBS = 6650.0
+BF16_FALLBACK_TFLOPS = 1590.0      # the profiling recipe's fallback (B200_PROFILING.md), used only without MEASURED_PEAKS.json
 
 
 # ----------------------------------------------------------------------------- utilities
@@ -497,11 +498,16 @@ def run_ours(args):
         counts["setk_gemm_flop"] = 4 * setk_rows * w.nRp * w.X        # (rows of THIS context: a Re shard when pooled)
     gemm_flop = counts["setk_gemm_flop"] * n_k / gemm_launches
     gemm_alu = gemm_flop / (FP64_PEAK_TFLOPS * 1e12) > counts["setk_stream_bytes"] / (hbm_peak * 1e9)
+    # a4 on the INT8 tensor cores (contract_i8.cuh): 21 digit-pair products of the real pair-form GEMM, 2 ops per INT8 MAC
+    i8_on = bool(ctx.get_tuning("i8")) and pair_rows > 0
+    contract_launches = max(1, kernels.get("contract", {}).get("launches_per_step", 1))
+    i8_ops = 21 * 2 * nq_l * (2 * w.N) * pair_rows * n_k / contract_launches if i8_on else 0
+    int8_peak_tops = 2.0 * float(peaks.get("bf16_tflops", BF16_FALLBACK_TFLOPS))
     per_launch = {
         "setk_stream": ("hbm", counts["setk_stream_bytes"]),
         # multi-k a1: g_W read once per launch, nk_b x the flops; bound = whichever floor is higher
         "setk_gemm": ("alu", gemm_flop) if gemm_alu else ("hbm", counts["setk_stream_bytes"]),
-        "contract": ("alu", counts["contract_flop"] * n_k / max(1, kernels.get("contract", {}).get("launches_per_step", 1))),
+        "contract": ("tensor", i8_ops) if i8_on else ("alu", counts["contract_flop"] * n_k / contract_launches),
     }
     # a5-a7: HBM-bound for small cells, FP64-bound for 4-atom / large: report against the higher floor.
     # Its flops are the ALGORITHMIC four-multiply count of SURVEY 8(d) (the kernel executes fewer: three-multiply product)
@@ -514,6 +520,12 @@ def run_ours(args):
             dur = kernels[kind]["avg_ms"] * 1e-3
             if bound == "hbm":
                 kernels[kind].update(bound="hbm", achieved=work / dur / 1e9, peak=hbm_peak, unit="GB/s")
+            elif bound == "tensor":
+                f64_flop = counts["contract_flop_4m"] * n_k / contract_launches
+                kernels[kind].update(bound="tensor", achieved=work / dur / 1e12, peak=int8_peak_tops, unit="TOP/s", dtype="s8",
+                                     int8_nominal_peak_tops=4500.0, frac_of_nominal=work / dur / 1e12 / 4500.0,
+                                     fp64_equivalent_tflops=f64_flop / dur / 1e12,
+                                     fp64_equivalent_over_fp64_peak=f64_flop / dur / 1e12 / FP64_PEAK_TFLOPS)
             else:
                 kernels[kind].update(bound="alu", achieved=work / dur / 1e12, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s")
             kernels[kind]["frac"] = kernels[kind]["achieved"] / kernels[kind]["peak"]
@@ -523,12 +535,19 @@ def run_ours(args):
     roofline = {"kernel": dominant, "bound": dk.get("bound"), "achieved": dk.get("achieved"), "peak": dk.get("peak"),
                 "unit": dk.get("unit"), "frac": dk.get("frac"), "traffic": traffic,
                 "peak_source": ("MEASURED_PEAKS.json hbm_gbs (%s)" % peak_src) if dk.get("bound") == "hbm"
+                else ("INT8 dense = 2 x MEASURED_PEAKS.json bf16_tflops (%s; burst figure: the kernel is timed alone; the "
+                      "guide's nominal INT8 : bf16 ratio is 4.5 : 2.25); nominal 4500 TOP/s" % peak_src) if dk.get("bound") == "tensor"
                 else "derived: 64 FP64 FMA/clk/SM x 148 SMs x 1.965 GHz x 2 = 37.24 TFLOP/s",
                 "share_of_step": dk["ms_total"] / sum(v["ms_total"] for v in kernels.values()),
                 "flop_per_complex_mac": counts["contract_flop_per_mac"] if dominant == "contract" else counts["flop_per_complex_mac"],
-                "note": "achieved counts EXECUTED flops: 4 per complex MAC in a4's +R/-R pair form (real phases x complex "
-                        "pair rows), 6 with the three-multiply product, 8 with the plain one; the algorithmic count of "
-                        "SURVEY 8(d) is 8"}
+                "note": ("a4 runs on the INT8 tensor cores by exact digit splitting (Ozaki scheme): every FP64 operand of the "
+                         "+R/-R pair form is six signed base-256 digits, 21 digit-pair INT8 GEMMs (tcgen05.mma kind::i8, INT32 "
+                         "accumulation in TMEM, exact) are recombined in the FP64 epilogue; achieved = 21 x 2 x q rows x 2 N x "
+                         "pair rows INT8 ops per launch / duration; fp64_equivalent_tflops (kernels.contract) divides SURVEY "
+                         "8(d)'s 8 real flop per complex MAC by the same duration") if dk.get("bound") == "tensor" else
+                        ("achieved counts EXECUTED flops: 4 per complex MAC in a4's +R/-R pair form (real phases x complex "
+                         "pair rows), 6 with the three-multiply product, 8 with the plain one; the algorithmic count of "
+                         "SURVEY 8(d) is 8")}
     fp64_probe = None
     if rank == 0:
         try:
@@ -600,13 +619,17 @@ def run_ours(args):
         c1 = harness.algorithmic_counts(w, nq=nq_l, m3=m3, pair_rows=ctx.get_tuning("pair_rows"))
         k3 = {kind: {"ms_total": ms_, "launches_per_step": n_, "avg_ms": ms_ / n_} for kind, (ms_, n_) in prof3.items() if n_}
         share = (re_hi - re_lo) / w.nRe if pooled else 1.0
-        for kind, bound, work in (("setk_stream", "hbm", c1["setk_stream_bytes"] * share), ("contract", "alu", c1["contract_flop"]),
+        i8_3 = bool(ctx.get_tuning("i8")) and ctx.get_tuning("pair_rows") > 0
+        for kind, bound, work in (("setk_stream", "hbm", c1["setk_stream_bytes"] * share),
+                                  ("contract", "tensor", 21 * 2 * nq_l * (2 * w.N) * ctx.get_tuning("pair_rows")) if i8_3
+                                  else ("contract", "alu", c1["contract_flop"]),
                                   ("rotate_epilogue", "alu" if rot_alu else "hbm", c1["rotate_flop"] if rot_alu else c1["rotate_bytes"])):
             if kind in k3:
                 dur = k3[kind]["avg_ms"] * 1e-3
-                peak_ = FP64_PEAK_TFLOPS if bound == "alu" else hbm_peak
-                ach = work / dur / (1e12 if bound == "alu" else 1e9)
-                k3[kind].update(bound=bound, achieved=ach, peak=peak_, unit="TFLOP/s" if bound == "alu" else "GB/s", frac=ach / peak_)
+                peak_ = {"alu": FP64_PEAK_TFLOPS, "tensor": int8_peak_tops, "hbm": hbm_peak}[bound]
+                ach = work / dur / (1e9 if bound == "hbm" else 1e12)
+                k3[kind].update(bound=bound, achieved=ach, peak=peak_, unit={"alu": "TFLOP/s", "tensor": "TOP/s", "hbm": "GB/s"}[bound],
+                                frac=ach / peak_)
         three_call = {"what": "phoebe_elph_set_k + phoebe_elph_q_batch per k-point (north_star's three-call boundary; g_W is "
                               "re-read for every k-point)", "value": pairs_per_step_all * n3 / (ms3 * 1e-3), "unit": UNIT,
                       "ms_per_step": ms3 / n3, "kernels": k3}

@@ -13,9 +13,10 @@
 // layout the rotation kernel reads.
 //
 // Operands are produced ALREADY TILED for the tensor core (no-swizzle K-major canonical layout: core matrices of
-// 8 rows x 16 bytes, 128 contiguous bytes each), so that a ring stage is twelve contiguous 1-D bulk copies:
-//   A digits  Ai8[d][m tile of 128][k chunk of 64][row group 16][k group 4][8 rows][16 bytes]      (k_qphase_i8)
-//   B digits  Bi8[slot][d][n' tile of 64][k chunk of 64][col group 8][k group 4][8 cols][16 bytes]  (k_pack_i8)
+// 8 rows x 16 bytes, 128 contiguous bytes each) with the six digit planes of a (tile, k chunk) side by side, so that a
+// ring stage is TWO contiguous 1-D bulk copies (the TMA unit takes ~100 clk per bulk request whatever its size):
+//   A digits  Ai8[m tile of 128][k chunk KC][d][row group 16][k group KC/16][8 rows][16 bytes]      (k_qphase_i8)
+//   B digits  Bi8[slot][n' tile of 64][k chunk KC][d][col group 8][k group KC/16][8 cols][16 bytes]  (k_pack_i8)
 // Kernel: warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warps 2..9 = epilogue (TMEM -> registers -> C).
 #pragma once
 #include "ptx_helpers.cuh"
@@ -23,7 +24,10 @@
 namespace pe {
 
 struct I8Cfg {
-    static constexpr int BM = 128, BN = 64, KC = 64, ND = 6, NLEV = 6, STAGES = 3;
+#ifndef PHOEBE_I8_KC
+#define PHOEBE_I8_KC 32
+#endif
+    static constexpr int BM = 128, BN = 64, KC = PHOEBE_I8_KC, ND = 6, NLEV = 6, STAGES = 216 * 1024 / (ND * (BM + BN) * KC);
     static constexpr int kThreads = 10 * 32;
     static constexpr int A_PLANE = BM * KC, B_PLANE = BN * KC;                    // bytes of one digit plane of a stage
     static constexpr int STAGE_BYTES = ND * (A_PLANE + B_PLANE);                 // 72 KB
@@ -43,13 +47,14 @@ __device__ __forceinline__ void i8_digits(double v, double inv_scale, int8_t (&d
     }
 }
 
-// byte offset of element (row, k) inside a digit plane tiled [row tile][k chunk][row group][k group][8][16]
+// byte offset of element (row, k) of digit 0 in the tiling [row tile][k chunk][digit][row group][k group][8][16];
+// digit d is d * rows_per_tile * KC bytes further
 __device__ __forceinline__ size_t i8_tiled_off(int row, int k, int rows_per_tile, int nchunks)
 {
     constexpr int KC = I8Cfg::KC;
     const int tile = row / rows_per_tile, rl = row - tile * rows_per_tile;
     const int chunk = k / KC, kl = k - chunk * KC;
-    return ((size_t)tile * nchunks + chunk) * (size_t)(rows_per_tile * KC) +
+    return ((size_t)tile * nchunks + chunk) * (size_t)(I8Cfg::ND * rows_per_tile * KC) +
            (size_t)(((rl >> 3) * (KC / 16) + (kl >> 4)) * 128 + (rl & 7) * 16 + (kl & 15));
 }
 
@@ -60,7 +65,7 @@ __device__ __forceinline__ size_t i8_tiled_off(int row, int k, int rows_per_tile
 // grid (ceil(ldq/128), ceil(Kc16/16)), block 128.
 __global__ void __launch_bounds__(128)
 k_qphase_i8(const double* __restrict__ q, const double* __restrict__ Rrow, const double* __restrict__ wrow, int K2, int Kc,
-            int Kc16, int nq, int Kpad, int ldq, double sgn, double inv_scaleA, int8_t* __restrict__ Ai8, size_t plane_bytes)
+            int Kc16, int nq, int Kpad, int ldq, double sgn, double inv_scaleA, int8_t* __restrict__ Ai8)
 {
     const int iq = blockIdx.x * 128 + threadIdx.x;
     if (iq >= ldq) return;
@@ -93,8 +98,8 @@ k_qphase_i8(const double* __restrict__ q, const double* __restrict__ Rrow, const
     const size_t os = has_sin ? i8_tiled_off(iq, Kc16 + r0, I8Cfg::BM, nchunks) : 0;
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-        *reinterpret_cast<int4*>(Ai8 + (size_t)i * plane_bytes + oc) = *reinterpret_cast<const int4*>(dc[i]);
-        if (has_sin) *reinterpret_cast<int4*>(Ai8 + (size_t)i * plane_bytes + os) = *reinterpret_cast<const int4*>(ds[i]);
+        *reinterpret_cast<int4*>(Ai8 + (size_t)i * I8Cfg::A_PLANE + oc) = *reinterpret_cast<const int4*>(dc[i]);
+        if (has_sin) *reinterpret_cast<int4*>(Ai8 + (size_t)i * I8Cfg::A_PLANE + os) = *reinterpret_cast<const int4*>(ds[i]);
     }
 }
 
@@ -138,7 +143,7 @@ __global__ void __launch_bounds__(128)
 k_pack_i8(const double2* __restrict__ g1, long long ld, long long strideS, int N, int Npad2, int Kr, int Kpad,
           const int* __restrict__ pa, const int* __restrict__ pb, const int* __restrict__ kind,
           const unsigned long long* __restrict__ cmax, double* __restrict__ sb, int ldsb, int8_t* __restrict__ Bi8,
-          size_t plane_bytes, size_t slot_bytes)
+          size_t slot_bytes)
 {
     const int np = blockIdx.x * 128 + threadIdx.x, slot = blockIdx.z;
     if (np >= Npad2) return;
@@ -168,7 +173,7 @@ k_pack_i8(const double2* __restrict__ g1, long long ld, long long strideS, int N
     const size_t o = i8_tiled_off(np, r0, I8Cfg::BN, Kpad / I8Cfg::KC);
 #pragma unroll
     for (int i = 0; i < 6; ++i)
-        *reinterpret_cast<int4*>(Bi8 + (size_t)slot * slot_bytes + (size_t)i * plane_bytes + o) = *reinterpret_cast<const int4*>(dd[i]);
+        *reinterpret_cast<int4*>(Bi8 + (size_t)slot * slot_bytes + (size_t)i * I8Cfg::B_PLANE + o) = *reinterpret_cast<const int4*>(dd[i]);
 }
 
 // ---- tcgen05 helpers (PTX ISA: tcgen05.*, sm_100a) -------------------------------------------------------------------
@@ -189,6 +194,11 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar)      // arrives on ba
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void umma_commit_mc(uint64_t* bar, uint16_t cta_mask)   // ... on bar of every CTA in cta_mask
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 :: "r"(smem_u32(bar)), "h"(cta_mask) : "memory");
+}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -200,9 +210,13 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 // C[q][n] (complex, layout CMap) = sum_r A[q][r] B'[r][(n, re|im)] from the digit planes.  M rows of A (q), N complex
 // columns, Kpad (multiple of 64) rows; Ai8 / Bi8 tiled as above (plane strides in bytes); sb = column scales of this slot.
 // rowsPerB > 0: stacked multi-k form, rows [j rowsPerB, (j+1) rowsPerB) use B slot j (rowsPerB a multiple of 128).
+// CL > 1: launched in clusters of CL CTAs that work on CL neighbouring column tiles of the SAME row tile: each CTA fetches
+// 1/CL of the A digit planes of a stage and multicasts it to the whole cluster (the A planes are 2/3 of a stage: L2 -> SM
+// traffic per tile 884 KB -> 590 KB (CL = 2), 442 KB (CL = 4)); a stage is refilled when every CTA of the cluster has
+// released it (tcgen05.commit multicast onto every CTA's empty barrier).
+template <int CL>
 __global__ void __launch_bounds__(I8Cfg::kThreads, 1)
-k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t* __restrict__ Bi8, size_t b_plane_bytes,
-              size_t b_slot_bytes, const double* __restrict__ sb, int ldsb, double scaleA, double2* __restrict__ C,
+k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, size_t b_slot_bytes, const double* __restrict__ sb, int ldsb, double scaleA, double2* __restrict__ C,
               long long ldc, int M, int N, int Kpad, int rowsPerB, int rowOffset, CMap cm)
 {
     using Cfg = I8Cfg;
@@ -216,7 +230,7 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 1);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, CL); }
         mbar_init(tfull, 1); mbar_init(tempty, 8);
         mbar_fence_init();
     }
@@ -226,30 +240,39 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CL > 1) cluster_sync_all();                     // the peers' barriers exist before anything is multicast to them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = *tmem_slot;
     const int nchunks = Kpad / KC;
     const int ntn = (2 * N + BN - 1) / BN, ntm = (M + BM - 1) / BM;
-    const int ntiles = ntn * ntm;                       // n fastest: the CTAs running together share a few A row blocks
+    // tile groups of CL neighbouring column tiles, n fastest: the CTAs running together share a few A row blocks
+    const int ntng = (ntn + CL - 1) / CL;
+    const int ngroups = ntng * ntm;
+    const int crank = CL > 1 ? (int)cluster_ctarank() : 0;
+    const int g0 = CL > 1 ? (int)cluster_id_x() : (int)blockIdx.x, gstep = CL > 1 ? (int)cluster_nid_x() : (int)gridDim.x;
+    constexpr uint16_t kMask = (uint16_t)((1u << CL) - 1u);
+    constexpr int A_STAGE = ND * Cfg::A_PLANE, B_STAGE = ND * Cfg::B_PLANE;
 
     if (warp == 0) {
-        // ================= TMA producer: twelve contiguous bulk copies per stage =================
+        // ================= TMA producer: two contiguous bulk copies per stage =================
         int s = 0; uint32_t ph = 0;
-        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int tm = tile / ntn, tn = tile - tm * ntn;
+        for (int g = g0; g < ngroups; g += gstep) {
+            const int tm = g / ntng, tn = min((g - tm * ntng) * CL + crank, ntn - 1);     // a tile past the edge re-reads the last one
             const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
-            const int8_t* a_src = Ai8 + (size_t)tm * nchunks * Cfg::A_PLANE;
-            const int8_t* b_src = Bi8 + (size_t)slot * b_slot_bytes + (size_t)tn * nchunks * Cfg::B_PLANE;
+            const int8_t* a_src = Ai8 + (size_t)tm * nchunks * A_STAGE;
+            const int8_t* b_src = Bi8 + (size_t)slot * b_slot_bytes + (size_t)tn * nchunks * B_STAGE;
             for (int c = 0; c < nchunks; ++c) {
                 mbar_wait(empty + s, ph ^ 1u);
-                if (lane == 0) mbar_arrive_expect_tx(full + s, (uint32_t)Cfg::STAGE_BYTES);
-                __syncwarp();
                 unsigned char* st = smem + (size_t)s * Cfg::STAGE_BYTES;
-                if (lane < ND)
-                    bulk_g2s(st + lane * Cfg::A_PLANE, a_src + (size_t)lane * a_plane_bytes + (size_t)c * Cfg::A_PLANE, Cfg::A_PLANE, full + s);
-                else if (lane < 2 * ND)
-                    bulk_g2s(st + ND * Cfg::A_PLANE + (lane - ND) * Cfg::B_PLANE,
-                             b_src + (size_t)(lane - ND) * b_plane_bytes + (size_t)c * Cfg::B_PLANE, Cfg::B_PLANE, full + s);
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(full + s, (uint32_t)Cfg::STAGE_BYTES);
+                    if (CL == 1) bulk_g2s(st, a_src + (size_t)c * A_STAGE, A_STAGE, full + s);
+                    else         // this CTA's 1/CL of the A planes, to every CTA of the cluster
+                        bulk_g2s_mc(st + crank * (A_STAGE / CL), a_src + (size_t)c * A_STAGE + crank * (A_STAGE / CL), A_STAGE / CL,
+                                    full + s, kMask);
+                    bulk_g2s(st + A_STAGE, b_src + (size_t)c * B_STAGE, B_STAGE, full + s);
+                }
+                __syncwarp();
                 if (++s == ST) { s = 0; ph ^= 1u; }
             }
         }
@@ -263,7 +286,7 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
         // instruction descriptor: D = S32, A = B = signed 8 bit, both K-major, M = 128, N in bits 17..22
         constexpr uint32_t idesc0 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BM >> 4) << 24);
         int s = 0; uint32_t ph = 0, tph = 0;
-        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        for (int g = g0; g < ngroups; g += gstep) {
             mbar_wait(tempty, tph ^ 1u);                 // the epilogue has read the previous tile's accumulators
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             for (int c = 0; c < nchunks; ++c) {
@@ -279,15 +302,18 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
                         for (int i = ND - 1; i >= 0; --i) {
                             const uint64_t da = umma_desc(a0 + i * Cfg::A_PLANE + ks * 256, 128, (KC / 16) * 128);
                             const int j0 = ND - 1 - i, nlev = i + 1;              // planes j0 .. 5 -> levels 0 .. i
-                            const int n1 = nlev > 4 ? 4 : nlev;                   // first instruction: levels 0 .. n1 - 1
+                            // more than four levels exceed N = 256: split 3 + rest (N = 192 + 128 / 192 runs faster than 256 + 64 / 128:
+                            // a narrow instruction is bound by its shared-memory reads of the A tile)
+                            const int n1 = nlev > 4 ? 3 : nlev;
                             umma_i8(tmem, da, umma_desc(b0 + j0 * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
                                     idesc0 | ((uint32_t)((n1 * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
                             if (nlev > 4)
-                                umma_i8(tmem + 4u * BN, da, umma_desc(b0 + (j0 + 4) * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
-                                        idesc0 | ((uint32_t)(((nlev - 4) * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
+                                umma_i8(tmem + 3u * BN, da, umma_desc(b0 + (j0 + 3) * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
+                                        idesc0 | ((uint32_t)(((nlev - 3) * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
                         }
                     }
-                    umma_commit(empty + s);               // frees the stage when these MMAs have read it
+                    // frees the stage (in every CTA of the cluster) when these MMAs have read it
+                    if (CL == 1) umma_commit(empty + s); else umma_commit_mc(empty + s, kMask);
                     if (c == nchunks - 1) umma_commit(tfull);
                 }
                 __syncwarp();
@@ -303,8 +329,8 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
         const int wq = warp & 3, half = (warp - 2) >> 2;
         uint32_t tph = 0;
         const double kscale = scaleA * 5.551115123125783e-17;        // 2^-54
-        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int tm = tile / ntn, tn = tile - tm * ntn;
+        for (int g = g0; g < ngroups; g += gstep) {
+            const int tm = g / ntng, tn = (g - tm * ntng) * CL + crank;             // tn >= ntn: nothing to store
             const int m = tm * BM + wq * 32 + lane;
             const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
             const int ncol = tn * (BN / 2) + half * 16 + (lane & 15);    // this lane's complex column (lanes 16..31 mirror)
@@ -324,7 +350,11 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
                 for (int e = 0; e < 16; ++e) {
                     const long long lo = (long long)(int)v[0][e] + ((long long)(int)v[1][e] << 8) + ((long long)(int)v[2][e] << 16);
                     const long long hi = (long long)(int)v[3][e] + ((long long)(int)v[4][e] << 8) + ((long long)(int)v[5][e] << 16);
-                    val[rd * 16 + e] = fma((double)hi, 16777216.0, (double)lo);   // exact up to the one final rounding
+                    // int64 -> double on the integer pipe plus one DADD (instead of I2F.F64.S64): for |x| < 2^51
+                    // the bit pattern of 1.5 * 2^52 plus x IS the double 1.5 * 2^52 + x; with the exponent raised by 24, + 2^24 x
+                    const double lod = __longlong_as_double(lo + 0x4338000000000000LL) - 6755399441055744.0;
+                    const double hid = __longlong_as_double(hi + 0x4338000000000000LL + (24LL << 52)) - 6755399441055744.0 * 16777216.0;
+                    val[rd * 16 + e] = hid + lod;                  // = hi 2^24 + lo, exact up to this one rounding
                 }
             }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -342,6 +372,7 @@ k_contract_i8(const int8_t* __restrict__ Ai8, size_t a_plane_bytes, const int8_t
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CL > 1) cluster_sync_all();                     // no CTA leaves while a peer may still multicast into it
     if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(Cfg::TMEM_COLS));
 }
 

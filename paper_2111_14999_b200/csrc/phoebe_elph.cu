@@ -196,6 +196,8 @@ struct phoebe_elph_ctx {
     bool Bi8_stale = true;    // the digit planes of g1' must be rebuilt (as g1P_stale)
     double i8_scaleA = 2.0;   // power-of-two scale of the phase matrix: 2 x the largest weight 1/deg_p, rounded up
     int last_i8 = -1;
+    int i8_cluster = 0;       // tuning "i8_cluster": 0 = choose, 1 / 2 / 4 = CTAs per cluster of the INT8 contraction (A planes multicast)
+    int last_i8_cluster = 0;
     bool last_fold = false;   // the last contraction went through the fold-capable launch sequence
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -674,7 +676,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             PE_CUDA(c, cudaGetLastError());
             pe::k_pack_i8<<<dim3(ceil_div(i8_Npad2, 128), i8_Kpad / 16, c->nk_have), 128, 0, c->stream>>>(
                 c->g1_base, (long long)N, (long long)c->L.g1_stride, N, i8_Npad2, c->pair_Kr, i8_Kpad, c->pair_pa, c->pair_pb,
-                c->pair_kind, cmax, sbv, c->L.i8_ldsb, Bi8, c->L.i8_b_plane, 6 * c->L.i8_b_plane);
+                c->pair_kind, cmax, sbv, c->L.i8_ldsb, Bi8, 6 * c->L.i8_b_plane);
             PE_CUDA(c, cudaGetLastError());
             c->Bi8_stale = false;
         }
@@ -724,7 +726,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
             if (use_i8) {
                 pe::k_qphase_i8<<<dim3(ceil_div(ncols, 128), c->pair_Kc4 / 16), 128, 0, c->stream>>>(
                     q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc, c->pair_Kc4, nqs, i8_Kpad, c->L.ldq,
-                    c->phase_sign, 1.0 / c->i8_scaleA, Ai8, c->L.i8_a_plane);
+                    c->phase_sign, 1.0 / c->i8_scaleA, Ai8);
             } else if (use_pair) {
                 dim3 grid(ceil_div(ncols, 256), std::min(c->pair_Kc4, 64));
                 pe::k_qphase_pair<<<grid, 256, 0, c->stream>>>(q + 3 * (size_t)qs, c->pair_R, c->pair_w, c->pair_K2, c->pair_Kc,
@@ -752,13 +754,42 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 g.strideBrow = (long long)c->L.g1_stride;
             }
             if (use_i8) {
-                PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_i8, pe::I8Cfg::kSmemBytes));
-                const int ntiles = ceil_div(nqs, pe::I8Cfg::BM) * ceil_div(2 * N, pe::I8Cfg::BN);
-                pe::k_contract_i8<<<std::min(ntiles, kSMs), pe::I8Cfg::kThreads, pe::I8Cfg::kSmemBytes, c->stream>>>(
-                    Ai8, c->L.i8_a_plane, Bi8 + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * 6 * c->L.i8_b_plane, c->L.i8_b_plane,
-                    6 * c->L.i8_b_plane, sbv + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * c->L.i8_ldsb, c->L.i8_ldsb, c->i8_scaleA,
-                    c->C, ldcq, nqs, N, i8_Kpad, rows_per_k, qs, cm);
-                PE_CUDA(c, cudaGetLastError());
+                // clusters of CL CTAs share the A digit planes of a row tile by multicast (contract_i8.cuh): tuning "i8_cluster"
+                const int ntm8 = ceil_div(nqs, pe::I8Cfg::BM), ntn8 = ceil_div(2 * N, pe::I8Cfg::BN);
+                int CL = c->i8_cluster;
+                if (CL != 1 && CL != 2 && CL != 4) CL = 1;       // measured (4-atom, band-window, large): multicast does not pay, L2 is not the limit
+                const void* kfn = CL == 4 ? (const void*)pe::k_contract_i8<4> : CL == 2 ? (const void*)pe::k_contract_i8<2>
+                                                                                      : (const void*)pe::k_contract_i8<1>;
+                PE_CUDA(c, ensure_smem_optin(kfn, pe::I8Cfg::kSmemBytes));
+                const int ngroups = ntm8 * ceil_div(ntn8, CL);
+                cudaLaunchConfig_t cfg = {};
+                cfg.blockDim = dim3(pe::I8Cfg::kThreads);
+                cfg.dynamicSmemBytes = pe::I8Cfg::kSmemBytes;
+                cfg.stream = c->stream;
+                cudaLaunchAttribute attr[1];
+                attr[0].id = cudaLaunchAttributeClusterDimension;
+                attr[0].val.clusterDim.x = CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+                cfg.attrs = attr; cfg.numAttrs = CL > 1 ? 1 : 0;
+                int nclusters = kSMs / CL;
+                if (CL > 1) {           // clusters that can be resident at once (a GPC's SM count need not be a multiple of CL)
+                    cfg.gridDim = dim3(kSMs / CL * CL);
+                    int nc = 0;
+                    PE_CUDA(c, cudaOccupancyMaxActiveClusters(&nc, kfn, &cfg));
+                    if (nc > 0) nclusters = std::min(nclusters, nc);
+                }
+                cfg.gridDim = dim3(std::min(ngroups, nclusters) * CL);
+                const int8_t* Bi8s = Bi8 + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * 6 * c->L.i8_b_plane;
+                const double* sbs = sbv + (size_t)(rows_per_k > 0 ? slot0 : c->k_sel) * c->L.i8_ldsb;
+                const int8_t* Ai8c = Ai8;
+                size_t b_sl = 6 * c->L.i8_b_plane;
+                int ldsb = c->L.i8_ldsb, Mi = nqs, Ni = N, Kp = i8_Kpad, rpk = rows_per_k, ro = qs;
+                double sA = c->i8_scaleA;
+                double2* Cp = c->C;
+                long long ldc8 = ldcq;
+                pe::CMap cm8 = cm;
+                void* kargs[] = {&Ai8c, &Bi8s, &b_sl, &sbs, &ldsb, &sA, &Cp, &ldc8, &Mi, &Ni, &Kp, &rpk, &ro, &cm8};
+                PE_CUDA(c, cudaLaunchKernelExC(&cfg, kfn, kargs));
+                c->last_i8_cluster = CL;
             } else if (use_pair) {
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair<false>, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
@@ -1574,6 +1605,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold")) { c->qfold = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "i8")) { c->i8 = value != 0 ? 1 : 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8_cluster")) { c->i8_cluster = (value == 1 || value == 2 || value == 4) ? value : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "setk_pair")) { c->setk_pair = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_blk")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
@@ -1612,7 +1644,8 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
         return PHOEBE_ELPH_OK;
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
-    if (!strcmp(key, "i8")) { *value = c->last_i8 < 0 ? c->i8 : c->last_i8; return PHOEBE_ELPH_OK; }   // did the last a4 run on INT8
+    if (!strcmp(key, "i8")) { *value = c->last_i8 < 0 ? c->i8 : c->last_i8; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8_cluster")) { *value = c->last_i8_cluster ? c->last_i8_cluster : c->i8_cluster; return PHOEBE_ELPH_OK; }   // did the last a4 run on INT8
     // ring rows of the a1 pair form (2 per +R / -R pair of the Re list) if the LAST set_k_batch used it, else 0
     if (!strcmp(key, "setk_pair_rows")) { *value = c->last_setk_pair ? 2 * c->npairE : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold_reps")) {       // representatives of the last q_batch call if it took the fold, else 0
