@@ -101,7 +101,8 @@ def test_ragged_small_cases(env, case, host):
 
 
 @pytest.mark.parametrize("knob", [{"tile": 32, "m3": 0}, {"tile": 64, "m3": 0}, {"tile": 32, "m3": 1},
-                                  {"tile": 64, "m3": 1}, {"tile": 64, "m3": 1, "planar": 0}, {"rot_plain": 1}, {"tile": 64, "pair": 2}, {"tile": 64, "pair": 0}],
+                                  {"tile": 64, "m3": 1}, {"tile": 64, "m3": 1, "planar": 0}, {"rot_plain": 1}, {"tile": 64, "pair": 2}, {"tile": 64, "pair": 0},
+                                  {"tile": 64, "pair": 2, "i8": 0}, {"tile": 64, "pair": 2, "i8": 1, "i8_cluster": 2}],
                          ids=lambda k: "_".join("%s%d" % kv for kv in k.items()))
 def test_forced_kernel_variants(env, knob):
     """Every kernel variant the dispatcher can pick is parity-checked on the same input."""
