@@ -324,6 +324,14 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               pairs (4 Kr < 6 nRp, Kr = real rows: 2 per pair or partner-less vector, 1 for R = 0); 0 = never; 2 = whenever
  *               the rows fit the operand buffers (Kr <= 1.5 nRp).  get_tuning("pair_rows") = Kr if the last contraction
  *               launch used the form, else 0.   "pair_ctas" 1 | 2 = persistent CTAs per SM of that kernel
+ *   "i8"        1 (default) = the pair form of a4 runs on the INT8 tensor cores (tcgen05.mma kind::i8, accumulators in
+ *               TMEM) by EXACT digit splitting: each FP64 operand is rounded to 48 bits relative to a power-of-two scale
+ *               (one for the phase matrix, one per column of g1') and written as six signed base-256 digits; the 21 digit
+ *               pairs of weight >= 256^5 are INT8 GEMMs with exact INT32 accumulation, recombined in 64-bit integers and
+ *               rounded once.  Normwise error ~1e-13 of a column's largest entry, results
+ *               bit-reproducible.  Taken whenever the pair form is and (stacked forms) the rows per k-point are a multiple
+ *               of 128; 0 = the FP64 tensor-core pair kernel.  get_tuning("i8") = 1 if the LAST contraction ran on INT8.
+ *               "i8_cluster" 0 | 1 (default) | 2 | 4 = CTAs per cluster of that kernel (the A digit planes multicast)
  *   "qfold"     1 = q lists that contain -q with q (uniform meshes; modulo a reciprocal lattice vector when all Rp are
  *               integer vectors) are contracted once per (q, -q) pair: the cosine rows of the pair form are even in q, the
  *               sine rows odd, C(+-q) = Ce +- Co.  The pairs are found on the device in every q_batch call (no host round
