@@ -359,6 +359,32 @@ const char* phoebe_elph_last_error(const phoebe_elph_ctx* ctx);
 
 const char* phoebe_elph_version(void);
 
+/* ---- Allocation-free variant of set_k (a1 + a2, Eq. 71) -------------------------------------------------
+ * For callers that cannot allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * No context, no workspace: the Fourier-summed, not yet rotated tensor T[nRp][nw][nw][nmodes] (the scratch the context-based
+ * path keeps in the caller's workspace) lives in a file-scope device array of PHOEBE_ELPH_NOALLOC_MAX_BYTES inside the
+ * library -- every GPU that loads the library holds it until the process exits.  The call launches two kernels on
+ * cuda_stream and returns without synchronising; it calls no cudaMalloc / cudaFree and no allocating library routine.
+ *   gW_dev     DEVICE complex128 [nRp][nRe][nw][nw][nmodes], 16-B aligned (as in phoebe_elph_setup); read once
+ *   Re_dev     DEVICE double [nRe][3] (crystal coordinates);  deg_e_dev DEVICE double [nRe] or NULL (= all 1)
+ *   k_host     HOST double [3], read before the call returns
+ *   Uk_dev     DEVICE complex128 [nw][nb1];  g1_out_dev DEVICE complex128 [nRp][nb1][nw][nmodes], written (caller-owned)
+ * Conventions: those of a fresh context (phase_sign = +1, U_k not conjugated).
+ * LIMIT: nRp * nw * nw * nmodes * 16 bytes <= PHOEBE_ELPH_NOALLOC_MAX_BYTES (e.g. the si-like cell: 343 * 8 * 8 * 6 * 16 =
+ * 2.1 MB); larger problems are rejected with E_DIMS and a text that says so -- use phoebe_elph_set_k with a workspace.
+ * SHARING: every call on a device uses the SAME array, which keeps the last call's contents (each call writes every element
+ * before reading it, so nothing needs clearing); calls that overlap on the GPU (two streams, concurrently replayed graphs)
+ * RACE on it: serialise them.
+ * phoebe_elph_noalloc_setup(): looks up the array's device address for the CURRENT device (once per device; the first use
+ * of a device may load the module): call it once per device before capturing; set_k_noalloc does the same lookup lazily.
+ * Errors: E_NULL, E_DIMS, E_ALIGN, E_CUDA; text via phoebe_elph_noalloc_last_error() (per host thread). */
+#define PHOEBE_ELPH_NOALLOC_MAX_BYTES (4u << 20)
+int phoebe_elph_noalloc_setup(void);
+int phoebe_elph_set_k_noalloc(const void* gW_dev, const double* Re_dev, const double* deg_e_dev, int32_t nRe, int32_t nRp,
+                              int32_t nw, int32_t nmodes, int32_t nb1, const double* k_host, const void* Uk_dev,
+                              void* g1_out_dev, void* cuda_stream);
+const char* phoebe_elph_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -27,6 +27,7 @@ EXPORTS = [
     "phoebe_elph_profile", "phoebe_elph_profile_read", "phoebe_elph_set_tuning", "phoebe_elph_get_tuning",
     "phoebe_elph_destroy", "phoebe_elph_last_error",
     "phoebe_elph_version",
+    "phoebe_elph_noalloc_setup", "phoebe_elph_set_k_noalloc", "phoebe_elph_noalloc_last_error",
 ]
 
 ERRORS = {0: "OK", -1: "E_NULL", -2: "E_DIMS", -3: "E_ALIGN", -4: "E_NO_K", -5: "E_WORKSPACE", -6: "E_CUDA"}
@@ -95,12 +96,51 @@ def load_library() -> ctypes.CDLL:
     lib.phoebe_elph_last_error.argtypes = [c_void_p]
     lib.phoebe_elph_last_error.restype = c_char_p
     lib.phoebe_elph_version.restype = c_char_p
+    lib.phoebe_elph_noalloc_setup.argtypes = []
+    lib.phoebe_elph_set_k_noalloc.argtypes = [c_void_p, c_void_p, c_void_p] + [c_int32] * 5 + [c_void_p] * 4
+    lib.phoebe_elph_noalloc_last_error.restype = c_char_p
     _lib = lib
     return lib
 
 
 def version() -> str:
     return load_library().phoebe_elph_version().decode()
+
+
+NOALLOC_MAX_BYTES = 4 << 20       # PHOEBE_ELPH_NOALLOC_MAX_BYTES of include/phoebe_elph.h
+
+
+def noalloc_setup():
+    """phoebe_elph_noalloc_setup: resolve the fixed scratch array's address on the current device (once per device)."""
+    lib = load_library()
+    rc = lib.phoebe_elph_noalloc_setup()
+    if rc:
+        raise PhoebeElphError(rc, "phoebe_elph_noalloc_setup", lib.phoebe_elph_noalloc_last_error().decode())
+
+
+def set_k_noalloc(gW, Re, deg_e, k, Uk, g1_out, stream=None):
+    """phoebe_elph_set_k_noalloc (a1 + a2 without context, workspace or allocation): gW [nRp][nRe][nw][nw][nm] complex128,
+    Re [nRe][3] float64, deg_e [nRe] float64 or None, Uk [nw][nb1] complex128, g1_out [nRp][nb1][nw][nm] complex128 -- all
+    CUDA tensors; k: three host floats.  Marshalling only; raises PhoebeElphError."""
+    import numpy as np
+    import torch
+    lib = load_library()
+    for name, t, dt in (("gW", gW, torch.complex128), ("Re", Re, torch.float64), ("Uk", Uk, torch.complex128),
+                        ("g1_out", g1_out, torch.complex128)) + ((("deg_e", deg_e, torch.float64),) if deg_e is not None else ()):
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise TypeError(f"set_k_noalloc: {name} must be a contiguous CUDA tensor of dtype {dt}")
+    nRp, nRe, nw, _, nm = gW.shape
+    nb1 = Uk.shape[1]
+    if tuple(Re.shape) != (nRe, 3) or Uk.shape[0] != nw or tuple(g1_out.shape) != (nRp, nb1, nw, nm):
+        raise ValueError("set_k_noalloc: inconsistent shapes")
+    k_arr = np.ascontiguousarray(k, dtype=np.float64)
+    if k_arr.shape != (3,):
+        raise ValueError("set_k_noalloc: k must be three numbers")
+    s = stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = lib.phoebe_elph_set_k_noalloc(gW.data_ptr(), Re.data_ptr(), deg_e.data_ptr() if deg_e is not None else None, nRe, nRp,
+                                       nw, nm, nb1, k_arr.ctypes.data, Uk.data_ptr(), g1_out.data_ptr(), s)
+    if rc:
+        raise PhoebeElphError(rc, "phoebe_elph_set_k_noalloc", lib.phoebe_elph_noalloc_last_error().decode())
 
 
 def workspace_bytes(dims: Dims, hbm_budget_bytes: int):

@@ -25,6 +25,7 @@ def _deps():
 
 OBJ_DIR = os.path.join(HERE, "build")
 ROT3_SRC = os.path.join(HERE, "csrc", "rot3_instances.cu")
+NOALLOC_SRC = os.path.join(HERE, "csrc", "noalloc.cu")       # phoebe_elph_set_k_noalloc: fixed device scratch, no workspace
 ROT3_PARTS = 4
 
 
@@ -45,6 +46,8 @@ def nvcc_cmds(verbose: bool = False):
     objs = [os.path.join(OBJ_DIR, "phoebe_elph.o")] + [os.path.join(OBJ_DIR, "rot3_part%d.o" % i) for i in range(ROT3_PARTS)]
     compiles = [base + ["-c", SRC, "-o", objs[0]]]
     compiles += [base + ["-DROT3_PART=%d" % i, "-c", ROT3_SRC, "-o", objs[1 + i]] for i in range(ROT3_PARTS)]
+    objs.append(os.path.join(OBJ_DIR, "noalloc.o"))
+    compiles.append(base + ["-c", NOALLOC_SRC, "-o", objs[-1]])
     compiles.append(base + ["-shared", "-o", PROBES_LIB, PROBES_SRC])
     link = [base[0], "-shared", "-o", LIB] + objs
     return compiles, link
