@@ -17,7 +17,7 @@
 // ring stage is TWO contiguous 1-D bulk copies (the TMA unit takes ~100 clk per bulk request whatever its size):
 //   A digits  Ai8[m tile of 128][k chunk KC][d][row group 16][k group KC/16][8 rows][16 bytes]      (k_qphase_i8)
 //   B digits  Bi8[slot][n' tile of 64][k chunk KC][d][col group 8][k group KC/16][8 cols][16 bytes]  (k_pack_i8)
-// Kernel: warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warps 2..9 = epilogue (TMEM -> registers -> C).
+// Kernel: warps 0..15 = epilogue (TMEM -> registers -> C), warp 16 = TMA producer, warp 17 = MMA issuer (one thread).
 #pragma once
 #include "ptx_helpers.cuh"
 
@@ -28,7 +28,11 @@ struct I8Cfg {
 #define PHOEBE_I8_KC 32
 #endif
     static constexpr int BM = 128, BN = 64, KC = PHOEBE_I8_KC, ND = 6, NLEV = 6, STAGES = 216 * 1024 / (ND * (BM + BN) * KC);
-    static constexpr int kThreads = 10 * 32;
+    static constexpr int EPI_WARPS = 16;
+    // warps 0..15 = epilogue (four warpgroups), warps 16..19 = the control warpgroup: 16 = TMA producer, 17 = MMA issuer,
+    // 18, 19 idle.  The register file is re-split at kernel start (setmaxnreg; pool = 640 threads x 96 at launch):
+    // 512 x 112 + 128 x 32 = 61440.
+    static constexpr int kThreads = (EPI_WARPS + 4) * 32, PW = EPI_WARPS, REGS_EPI = 112, REGS_CTRL = 32;
     static constexpr int A_PLANE = BM * KC, B_PLANE = BN * KC;                    // bytes of one digit plane of a stage
     static constexpr int STAGE_BYTES = ND * (A_PLANE + B_PLANE);                 // 72 KB
     static constexpr size_t kSmemBytes = (size_t)STAGES * STAGE_BYTES + 1024 + 256;   // + alignment slack + barriers
@@ -231,10 +235,10 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, CL); }
-        mbar_init(tfull, 1); mbar_init(tempty, 8);
+        mbar_init(tfull, 1); mbar_init(tempty, Cfg::EPI_WARPS);
         mbar_fence_init();
     }
-    if (warp == 1) {
+    if (warp == Cfg::PW + 1) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(tmem_slot)), "r"(Cfg::TMEM_COLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
@@ -253,7 +257,9 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
     constexpr uint16_t kMask = (uint16_t)((1u << CL) - 1u);
     constexpr int A_STAGE = ND * Cfg::A_PLANE, B_STAGE = ND * Cfg::B_PLANE;
 
-    if (warp == 0) {
+    if (warp >= Cfg::PW) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(Cfg::REGS_CTRL));
+    if (warp == Cfg::PW) {
         // ================= TMA producer: two contiguous bulk copies per stage =================
         int s = 0; uint32_t ph = 0;
         for (int g = g0; g < ngroups; g += gstep) {
@@ -276,7 +282,7 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
                 if (++s == ST) { s = 0; ph ^= 1u; }
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == Cfg::PW + 1) {
         // ================= MMA issuer (one thread) =================
         // Digit plane A_i meets the B' planes j = 5 - i .. 5, whose products belong to the levels 0 .. i: the planes are
         // contiguous in the stage and the level accumulators contiguous in TMEM, so ONE instruction with N = 64 (i + 1)
@@ -321,59 +327,63 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
             }
             tph ^= 1u;
         }
+    }
     } else {
-        // ================= epilogue warps (8): TMEM lanes 32 (warp % 4) .. + 31 = rows; half h = 32 real columns ========
-        // Phase A reads the six levels of the warp's 32 columns and recombines them (exactly, in 64-bit integers) into 32
-        // doubles held in registers, then hands the accumulators back to the MMA warp; phase B scales and stores while the
-        // next tile's MMAs run.  Column offsets (CMap) and scales are computed once per tile by lanes 0..15 and broadcast.
-        const int wq = warp & 3, half = (warp - 2) >> 2;
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::REGS_EPI));
+        // ================= epilogue warps (16): TMEM lanes 32 (warp % 4) .. + 31 = rows; column group cg = 16 real columns ===
+        // Each warp pulls the six levels of its 32 x 16 block into registers (96 raw INT32 per thread) and hands the
+        // accumulators back to the MMA warp AT ONCE: only the TMEM read-out itself is not overlapped with the next tile's
+        // MMAs (six levels x 64 columns = 384 of the 512 TMEM columns leave no room for a second accumulator set).  The exact
+        // recombination in 64-bit integers, the scaling and the stores then run beside the MMAs.  Column offsets (CMap) and
+        // scales are computed once per tile by lanes 0..7 and broadcast.
+        constexpr int CW = BN / (Cfg::EPI_WARPS / 4);               // real columns per warp: 16
+        static_assert(CW == 16, "one tcgen05.ld 32x32b.x16 per level and warp");
+        const int wq = warp & 3, cg = warp >> 2;
         uint32_t tph = 0;
         const double kscale = scaleA * 5.551115123125783e-17;        // 2^-54
         for (int g = g0; g < ngroups; g += gstep) {
             const int tm = g / ntng, tn = (g - tm * ntng) * CL + crank;             // tn >= ntn: nothing to store
             const int m = tm * BM + wq * 32 + lane;
             const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
-            const int ncol = tn * (BN / 2) + half * 16 + (lane & 15);    // this lane's complex column (lanes 16..31 mirror)
+            const int ncol = tn * (BN / 2) + cg * (CW / 2) + (lane & 7);    // this lane's complex column (lanes 8..31 mirror)
             long long off_l = -1; double sc_l = 0.0;
             if (ncol < N) { off_l = cmap_off(ncol, cm); sc_l = kscale * sb[(size_t)slot * ldsb + ncol]; }
-            double val[32];
+            uint32_t v[Cfg::NLEV][16];
             mbar_wait(tfull, tph);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-            for (int rd = 0; rd < 2; ++rd) {
-                uint32_t v[Cfg::NLEV][16];
-#pragma unroll
-                for (int l = 0; l < Cfg::NLEV; ++l)
-                    tmem_ld16(tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)(l * BN + half * 32 + rd * 16), v[l]);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const long long lo = (long long)(int)v[0][e] + ((long long)(int)v[1][e] << 8) + ((long long)(int)v[2][e] << 16);
-                    const long long hi = (long long)(int)v[3][e] + ((long long)(int)v[4][e] << 8) + ((long long)(int)v[5][e] << 16);
-                    // int64 -> double on the integer pipe plus one DADD (instead of I2F.F64.S64): for |x| < 2^51
-                    // the bit pattern of 1.5 * 2^52 plus x IS the double 1.5 * 2^52 + x; with the exponent raised by 24, + 2^24 x
-                    const double lod = __longlong_as_double(lo + 0x4338000000000000LL) - 6755399441055744.0;
-                    const double hid = __longlong_as_double(hi + 0x4338000000000000LL + (24LL << 52)) - 6755399441055744.0 * 16777216.0;
-                    val[rd * 16 + e] = hid + lod;                  // = hi 2^24 + lo, exact up to this one rounding
-                }
-            }
+            for (int l = 0; l < Cfg::NLEV; ++l)
+                tmem_ld16(tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)(l * BN + cg * CW), v[l]);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty);
             tph ^= 1u;
             double2* crow = C + (size_t)min(m, M - 1) * ldc;
 #pragma unroll
-            for (int jc = 0; jc < 16; ++jc) {
+            for (int jc = 0; jc < CW / 2; ++jc) {
+                double val[2];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int e = 2 * jc + h;
+                    const long long lo = (long long)(int)v[0][e] + ((long long)(int)v[1][e] << 8) + ((long long)(int)v[2][e] << 16);
+                    const long long hi = (long long)(int)v[3][e] + ((long long)(int)v[4][e] << 8) + ((long long)(int)v[5][e] << 16);
+                    // int64 -> double on the integer pipe plus one DADD (instead of I2F.F64.S64): for |x| < 2^51
+                    // the bit pattern of 1.5 * 2^52 plus x IS the double 1.5 * 2^52 + x; with the exponent raised by 24, + 2^24 x
+                    const double lod = __longlong_as_double(lo + 0x4338000000000000LL) - 6755399441055744.0;
+                    const double hid = __longlong_as_double(hi + 0x4338000000000000LL + (24LL << 52)) - 6755399441055744.0 * 16777216.0;
+                    val[h] = hid + lod;                            // = hi 2^24 + lo, exact up to this one rounding
+                }
                 const long long off = __shfl_sync(0xffffffffu, off_l, jc);
                 const double sc = __shfl_sync(0xffffffffu, sc_l, jc);
-                if (m < M && off >= 0) crow[off] = make_double2(val[2 * jc] * sc, val[2 * jc + 1] * sc);
+                if (m < M && off >= 0) crow[off] = make_double2(val[0] * sc, val[1] * sc);
             }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     if (CL > 1) cluster_sync_all();                     // no CTA leaves while a peer may still multicast into it
-    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(Cfg::TMEM_COLS));
+    if (warp == Cfg::PW + 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(Cfg::TMEM_COLS));
 }
 
 }  // namespace pe
