@@ -523,6 +523,7 @@ def run_ours(args):
             elif bound == "tensor":
                 f64_flop = counts["contract_flop_4m"] * n_k / contract_launches
                 kernels[kind].update(bound="tensor", achieved=work / dur / 1e12, peak=int8_peak_tops, unit="TOP/s", dtype="s8",
+                                     grid_ctas=ctx.get_tuning("i8_grid"), cluster=ctx.get_tuning("i8_cluster"),
                                      int8_nominal_peak_tops=4500.0, frac_of_nominal=work / dur / 1e12 / 4500.0,
                                      fp64_equivalent_tflops=f64_flop / dur / 1e12,
                                      fp64_equivalent_over_fp64_peak=f64_flop / dur / 1e12 / FP64_PEAK_TFLOPS)

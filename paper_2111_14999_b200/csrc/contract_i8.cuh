@@ -287,8 +287,9 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
         // Digit plane A_i meets the B' planes j = 5 - i .. 5, whose products belong to the levels 0 .. i: the planes are
         // contiguous in the stage and the level accumulators contiguous in TMEM, so ONE instruction with N = 64 (i + 1)
         // does all of them and reads the A tile from shared memory once (the unit's limit is N <= 256: i = 4 and 5 take two).
-        // Shared-memory reads per 32-deep step: 75 KB instead of the 126 KB of 21 single-level instructions -- below the
-        // 128 B/clk the tensor pipe's own time (693 clk) allows.
+        // Shared-memory reads per 32-deep step: 75 KB instead of the 126 KB of 21 single-level instructions.  With the 36 KB
+        // the TMA unit writes per step that is 111 KB = 867 clk at the SM's 128 B/clk, against 725 clk of tensor-pipe time:
+        // the kernel is bound by shared-memory bandwidth (measured: 925-966 clk per step, tensor pipe 68 % active).
         // instruction descriptor: D = S32, A = B = signed 8 bit, both K-major, M = 128, N in bits 17..22
         constexpr uint32_t idesc0 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BM >> 4) << 24);
         int s = 0; uint32_t ph = 0, tph = 0;

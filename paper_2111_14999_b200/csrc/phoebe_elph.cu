@@ -196,8 +196,8 @@ struct phoebe_elph_ctx {
     bool Bi8_stale = true;    // the digit planes of g1' must be rebuilt (as g1P_stale)
     double i8_scaleA = 2.0;   // power-of-two scale of the phase matrix: 2 x the largest weight 1/deg_p, rounded up
     int last_i8 = -1;
-    int i8_cluster = 0;       // tuning "i8_cluster": 0 = choose, 1 / 2 / 4 = CTAs per cluster of the INT8 contraction (A planes multicast)
-    int last_i8_cluster = 0;
+    int i8_cluster = 0;       // tuning "i8_cluster": 0 = choose, 1 / 2 / 4 / 8 = CTAs per cluster of the INT8 contraction (A planes multicast)
+    int last_i8_cluster = 0, last_i8_grid = 0;
     bool last_fold = false;   // the last contraction went through the fold-capable launch sequence
     // q_batch_host_async: copy-in / copy-out streams and the events that chain them to the compute stream
     cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -758,9 +758,9 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 // clusters of CL CTAs share the A digit planes of a row tile by multicast (contract_i8.cuh): tuning "i8_cluster"
                 const int ntm8 = ceil_div(nqs, pe::I8Cfg::BM), ntn8 = ceil_div(2 * N, pe::I8Cfg::BN);
                 int CL = c->i8_cluster;
-                if (CL != 1 && CL != 2 && CL != 4) CL = 1;       // measured (4-atom, band-window, large): multicast does not pay, L2 is not the limit
-                const void* kfn = CL == 4 ? (const void*)pe::k_contract_i8<4> : CL == 2 ? (const void*)pe::k_contract_i8<2>
-                                                                                      : (const void*)pe::k_contract_i8<1>;
+                if (CL != 1 && CL != 2 && CL != 4 && CL != 8) CL = 1;       // measured (4-atom, band-window, large): 2 and 4 change nothing; 8 is 12 % faster per CTA but only 15 clusters (120 CTAs) fit
+                const void* kfn = CL == 8 ? (const void*)pe::k_contract_i8<8> : CL == 4 ? (const void*)pe::k_contract_i8<4>
+                                : CL == 2 ? (const void*)pe::k_contract_i8<2> : (const void*)pe::k_contract_i8<1>;
                 PE_CUDA(c, ensure_smem_optin(kfn, pe::I8Cfg::kSmemBytes));
                 const int ngroups = ntm8 * ceil_div(ntn8, CL);
                 cudaLaunchConfig_t cfg = {};
@@ -791,6 +791,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                 void* kargs[] = {&Ai8c, &Bi8s, &b_sl, &sbs, &ldsb, &sA, &Cp, &ldc8, &Mi, &Ni, &Kp, &rpk, &ro, &cm8};
                 PE_CUDA(c, cudaLaunchKernelExC(&cfg, kfn, kargs));
                 c->last_i8_cluster = CL;
+                c->last_i8_grid = (int)cfg.gridDim.x;
             } else if (use_pair) {
                 PE_CUDA(c, ensure_smem_optin((const void*)pe::k_contract_pair<false>, pe::PairCfg::kSmemBytes));
                 const int ntiles = ceil_div(nqs, 64) * ceil_div(N, 64);
@@ -1606,7 +1607,7 @@ int phoebe_elph_set_tuning(phoebe_elph_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "rot_plain")) { c->rot_plain = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold")) { c->qfold = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "i8")) { c->i8 = value != 0 ? 1 : 0; return PHOEBE_ELPH_OK; }
-    if (!strcmp(key, "i8_cluster")) { c->i8_cluster = (value == 1 || value == 2 || value == 4) ? value : 0; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8_cluster")) { c->i8_cluster = (value == 1 || value == 2 || value == 4 || value == 8) ? value : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "setk_pair")) { c->setk_pair = value != 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "rot_blk")) {
         if (value < 0 || value > 2) return fail(c, PHOEBE_ELPH_E_DIMS, "rot_blk must be 0, 1 or 2");
@@ -1646,7 +1647,8 @@ int phoebe_elph_get_tuning(const phoebe_elph_ctx* c, const char* key, int64_t* v
     }
     if (!strcmp(key, "s_alloc")) { *value = c->L.S_alloc; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "i8")) { *value = c->last_i8 < 0 ? c->i8 : c->last_i8; return PHOEBE_ELPH_OK; }
-    if (!strcmp(key, "i8_cluster")) { *value = c->last_i8_cluster ? c->last_i8_cluster : c->i8_cluster; return PHOEBE_ELPH_OK; }   // did the last a4 run on INT8
+    if (!strcmp(key, "i8_cluster")) { *value = c->last_i8_cluster ? c->last_i8_cluster : c->i8_cluster; return PHOEBE_ELPH_OK; }
+    if (!strcmp(key, "i8_grid")) { *value = c->last_i8_grid; return PHOEBE_ELPH_OK; }      // CTAs of the last INT8 contraction launch   // did the last a4 run on INT8
     // ring rows of the a1 pair form (2 per +R / -R pair of the Re list) if the LAST set_k_batch used it, else 0
     if (!strcmp(key, "setk_pair_rows")) { *value = c->last_setk_pair ? 2 * c->npairE : 0; return PHOEBE_ELPH_OK; }
     if (!strcmp(key, "qfold_reps")) {       // representatives of the last q_batch call if it took the fold, else 0

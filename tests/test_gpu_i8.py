@@ -75,9 +75,9 @@ def test_i8_matches_oracle_and_fp64_pair_kernel(env, case):
     assert np.array_equal(out_i8, out_again)               # integer accumulation: bit-reproducible
 
 
-@pytest.mark.parametrize("cl", [1, 2, 4])
+@pytest.mark.parametrize("cl", [1, 2, 4, 8])
 def test_i8_cluster_variants_are_bit_identical(env, cl):
-    """Clusters of 1 / 2 / 4 CTAs (A digit planes multicast) compute the same integers: identical bits; an odd number of
+    """Clusters of 1 / 2 / 4 / 8 CTAs (A digit planes multicast) compute the same integers: identical bits; an odd number of
     column tiles leaves one CTA of the last cluster without a tile of its own."""
     wl, oracle, harness = env["wl"], env["oracle"], env["harness"]
     w = wl.custom(nw=6, nb1=5, nb2=6, nm=9, grid_e=(2, 2, 1), grid_p=(3, 3, 3), nq=700, cfg_id=171)   # 2 N = 540: 9 column tiles
