@@ -211,6 +211,16 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
                  : "r"(taddr));
 }
 
+// 16 TMEM lanes x 16 columns in the matrix-fragment shape: lane t gets rows t/4 and t/4 + 8, column pairs 2 (t%4) + {0, 1} and
+// 8 + 2 (t%4) + {0, 1}: r[0..1] = (row t/4, pair t%4), r[2..3] = (row t/4 + 8, same pair), r[4..7] the same for the pair 4 + t%4
+// (layout read back from the hardware with a tcgen05.st / tcgen05.ld probe)
+__device__ __forceinline__ void tmem_ld_16x256b_x2(uint32_t taddr, uint32_t (&r)[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr));
+}
+
 // C[q][n] (complex, layout CMap) = sum_r A[q][r] B'[r][(n, re|im)] from the digit planes.  M rows of A (q), N complex
 // columns, Kpad (multiple of 64) rows; Ai8 / Bi8 tiled as above (plane strides in bytes); sb = column scales of this slot.
 // rowsPerB > 0: stacked multi-k form, rows [j rowsPerB, (j+1) rowsPerB) use B slot j (rowsPerB a multiple of 128).
@@ -252,6 +262,18 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
     // tile groups of CL neighbouring column tiles, n fastest: the CTAs running together share a few A row blocks
     const int ntng = (ntn + CL - 1) / CL;
     const int ngroups = ntng * ntm;
+    // Order of the tile groups: PANELS of as many column groups as there are CTAs (clusters) in flight, all row tiles of a
+    // panel before the next panel -- a CTA keeps its column tile while the row tiles go by, so the B digits of a panel
+    // (148 x 64 columns x Kpad x 6 B <= 44 MB) stay in L2 however wide g1' is (large: 141 MB of B digits per slot were
+    // re-read from DRAM for every row tile in the plain n-fastest order: 11.7 GB per launch), and the A tile of the moment
+    // is shared by all CTAs.
+    const int pw = min(CL > 1 ? (int)cluster_nid_x() : (int)gridDim.x, ntng);
+    auto group_tile = [&](int g, int& tm, int& tng) {
+        const int per_panel = pw * ntm, panel = g / per_panel, r = g - panel * per_panel;
+        const int w = min(pw, ntng - panel * pw);          // the last panel may be narrower
+        tm = r / w;
+        tng = panel * pw + (r - tm * w);
+    };
     const int crank = CL > 1 ? (int)cluster_ctarank() : 0;
     const int g0 = CL > 1 ? (int)cluster_id_x() : (int)blockIdx.x, gstep = CL > 1 ? (int)cluster_nid_x() : (int)gridDim.x;
     constexpr uint16_t kMask = (uint16_t)((1u << CL) - 1u);
@@ -263,7 +285,9 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
         // ================= TMA producer: two contiguous bulk copies per stage =================
         int s = 0; uint32_t ph = 0;
         for (int g = g0; g < ngroups; g += gstep) {
-            const int tm = g / ntng, tn = min((g - tm * ntng) * CL + crank, ntn - 1);     // a tile past the edge re-reads the last one
+            int tm, tng;
+            group_tile(g, tm, tng);
+            const int tn = min(tng * CL + crank, ntn - 1);                          // a tile past the edge re-reads the last one
             const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
             const int8_t* a_src = Ai8 + (size_t)tm * nchunks * A_STAGE;
             const int8_t* b_src = Bi8 + (size_t)slot * b_slot_bytes + (size_t)tn * nchunks * B_STAGE;
@@ -332,52 +356,65 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Cfg::REGS_EPI));
         // ================= epilogue warps (16): TMEM lanes 32 (warp % 4) .. + 31 = rows; column group cg = 16 real columns ===
-        // Each warp pulls the six levels of its 32 x 16 block into registers (96 raw INT32 per thread) and hands the
+        // Each warp pulls the six levels of its 32 x 16 block into registers (96 raw INT32 per thread, tcgen05.ld in the
+        // 16x256b fragment shape) and hands the
         // accumulators back to the MMA warp AT ONCE: only the TMEM read-out itself is not overlapped with the next tile's
         // MMAs (six levels x 64 columns = 384 of the 512 TMEM columns leave no room for a second accumulator set).  The exact
         // recombination in 64-bit integers, the scaling and the stores then run beside the MMAs.  Column offsets (CMap) and
         // scales are computed once per tile by lanes 0..7 and broadcast.
         constexpr int CW = BN / (Cfg::EPI_WARPS / 4);               // real columns per warp: 16
-        static_assert(CW == 16, "one tcgen05.ld 32x32b.x16 per level and warp");
+        static_assert(CW == 16, "two tcgen05.ld 16x256b.x2 per level and warp");
         const int wq = warp & 3, cg = warp >> 2;
         uint32_t tph = 0;
         const double kscale = scaleA * 5.551115123125783e-17;        // 2^-54
         for (int g = g0; g < ngroups; g += gstep) {
-            const int tm = g / ntng, tn = (g - tm * ntng) * CL + crank;             // tn >= ntn: nothing to store
-            const int m = tm * BM + wq * 32 + lane;
+            int tm, tng;
+            group_tile(g, tm, tng);
+            const int tn = tng * CL + crank;                                        // tn >= ntn: nothing to store
             const int slot = rowsPerB > 0 ? (rowOffset + tm * BM) / rowsPerB : 0;
             const int ncol = tn * (BN / 2) + cg * (CW / 2) + (lane & 7);    // this lane's complex column (lanes 8..31 mirror)
             long long off_l = -1; double sc_l = 0.0;
             if (ncol < N) { off_l = cmap_off(ncol, cm); sc_l = kscale * sb[(size_t)slot * ldsb + ncol]; }
-            uint32_t v[Cfg::NLEV][16];
+            uint32_t v[Cfg::NLEV][2][8];                  // [level][16-lane half][fragment register]
             mbar_wait(tfull, tph);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
             for (int l = 0; l < Cfg::NLEV; ++l)
-                tmem_ld16(tmem + ((uint32_t)(wq * 32) << 16) + (uint32_t)(l * BN + cg * CW), v[l]);
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh)
+                    tmem_ld_16x256b_x2(tmem + ((uint32_t)(wq * 32 + 16 * hh) << 16) + (uint32_t)(l * BN + cg * CW), v[l][hh]);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty);
             tph ^= 1u;
-            double2* crow = C + (size_t)min(m, M - 1) * ldc;
+            // In the fragment shape four neighbouring lanes hold four neighbouring complex columns of ONE row: a store
+            // instruction writes 8 rows x 64 contiguous bytes (whole 32-byte sectors) instead of 32 rows x 16 bytes.
 #pragma unroll
-            for (int jc = 0; jc < CW / 2; ++jc) {
-                double val[2];
+            for (int cs = 0; cs < 2; ++cs) {
+                const int csrc = cs * 4 + (lane & 3);                   // this lane's complex column of the warp's eight
+                const long long off = __shfl_sync(0xffffffffu, off_l, csrc);
+                const double sc = __shfl_sync(0xffffffffu, sc_l, csrc);
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int e = 2 * jc + h;
-                    const long long lo = (long long)(int)v[0][e] + ((long long)(int)v[1][e] << 8) + ((long long)(int)v[2][e] << 16);
-                    const long long hi = (long long)(int)v[3][e] + ((long long)(int)v[4][e] << 8) + ((long long)(int)v[5][e] << 16);
-                    // int64 -> double on the integer pipe plus one DADD (instead of I2F.F64.S64): for |x| < 2^51
-                    // the bit pattern of 1.5 * 2^52 plus x IS the double 1.5 * 2^52 + x; with the exponent raised by 24, + 2^24 x
-                    const double lod = __longlong_as_double(lo + 0x4338000000000000LL) - 6755399441055744.0;
-                    const double hid = __longlong_as_double(hi + 0x4338000000000000LL + (24LL << 52)) - 6755399441055744.0 * 16777216.0;
-                    val[h] = hid + lod;                            // = hi 2^24 + lo, exact up to this one rounding
+                for (int hh = 0; hh < 2; ++hh) {
+#pragma unroll
+                    for (int rs = 0; rs < 2; ++rs) {
+                        const int m = tm * BM + wq * 32 + 16 * hh + 8 * rs + (lane >> 2);
+                        double val[2];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const int e = cs * 4 + rs * 2 + h;
+                            const long long lo = (long long)(int)v[0][hh][e] + ((long long)(int)v[1][hh][e] << 8) + ((long long)(int)v[2][hh][e] << 16);
+                            const long long hi = (long long)(int)v[3][hh][e] + ((long long)(int)v[4][hh][e] << 8) + ((long long)(int)v[5][hh][e] << 16);
+                            // int64 -> double on the integer pipe plus one DADD (instead of I2F.F64.S64): for |x| < 2^51
+                            // the bit pattern of 1.5 * 2^52 plus x IS the double 1.5 * 2^52 + x; with the exponent raised by 24, + 2^24 x
+                            const double lod = __longlong_as_double(lo + 0x4338000000000000LL) - 6755399441055744.0;
+                            const double hid = __longlong_as_double(hi + 0x4338000000000000LL + (24LL << 52)) - 6755399441055744.0 * 16777216.0;
+                            val[h] = hid + lod;                        // = hi 2^24 + lo, exact up to this one rounding
+                        }
+                        if (m < M && off >= 0) C[(size_t)m * ldc + off] = make_double2(val[0] * sc, val[1] * sc);
+                    }
                 }
-                const long long off = __shfl_sync(0xffffffffu, off_l, jc);
-                const double sc = __shfl_sync(0xffffffffu, sc_l, jc);
-                if (m < M && off >= 0) crow[off] = make_double2(val[0] * sc, val[1] * sc);
             }
         }
     }
