@@ -39,16 +39,36 @@ struct I8Cfg {
     static constexpr int TMEM_COLS = 512;                                        // NLEV * BN = 384 used
 };
 
-// six balanced base-256 digits of round(v * inv_scale * 2^47); |v * inv_scale| <= 1/2
-__device__ __forceinline__ void i8_digits(double v, double inv_scale, int8_t (&d)[6])
+// six balanced base-256 digits of X = round(v * inv_scale * 2^47), |v * inv_scale| <= 1/2, as the six low BYTES of the result
+// (byte i = digit i, a signed 8-bit number): with K = 128 (1 + 256 + ... + 256^5), Y = X + K is positive and below 2^48, its
+// unsigned bytes y_i give X = sum_i (y_i - 128) 256^i, and y_i - 128 as int8 is y_i ^ 0x80 -- one add and one xor instead of
+// six extract / subtract / shift rounds.
+__device__ __forceinline__ unsigned long long i8_digits_packed(double v, double inv_scale)
 {
-    long long X = __double2ll_rn(v * inv_scale * 140737488355328.0);             // 2^47
+    const long long X = __double2ll_rn(v * inv_scale * 140737488355328.0);       // 2^47
+    return ((unsigned long long)X + 0x0000808080808080ULL) ^ 0x0000808080808080ULL;
+}
+// byte i (0..3) of each of four words -> one word (a's byte lowest)
+template <int I>
+__device__ __forceinline__ uint32_t i8_pick4(uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    constexpr uint32_t sel = (uint32_t)I | ((uint32_t)(4 + I) << 4);
+    return __byte_perm(__byte_perm(a, b, sel), __byte_perm(c, d, sel), 0x5410);
+}
+// digit plane I (0..5) of sixteen packed digit sets z[0..15] -> the 16 bytes of a core-matrix row
+template <int I>
+__device__ __forceinline__ int4 i8_plane16(const unsigned long long (&z)[16])
+{
+    uint32_t w[4];
 #pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        const int di = (int)((X + 128) & 255) - 128;
-        d[i] = (int8_t)di;
-        X = (X - di) >> 8;
+    for (int g = 0; g < 4; ++g) {
+        if (I < 4)
+            w[g] = i8_pick4<(I & 3)>((uint32_t)z[4 * g], (uint32_t)z[4 * g + 1], (uint32_t)z[4 * g + 2], (uint32_t)z[4 * g + 3]);
+        else
+            w[g] = i8_pick4<(I & 3)>((uint32_t)(z[4 * g] >> 32), (uint32_t)(z[4 * g + 1] >> 32), (uint32_t)(z[4 * g + 2] >> 32),
+                                     (uint32_t)(z[4 * g + 3] >> 32));
     }
+    return make_int4((int)w[0], (int)w[1], (int)w[2], (int)w[3]);
 }
 
 // byte offset of element (row, k) of digit 0 in the tiling [row tile][k chunk][digit][row group][k group][8][16];
@@ -78,7 +98,7 @@ k_qphase_i8(const double* __restrict__ q, const double* __restrict__ Rrow, const
     double q0 = 0.0, q1 = 0.0, q2 = 0.0;
     const bool valid = iq < nq;
     if (valid) { q0 = q[3 * (size_t)iq]; q1 = q[3 * (size_t)iq + 1]; q2 = q[3 * (size_t)iq + 2]; }
-    int8_t dc[6][16], ds[6][16];
+    unsigned long long zc[16], zs[16];
 #pragma unroll
     for (int u = 0; u < 16; ++u) {
         const int r = r0 + u;
@@ -89,22 +109,17 @@ k_qphase_i8(const double* __restrict__ q, const double* __restrict__ Rrow, const
             sincospi(2.0 * x, &sn, &cs);
             vc = wrow[r] * cs; vs = (r < K2) ? wrow[r] * sgn * sn : 0.0;
         }
-        int8_t d[6];
-        i8_digits(vc, inv_scaleA, d);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) dc[i][u] = d[i];
-        i8_digits(vs, inv_scaleA, d);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) ds[i][u] = d[i];
+        zc[u] = i8_digits_packed(vc, inv_scaleA);
+        zs[u] = i8_digits_packed(vs, inv_scaleA);
     }
     const size_t oc = i8_tiled_off(iq, r0, I8Cfg::BM, nchunks);
     const bool has_sin = r0 < K2;                          // the sine group of these 16 rows exists
     const size_t os = has_sin ? i8_tiled_off(iq, Kc16 + r0, I8Cfg::BM, nchunks) : 0;
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        *reinterpret_cast<int4*>(Ai8 + (size_t)i * I8Cfg::A_PLANE + oc) = *reinterpret_cast<const int4*>(dc[i]);
-        if (has_sin) *reinterpret_cast<int4*>(Ai8 + (size_t)i * I8Cfg::A_PLANE + os) = *reinterpret_cast<const int4*>(ds[i]);
-    }
+#define PE_I8_STORE_PLANE(I)                                                                                     \
+    *reinterpret_cast<int4*>(Ai8 + (size_t)(I) * I8Cfg::A_PLANE + oc) = i8_plane16<I>(zc);                       \
+    if (has_sin) *reinterpret_cast<int4*>(Ai8 + (size_t)(I) * I8Cfg::A_PLANE + os) = i8_plane16<I>(zs);
+    PE_I8_STORE_PLANE(0) PE_I8_STORE_PLANE(1) PE_I8_STORE_PLANE(2) PE_I8_STORE_PLANE(3) PE_I8_STORE_PLANE(4) PE_I8_STORE_PLANE(5)
+#undef PE_I8_STORE_PLANE
 }
 
 // column maxima of B': cmax[slot][n] = max_r |pair row r of column n| (re or im), as the bit pattern of the non-negative
@@ -157,7 +172,7 @@ k_pack_i8(const double2* __restrict__ g1, long long ld, long long strideS, int N
     const double inv = colok ? 1.0 / scale : 0.0;
     if (colok && c == 0 && blockIdx.y == 0) sb[(size_t)slot * ldsb + n] = scale;      // the GEMM epilogue's column scale
     const double2* s = g1 + (size_t)slot * strideS + (colok ? n : 0);
-    int8_t dd[6][16];
+    unsigned long long z[16];
 #pragma unroll
     for (int u = 0; u < 16; ++u) {
         const int r = r0 + u;
@@ -169,15 +184,15 @@ k_pack_i8(const double2* __restrict__ g1, long long ld, long long strideS, int N
             if (kind[r] == 0) v = c ? a.y + b.y : a.x + b.x;            // a + b
             else v = c ? a.x - b.x : -(a.y - b.y);                      // i (a - b)
         }
-        int8_t d[6];
-        i8_digits(v, inv, d);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) dd[i][u] = d[i];
+        z[u] = i8_digits_packed(v, inv);
     }
-    const size_t o = i8_tiled_off(np, r0, I8Cfg::BN, Kpad / I8Cfg::KC);
-#pragma unroll
-    for (int i = 0; i < 6; ++i)
-        *reinterpret_cast<int4*>(Bi8 + (size_t)slot * slot_bytes + (size_t)i * I8Cfg::B_PLANE + o) = *reinterpret_cast<const int4*>(dd[i]);
+    int8_t* dst = Bi8 + (size_t)slot * slot_bytes + i8_tiled_off(np, r0, I8Cfg::BN, Kpad / I8Cfg::KC);
+    *reinterpret_cast<int4*>(dst + 0 * (size_t)I8Cfg::B_PLANE) = i8_plane16<0>(z);
+    *reinterpret_cast<int4*>(dst + 1 * (size_t)I8Cfg::B_PLANE) = i8_plane16<1>(z);
+    *reinterpret_cast<int4*>(dst + 2 * (size_t)I8Cfg::B_PLANE) = i8_plane16<2>(z);
+    *reinterpret_cast<int4*>(dst + 3 * (size_t)I8Cfg::B_PLANE) = i8_plane16<3>(z);
+    *reinterpret_cast<int4*>(dst + 4 * (size_t)I8Cfg::B_PLANE) = i8_plane16<4>(z);
+    *reinterpret_cast<int4*>(dst + 5 * (size_t)I8Cfg::B_PLANE) = i8_plane16<5>(z);
 }
 
 // ---- tcgen05 helpers (PTX ISA: tcgen05.*, sm_100a) -------------------------------------------------------------------
