@@ -350,7 +350,11 @@ int launch_setk_rotate(phoebe_elph_ctx* c, const double2* T, int S, const double
     const phoebe_elph_dims& d = c->dims;
     const int Y = d.nw * d.nmodes, N = nb1 * Y;
     LaunchScope ls(c, PHOEBE_ELPH_K_SETK_ROTATE);
-    const int TR = 128;
+    // threads per block over y: the largest of 128 / 64 / 32 that leaves the fewest idle threads in the last block
+    // (Y = 192 -> 64: three full blocks instead of one and a half; Y = 48 -> 64 instead of 128)
+    int TR = 128;
+    for (int t : {64, 32})
+        if (ceil_div(Y, t) * t < ceil_div(Y, TR) * TR) TR = t;
     if (nb1 <= 4) {
         const int ng = ceil_div(nb1, 4);
         dim3 grid(ceil_div(Y, TR), d.nRp, ng * nk);
