@@ -793,6 +793,10 @@ def run_ours(args):
             "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": _with_multi(_with_kbatch(_config_dict(w, world, args.scaling, args.pool), kb), multi),
             "clocks": clocks,
+            # inputs, outputs and every step but a4 are FP64; a4 (default path) = exact s8 digit products with s32 accumulation
+            # that reproduce the FP64 contraction to 3-5e-13 of max |g|^2 (tests/test_gpu_i8.py; --tune i8=0: FP64 DMMA)
+            "arithmetic": {"a1_a2_a3_a5_a6_a7": "f64", "a4": "s8 x s8 -> s32 digit products of 48-bit operands (exact), f64 epilogue"
+                           if i8_on else "f64"},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "steps": e2e_steps, "api": "q_batch_host" if args.e2e_sync else
                     ("set_k_batch_host + q_batch_multi_host_async + wait" if multi else "q_batch_host_async + wait")},
