@@ -6,9 +6,10 @@
 // whole phase matrix, |A| <= max weight; B': one scale per complex column n = twice the column's largest magnitude) and
 // split into SIX balanced base-256 digits d_i in [-128, 127]:   x = scale * sum_i d_i 256^i / 2^47.
 // Then  A B' = sA sB 2^-94 sum_{i,j} 256^(i+j) (A_i B'_j)  with A_i B'_j an INT8 x INT8 GEMM whose INT32 accumulation is
-// EXACT (|sum| <= 6 * 736 * 128^2 < 2^27).  The 21 digit pairs with i + j >= 5 are kept, summed per level l = i + j - 5 in
-// six TMEM accumulators; the dropped pairs are below 2^-45 of scale_A * scale_B per term -- a NORMWISE error of ~1e-13 of
-// the column scale, inside the 1e-10 parity bar with two orders of magnitude to spare.  The levels
+// EXACT (|sum| <= 6 pairs * rows * 128^2 < 2^31 for up to 16384 rows).  The 21 digit pairs with i + j >= 5 are kept, summed
+// per level l = i + j - 5 in six TMEM accumulators; the dropped pairs are below 5 * 2^-48 of scale_A * scale_B per term -- a
+// NORMWISE error, measured 3-5e-13 of max |g|^2 against the oracle, inside the 1e-10 parity bar with two orders of magnitude
+// to spare.  The levels
 // are recombined exactly in 64-bit integers (two halves) and rounded once, in the FP64 epilogue that writes C in the
 // layout the rotation kernel reads.
 //
@@ -34,7 +35,7 @@ struct I8Cfg {
     // 512 x 112 + 128 x 32 = 61440.
     static constexpr int kThreads = (EPI_WARPS + 4) * 32, PW = EPI_WARPS, REGS_EPI = 112, REGS_CTRL = 32;
     static constexpr int A_PLANE = BM * KC, B_PLANE = BN * KC;                    // bytes of one digit plane of a stage
-    static constexpr int STAGE_BYTES = ND * (A_PLANE + B_PLANE);                 // 72 KB
+    static constexpr int STAGE_BYTES = ND * (A_PLANE + B_PLANE);                 // 36 KB (KC = 32): six stages
     static constexpr size_t kSmemBytes = (size_t)STAGES * STAGE_BYTES + 1024 + 256;   // + alignment slack + barriers
     static constexpr int TMEM_COLS = 512;                                        // NLEV * BN = 384 used
 };
