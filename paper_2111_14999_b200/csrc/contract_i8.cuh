@@ -20,6 +20,8 @@
 //   B digits  Bi8[slot][n' tile of 64][k chunk KC][d][col group 8][k group KC/16][8 cols][16 bytes]  (k_pack_i8)
 // Kernel: warps 0..15 = epilogue (TMEM -> registers -> C), warp 16 = TMA producer, warp 17 = MMA issuer (one thread).
 #pragma once
+#include <math_constants.h>
+
 #include "ptx_helpers.cuh"
 
 namespace pe {
@@ -142,6 +144,7 @@ k_i8_colmax(const double2* __restrict__ g1, long long ld, long long strideS, int
         const double2 b = ib >= 0 ? s[(size_t)ib * ld] : make_double2(0.0, 0.0);
         const double x = kind[r] == 0 ? a.x + b.x : a.y - b.y, y = kind[r] == 0 ? a.y + b.y : a.x - b.x;
         m = fmax(m, fmax(fabs(x), fabs(y)));
+        if (!(isfinite(x) && isfinite(y))) m = CUDART_INF;        // NaN / Inf in g1': the whole column becomes NaN (as in FP64)
     }
     if (m > 0.0) atomicMax(cmax + (size_t)slot * ldsb + n, (unsigned long long)__double_as_longlong(m));
 }
@@ -151,6 +154,7 @@ __device__ __forceinline__ double i8_scale_of(unsigned long long mbits)
 {
     const double m = __longlong_as_double((long long)mbits);
     if (!(m > 0.0)) return 1.0;
+    if (isinf(m)) return m;          // a non-finite column: digits 0 (1 / inf), result 0 * inf = NaN
     int e = 0;
     frexp(m, &e);
     return ldexp(1.0, e + 1);

@@ -170,3 +170,21 @@ def test_i8_stacked_multi_k_and_fallback(env):
             ref = oracle.elph(gW_np, wl.Re_vectors(w), wl.Rp_vectors(w), None, None, wl.k_points(w)[i], Uks[i],
                               st[0][i], st[1][i], st[2][i], st[3][i])
             assert _relerr(multi[i], ref) <= TOL
+
+
+def test_i8_non_finite_input_becomes_nan(env):
+    """A NaN in g_W must not come out as a finite number.  It reaches one column (w2, kappa) of g1' for every b1 (0 * NaN in the
+    U_k rotation), the column-maximum pass flags that column, the contraction returns NaN there, and the two rotations spread it
+    over every |g|^2 -- on the INT8 path exactly as on the FP64 one."""
+    wl, harness = env["wl"], env["harness"]
+    w = wl.custom(nw=4, nb1=3, nb2=4, nm=3, grid_e=(2, 2, 1), grid_p=(3, 3, 3), nq=140, cfg_id=176)
+    a = _inputs(wl, w)
+    gW = a["gW"].copy()
+    gW[5, 1, 1, 2, 0] = np.nan                 # [p][e][w1][w2][kappa]
+    for i8 in (1, 0):
+        ctx = _ctx(env, w, gW, 140, i8)
+        ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+        out = ctx.q_batch(*harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])).cpu().numpy()
+        assert ctx.get_tuning("i8") == i8
+        ctx.close()
+        assert np.all(np.isnan(out))
