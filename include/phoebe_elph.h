@@ -332,7 +332,8 @@ int phoebe_elph_profile_read(phoebe_elph_ctx* ctx, double* ms, int64_t* launches
  *               bit-reproducible.  Taken whenever the pair form is and (stacked forms) the rows per k-point are a multiple
  *               of 128; 0 = the FP64 tensor-core pair kernel.  get_tuning("i8") = 1 if the LAST contraction ran on INT8.
  *               Domain: column maxima of g1' within ~[1e-290, 1e290]; a NaN / Inf in g1' turns its whole column of the
- *               contraction (hence every |g|^2 that column enters) into NaN, as FP64 arithmetic would.
+ *               contraction (hence every |g|^2 that column enters) into NaN, as FP64 arithmetic would.  The q-points must be
+ *               finite (a NaN wavevector gives undefined phase digits, not NaN).
  *               "i8_cluster" 0 | 1 (default) | 2 | 4 | 8 = CTAs per cluster of that kernel (the A digit planes multicast);
  *               get_tuning("i8_grid") = CTAs of the last launch (clusters of 8: 15 fit a B200 = 120 CTAs)
  *   "qfold"     1 = q lists that contain -q with q (uniform meshes; modulo a reciprocal lattice vector when all Rp are
