@@ -188,3 +188,21 @@ def test_i8_non_finite_input_becomes_nan(env):
         assert ctx.get_tuning("i8") == i8
         ctx.close()
         assert np.all(np.isnan(out))
+
+
+def test_i8_row_limit_falls_back_to_fp64(env):
+    """Exact INT32 accumulation holds for up to 16384 pair rows (6 digit pairs x rows x 128^2 < 2^31): a longer lattice-vector
+    list takes the FP64 pair kernel, one just below the limit stays on the INT8 path (128 chunks per tile through a 6-stage ring)."""
+    wl, oracle, harness = env["wl"], env["oracle"], env["harness"]
+    for grid_p, expect_i8 in (((27, 27, 23), 0), ((25, 25, 25), 1)):          # 16767 and 15625 vectors
+        w = wl.custom(nw=2, nb1=2, nb2=2, nm=1, grid_e=(1, 1, 1), grid_p=grid_p, lam=40.0, nq=130, cfg_id=177)
+        a = _inputs(wl, w)
+        ref = oracle.elph(a["gW"], a["Re"], a["Rp"], None, None, a["k"], a["Uk"], a["q"], a["Ukq"], a["ev"], a["om"])
+        ctx = _ctx(env, w, a["gW"], 130, 1)
+        rows = ctx.get_tuning("pair_rows")
+        assert (rows > 16384) == (expect_i8 == 0)
+        ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+        out = ctx.q_batch(*harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])).cpu().numpy()
+        assert ctx.get_tuning("i8") == expect_i8
+        ctx.close()
+        assert _relerr(out, ref) <= TOL
