@@ -530,6 +530,19 @@ def run_ours(args):
             else:
                 kernels[kind].update(bound="alu", achieved=work / dur / 1e12, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s")
             kernels[kind]["frac"] = kernels[kind]["achieved"] / kernels[kind]["peak"]
+    # the small kernels of the step, against the HBM floor of their ALGORITHMIC bytes per step:
+    #   a2 k_setk_rotate: T read once (16 nRp X per k), g1' written (16 nRp N per k)
+    #   a3 phases: the A operand written once (INT8: 6 digit planes of Kr real rows per q; FP64 pair form: 8 Kr per q)
+    #   pack: g1' read once, the operand copy written (INT8: 6 planes x 2 real columns of Kr rows; FP64 pair rows: 16 Kr N)
+    nb1_l = w.nb1
+    small = {"setk_rotate": 16.0 * w.nRp * (w.X + nb1_l * w.nw * w.nm) * n_k,
+             "qphase": (6.0 if i8_on else 8.0) * max(pair_rows, 1) * nq_l * n_k if pair_rows else 16.0 * w.nRp * nq_l * n_k,
+             "pack": (16.0 * w.nRp * w.N + (12.0 if i8_on else 16.0) * max(pair_rows, 1) * w.N) * n_k if pair_rows else 0.0}
+    for kind, bytes_step in small.items():
+        if kind in kernels and bytes_step > 0 and "bound" not in kernels[kind]:
+            dur = kernels[kind]["ms_total"] * 1e-3
+            kernels[kind].update(bound="hbm", achieved=bytes_step / dur / 1e9, peak=hbm_peak, unit="GB/s",
+                                 frac=bytes_step / dur / 1e9 / hbm_peak, per="step (all launches of the kind)")
     dominant = max(kernels, key=lambda kk: kernels[kk]["ms_total"])
     dk = kernels[dominant]
     traffic = _ncu_traffic(w.name, dominant)
