@@ -8,7 +8,7 @@
 // Then  A B' = sA sB 2^-94 sum_{i,j} 256^(i+j) (A_i B'_j)  with A_i B'_j an INT8 x INT8 GEMM whose INT32 accumulation is
 // EXACT (|sum| <= 6 pairs * rows * 128^2 < 2^31 for up to 16384 rows).  The 21 digit pairs with i + j >= 5 are kept, summed
 // per level l = i + j - 5 in six TMEM accumulators; the dropped pairs are below 5 * 2^-48 of scale_A * scale_B per term -- a
-// NORMWISE error, measured 3-5e-13 of max |g|^2 against the oracle, inside the 1e-10 parity bar with two orders of magnitude
+// NORMWISE error, measured 3-5e-13 of max |g|^2 in the parity tests, inside the 1e-10 parity bar with two orders of magnitude
 // to spare.  The levels
 // are recombined exactly in 64-bit integers (two halves) and rounded once, in the FP64 epilogue that writes C in the
 // layout the rotation kernel reads.
