@@ -473,10 +473,14 @@ def run_ours(args):
     # ---- per-kernel durations (CUDA events inside the library, on its stream) ---
     ctx.profile(True)
     prof_steps = max(1, min(args.steps, 3))
+    ep0, ep1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ep0.record()
     for _ in range(prof_steps):
         step()
+    ep1.record()
     prof = ctx.profile_read()
     ctx.profile(False)
+    profiled_step_ms = ep0.elapsed_time(ep1) / prof_steps      # the same steps, end to end, with the per-kernel events in
     m3 = bool(ctx.get_tuning("m3"))
     pair_rows = ctx.get_tuning("pair_rows")     # > 0: a4 runs the +R / -R pair form (4 real flop per MAC)
     counts = harness.algorithmic_counts(w, nq=nq_l, m3=m3, pair_rows=pair_rows)
@@ -816,6 +820,8 @@ def run_ours(args):
             "gpu_launches": int(gpu_launches),
             "roofline": roofline,
             "kernels": kernels,
+            # sum of the kernels' own durations vs the step they were measured in (gaps between launches) vs the timed loop
+            "kernel_sum_ms": sum(v["ms_total"] for v in kernels.values()), "profiled_step_ms": profiled_step_ms,
             "fp64_probe": fp64_probe,
             "fp64_ceilings": ceilings,
             "three_call": three_call,
