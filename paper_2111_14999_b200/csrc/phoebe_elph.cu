@@ -668,7 +668,7 @@ int run_q_batch(phoebe_elph_ctx* c, int nq, int nb2, const double* q, const doub
                             (rows_per_k == 0 || rows_per_k % pe::I8Cfg::BM == 0) &&    // a row tile must not straddle two k slots
                             c->pair_Kr <= 16384;      // exact INT32 accumulation: 6 digit pairs x rows x 128^2 < 2^31
         c->last_i8 = use_i8 ? 1 : 0;
-        const int i8_Kpad = (int)align_up((size_t)c->pair_Kr, 64), i8_Npad2 = (int)align_up((size_t)2 * N, 64);
+        const int i8_Kpad = (int)align_up((size_t)c->pair_Kr, pe::I8Cfg::KC), i8_Npad2 = (int)align_up((size_t)2 * N, 64);
         int8_t* Ai8 = reinterpret_cast<int8_t*>(c->ws + c->L.off_Ai8);
         int8_t* Bi8 = reinterpret_cast<int8_t*>(c->ws + c->L.off_Bi8);
         double* sbv = reinterpret_cast<double*>(c->ws + c->L.off_sb);
