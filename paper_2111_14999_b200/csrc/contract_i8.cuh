@@ -214,6 +214,29 @@ __device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t d
                  "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}\n"
                  :: "r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(0u) : "memory");
 }
+// The same, executed by ALL lanes of the (converged) MMA warp with the instruction itself predicated on `leader`: inside an
+// `if (lane == 0)` branch ptxas cannot prove the descriptors warp-uniform and wraps every tcgen05.mma in an ELECT / R2UR
+// broadcast loop (~20 instructions per MMA).  Predicated in converged code, with the stage address made uniform by a shuffle,
+// the descriptors are computed in uniform registers.  (Measured: the kernel time did not change -- the issuing thread was
+// not the limit, it blocks on the tensor pipe's queue -- the lighter instruction stream is kept.)
+__device__ __forceinline__ void umma_i8_p(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate, uint32_t leader)
+{
+    asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %6, 0;\n\t"
+                 "@q tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}\n"
+                 :: "r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(0u), "r"(leader) : "memory");
+}
+__device__ __forceinline__ void umma_commit_p(uint64_t* bar, uint32_t leader)
+{
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t"
+                 "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}\n"
+                 :: "r"(smem_u32(bar)), "r"(leader) : "memory");
+}
+__device__ __forceinline__ void umma_commit_mc_p(uint64_t* bar, uint16_t cta_mask, uint32_t leader)
+{
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t"
+                 "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n\t}\n"
+                 :: "r"(smem_u32(bar)), "h"(cta_mask), "r"(leader) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint64_t* bar)      // arrives on bar when all MMAs issued so far have completed
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(bar)) : "memory");
@@ -327,7 +350,7 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
             }
         }
     } else if (warp == Cfg::PW + 1) {
-        // ================= MMA issuer (one thread) =================
+        // ================= MMA issuer (one elected lane; the warp stays converged) =================
         // Digit plane A_i meets the B' planes j = 5 - i .. 5, whose products belong to the levels 0 .. i: the planes are
         // contiguous in the stage and the level accumulators contiguous in TMEM, so ONE instruction with N = 64 (i + 1)
         // does all of them and reads the A tile from shared memory once (the unit's limit is N <= 256: i = 4 and 5 take two).
@@ -337,14 +360,18 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
         // instruction descriptor: D = S32, A = B = signed 8 bit, both K-major, M = 128, N in bits 17..22
         constexpr uint32_t idesc0 = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BM >> 4) << 24);
         int s = 0; uint32_t ph = 0, tph = 0;
+        const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);
         for (int g = g0; g < ngroups; g += gstep) {
             mbar_wait(tempty, tph ^ 1u);                 // the epilogue has read the previous tile's accumulators
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             for (int c = 0; c < nchunks; ++c) {
                 mbar_wait(full + s, ph);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                if (lane == 0) {
-                    const uint32_t a0 = smem_u32(smem + (size_t)s * Cfg::STAGE_BYTES), b0 = a0 + ND * Cfg::A_PLANE;
+                {
+                    const uint32_t leader = lane == 0 ? 1u : 0u;
+                    // (a shuffle from lane 0 tells the compiler the address is warp-uniform: the descriptor arithmetic then runs
+                    //  in uniform registers)
+                    const uint32_t a0 = __shfl_sync(0xffffffffu, smem_u32(smem + (size_t)s * Cfg::STAGE_BYTES), 0), b0 = a0 + ND * Cfg::A_PLANE;
 #pragma unroll
                     for (int ks = 0; ks < KC / 32; ++ks) {
                         const uint32_t acc = (c == 0 && ks == 0) ? 0u : 1u;
@@ -356,16 +383,16 @@ k_contract_i8(const int8_t* __restrict__ Ai8, const int8_t* __restrict__ Bi8, si
                             // more than four levels exceed N = 256: split 3 + rest (N = 192 + 128 / 192 runs faster than 256 + 64 / 128:
                             // a narrow instruction is bound by its shared-memory reads of the A tile)
                             const int n1 = nlev > 4 ? 3 : nlev;
-                            umma_i8(tmem, da, umma_desc(b0 + j0 * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
-                                    idesc0 | ((uint32_t)((n1 * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
+                            umma_i8_p(tmem_u, da, umma_desc(b0 + j0 * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
+                                      idesc0 | ((uint32_t)((n1 * BN) >> 3) << 17), i == ND - 1 ? acc : 1u, leader);
                             if (nlev > 4)
-                                umma_i8(tmem + 3u * BN, da, umma_desc(b0 + (j0 + 3) * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
-                                        idesc0 | ((uint32_t)(((nlev - 3) * BN) >> 3) << 17), i == ND - 1 ? acc : 1u);
+                                umma_i8_p(tmem_u + 3u * BN, da, umma_desc(b0 + (j0 + 3) * Cfg::B_PLANE + ks * 256, 128, (KC / 16) * 128),
+                                          idesc0 | ((uint32_t)(((nlev - 3) * BN) >> 3) << 17), i == ND - 1 ? acc : 1u, leader);
                         }
                     }
                     // frees the stage (in every CTA of the cluster) when these MMAs have read it
-                    if (CL == 1) umma_commit(empty + s); else umma_commit_mc(empty + s, kMask);
-                    if (c == nchunks - 1) umma_commit(tfull);
+                    if (CL == 1) umma_commit_p(empty + s, leader); else umma_commit_mc_p(empty + s, kMask, leader);
+                    if (c == nchunks - 1) umma_commit_p(tfull, leader);
                 }
                 __syncwarp();
                 if (++s == ST) { s = 0; ph ^= 1u; }
