@@ -206,3 +206,25 @@ def test_i8_row_limit_falls_back_to_fp64(env):
         assert ctx.get_tuning("i8") == expect_i8
         ctx.close()
         assert _relerr(out, ref) <= TOL
+
+
+def test_i8_bits_do_not_depend_on_the_batching(env):
+    """Integer accumulation has no rounding order: the same q-points give the same bits whether they are contracted in one
+    launch, in sub-batches of 128 (tuning nq_sub), as a prefix of the list, or in another position of a longer list."""
+    wl, harness = env["wl"], env["harness"]
+    w = wl.custom(nw=5, nb1=4, nb2=5, nm=6, grid_e=(2, 2, 1), grid_p=(3, 3, 3), nq=700, cfg_id=178)
+    a = _inputs(wl, w)
+    ctx = _ctx(env, w, a["gW"], 700, 1)
+    ctx.set_k(a["k"], harness.to_device([a["Uk"]])[0])
+    d = harness.to_device([a["q"], a["Ukq"], a["ev"], a["om"]])
+    whole = ctx.q_batch(*d).cpu().numpy()
+    ctx.set_tuning("nq_sub", 128)
+    split = ctx.q_batch(*d).cpu().numpy()
+    assert ctx.launch_counts()["contract"] == 1 + 6
+    ctx.set_tuning("nq_sub", 1 << 20)
+    prefix = ctx.q_batch(*[t[:300].contiguous() for t in d]).cpu().numpy()
+    shifted = ctx.q_batch(*[t[211:].contiguous() for t in d]).cpu().numpy()
+    ctx.close()
+    assert np.array_equal(whole, split)
+    assert np.array_equal(whole[:300], prefix)
+    assert np.array_equal(whole[211:], shifted)
